@@ -1,0 +1,353 @@
+// api.cu -- the C ABI of include/ddhf.h: handle, constant tables, workspace layout, the
+// per-window launch sequence and the host-buffer (end-to-end) variant.
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <string>
+#include <vector>
+
+#include "ddhf_internal.cuh"
+
+namespace ddhf {
+int fma_probe(float ms_target, float *tflops, cudaStream_t st);
+}
+
+using namespace ddhf;
+
+struct ddhf_handle {
+    ddhf_config cfg;
+    int np = 0;
+    int sm_count = 0;
+    int n_tiles = 0;
+    int comp_cap = 0;
+    int launches = 0;
+    ScoreParams sp{};
+    uint64_t g_f0 = 0, g_d = 0, g_h = 0;
+    CandTable *d_cand = nullptr;
+    // workspace offsets (bytes)
+    size_t off_cnt = 0, off_pairs = 0, off_work = 0, off_tiles = 0, off_class = 0, off_cursor = 0,
+           off_parent = 0, off_slot = 0, off_comp = 0, off_comp_label = 0, off_ctiles = 0, ws_bytes = 0;
+    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    bool timed_once = false;
+    // buffers of the host-buffer variant
+    ddhf_event *hb_events = nullptr;
+    void *hb_ws = nullptr;
+    ddhf_outputs hb_out{};
+    bool hb_ready = false;
+    std::string err;
+};
+
+static std::string g_create_err;
+
+static int fail(ddhf_handle *h, int code, const std::string &msg)
+{
+    if (h) h->err = msg; else g_create_err = msg;
+    return code;
+}
+
+static size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+
+static uint64_t freq_const(double f_hz)
+{
+    // round(2^64 * f * 1e-6): phase in turns of f at integer microsecond t is hi32(G * t)
+    const long double x = static_cast<long double>(f_hz) / 1.0e6L;
+    return static_cast<uint64_t>(llroundl(ldexpl(x, 64)));
+}
+
+extern "C" const char *ddhf_version(void) { return "ddhf-b200 0.1 (sm_100a)"; }
+
+extern "C" const char *ddhf_last_error(const ddhf_handle *h)
+{
+    return h ? h->err.c_str() : g_create_err.c_str();
+}
+
+extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
+{
+    if (out) *out = nullptr;
+    if (!cfg || !out) return fail(nullptr, DDHF_E_INVAL, "ddhf_create: NULL argument");
+    const ddhf_config &c = *cfg;
+    const long long np = static_cast<long long>(c.width) * c.height;
+    if (c.width < 1 || c.height < 1 || c.width > 65535 || c.height > 65535 || np > (4ll << 20))
+        return fail(nullptr, DDHF_E_INVAL, "ddhf_create: sensor size out of range (<= 4 Mi pixels)");
+    if (c.n_freq < 8 || c.n_freq > 2048)
+        return fail(nullptr, DDHF_E_INVAL, "ddhf_create: n_freq must be in [8, 2048]");
+    if (!(c.df_hz > 0) || !(c.f_min_hz >= 0) || c.f_min_hz + (c.n_freq + 64) * c.df_hz >= 4.0e5)
+        return fail(nullptr, DDHF_E_INVAL, "ddhf_create: frequency grid out of range (0 <= f < 400 kHz)");
+    if (c.n_f0 < 1 || c.n_f0 > kMaxF0 || c.n_harm < 1 || c.n_harm > kMaxHarm || c.half_bw_bins < 0 ||
+        c.h_min < 1 || !(c.f0_step_hz >= 0) || !(c.f0_min_hz > 0))
+        return fail(nullptr, DDHF_E_INVAL, "ddhf_create: comb parameters out of range");
+    if (c.k_lo < 0 || c.k_lo >= c.n_freq || !(c.sf_eps > 0))
+        return fail(nullptr, DDHF_E_INVAL, "ddhf_create: k_lo / sf_eps out of range");
+    if (c.max_events < 1 || c.max_events >= (1ll << 31) || c.max_active < 1 || c.max_boxes < 1)
+        return fail(nullptr, DDHF_E_INVAL, "ddhf_create: capacities out of range");
+
+    ddhf_handle *h = new (std::nothrow) ddhf_handle();
+    if (!h) return fail(nullptr, DDHF_E_NOMEM, "ddhf_create: out of host memory");
+    h->cfg = c;
+    h->np = static_cast<int>(np);
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        delete h;
+        return fail(nullptr, DDHF_E_CUDA, "ddhf_create: no CUDA device");
+    }
+
+    // ---- comb tables (R7-R10): harmonic centres, validity prefix, union intervals, rank ----
+    std::vector<CandTable> tab(c.n_f0);
+    const int nb = c.n_freq - c.k_lo, d = c.half_bw_bins;
+    int r0 = 1 << 30, r1 = -1;
+    for (int ci = 0; ci < c.n_f0; ++ci) {
+        CandTable &t = tab[ci];
+        memset(&t, 0, sizeof(t));
+        const double f0 = c.f0_min_hz + ci * c.f0_step_hz;
+        int mv = 0;
+        for (int m = 1; m <= c.n_harm; ++m) {
+            const long long km = static_cast<long long>(floor((m * f0 - c.f_min_hz) / c.df_hz + 0.5));
+            if (km - d < c.k_lo || km + d > c.n_freq - 1) break;
+            t.kc[m - 1] = static_cast<int16_t>(km);
+            mv = m;
+        }
+        if (mv < c.h_min) continue;
+        int ni = 0, n_excl = 0;
+        for (int m = 0; m < mv; ++m) {
+            const int lo = t.kc[m] - d, hi = t.kc[m] + d;
+            if (ni > 0 && lo <= t.hi[ni - 1]) {
+                if (hi > t.hi[ni - 1]) { n_excl += hi - t.hi[ni - 1]; t.hi[ni - 1] = static_cast<int16_t>(hi); }
+            } else {
+                t.lo[ni] = static_cast<int16_t>(lo);
+                t.hi[ni] = static_cast<int16_t>(hi);
+                n_excl += hi - lo + 1;
+                ++ni;
+            }
+        }
+        const int n_comp = nb - n_excl;
+        if (n_comp <= 0) continue;
+        t.m_valid = static_cast<int16_t>(mv);
+        t.n_int = static_cast<int16_t>(ni);
+        t.n_excl = static_cast<int16_t>(n_excl);
+        t.rank = static_cast<int16_t>((n_comp - 1) / 2);
+        r0 = t.rank < r0 ? t.rank : r0;
+        r1 = t.rank + n_excl > r1 ? t.rank + n_excl : r1;
+    }
+    if (r1 < 0) { r0 = 0; r1 = 0; }
+    if (ndft_band_size(c.n_freq, r0, r1) == 0) {
+        delete h;
+        return fail(nullptr, DDHF_E_INVAL,
+                    "ddhf_create: harmonic windows exclude too many bins for the band sorter "
+                    "(n_harm * (2 half_bw_bins + 1) too large for n_freq)");
+    }
+    if (cudaMalloc(&h->d_cand, sizeof(CandTable) * c.n_f0) != cudaSuccess ||
+        cudaMemcpy(h->d_cand, tab.data(), sizeof(CandTable) * c.n_f0, cudaMemcpyHostToDevice) != cudaSuccess) {
+        const std::string msg = std::string("ddhf_create: ") + cudaGetErrorString(cudaGetLastError());
+        if (h->d_cand) cudaFree(h->d_cand);
+        delete h;
+        return fail(nullptr, DDHF_E_CUDA, msg);
+    }
+    h->sp.n_freq = c.n_freq; h->sp.k_lo = c.k_lo; h->sp.n_f0 = c.n_f0; h->sp.half_bw = d;
+    h->sp.r0 = r0; h->sp.r1 = r1;
+    h->sp.tau_sf = c.tau_sf; h->sp.tau_comb = c.tau_comb; h->sp.sf_eps = c.sf_eps;
+    h->sp.score_all = (c.flags & DDHF_FLAG_SCORE_ALL) ? 1 : 0;
+    h->sp.cand = h->d_cand;
+
+    // ---- fixed-point frequency constants of the factorised NDFT ------------------------------
+    const int tn = ndft_tn(c.n_freq);
+    h->g_h = freq_const(16.0 * c.df_hz);
+    h->g_d = freq_const(c.df_hz);
+    h->g_f0 = freq_const(c.f_min_hz + (32.0 * tn - 16.0) * c.df_hz);
+
+    // ---- workspace layout -----------------------------------------------------------------------
+    h->n_tiles = (h->np + kScanTile - 1) / kScanTile;
+    h->comp_cap = ((c.width + 1) / 2) * ((c.height + 1) / 2);     // most 8-connected components possible
+    size_t o = 0;
+    h->off_cnt = o;        o = align_up(o + sizeof(int32_t) * h->np);
+    h->off_pairs = o;      o = align_up(o + sizeof(uint64_t) * static_cast<size_t>(c.max_events));
+    h->off_work = o;       o = align_up(o + sizeof(WorkItem) * static_cast<size_t>(h->np));
+    h->off_tiles = o;      o = align_up(o + sizeof(int32_t) * 4 * 1024);
+    h->off_class = o;      o = align_up(o + sizeof(int32_t) * 2 * kNumClasses);
+    h->off_cursor = o;     o = align_up(o + 256);
+    h->off_parent = o;     o = align_up(o + sizeof(int32_t) * h->np);
+    h->off_slot = o;       o = align_up(o + sizeof(int32_t) * h->np);
+    h->off_comp = o;       o = align_up(o + sizeof(int32_t) * 5 * static_cast<size_t>(h->comp_cap));
+    h->off_comp_label = o; o = align_up(o + sizeof(int32_t) * static_cast<size_t>(h->comp_cap));
+    h->off_ctiles = o;     o = align_up(o + sizeof(int32_t) * 2 * 1024);
+    h->ws_bytes = o;
+
+    if (c.flags & DDHF_FLAG_TIMING)
+        for (int i = 0; i < 4; ++i) cudaEventCreate(&h->ev[i]);
+    *out = h;
+    return DDHF_OK;
+}
+
+extern "C" size_t ddhf_workspace_bytes(const ddhf_handle *h) { return h ? h->ws_bytes : 0; }
+
+extern "C" int ddhf_launches_per_window(const ddhf_handle *h) { return h ? h->launches : 0; }
+
+extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n, int64_t t0_us,
+                           int64_t window_us, void *d_workspace, const ddhf_outputs *out,
+                           void *cuda_stream)
+{
+    if (!h) return DDHF_E_INVAL;
+    if (!out || !d_workspace || (n > 0 && !d_events))
+        return fail(h, DDHF_E_INVAL, "ddhf_window: NULL argument");
+    if (!out->row_ptr || !out->csr_ev || !out->active_idx || !out->sf || !out->score || !out->f0_idx ||
+        !out->mask || !out->boxes || !out->counters)
+        return fail(h, DDHF_E_INVAL, "ddhf_window: a required output pointer is NULL");
+    if (n < 0 || window_us <= 0 || window_us >= (1ll << 31))
+        return fail(h, DDHF_E_INVAL, "ddhf_window: n or window_us out of range");
+    if (n > h->cfg.max_events) return fail(h, DDHF_E_CAPACITY, "ddhf_window: n > max_events");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    char *ws = static_cast<char *>(d_workspace);
+    const ddhf_config &c = h->cfg;
+    const bool timing = (c.flags & DDHF_FLAG_TIMING) != 0;
+
+    IngestParams ip{};
+    ip.events = d_events; ip.n = n; ip.t0 = t0_us; ip.t1 = t0_us + window_us;
+    ip.width = c.width; ip.height = c.height; ip.np = h->np;
+    ip.n_min = c.n_min; ip.max_active = c.max_active;
+    ip.cnt = reinterpret_cast<int32_t *>(ws + h->off_cnt);
+    ip.row_ptr = out->row_ptr; ip.csr_ev = out->csr_ev;
+    ip.pairs = reinterpret_cast<uint64_t *>(ws + h->off_pairs);
+    ip.active_idx = out->active_idx;
+    ip.work = reinterpret_cast<WorkItem *>(ws + h->off_work);
+    int32_t *tiles = reinterpret_cast<int32_t *>(ws + h->off_tiles);
+    ip.tile_sum = tiles; ip.tile_act = tiles + 1024; ip.tile_off = tiles + 2048; ip.tile_aoff = tiles + 3072;
+    ip.class_cnt = reinterpret_cast<int32_t *>(ws + h->off_class);
+    ip.class_cur = ip.class_cnt + kNumClasses;
+    ip.counters = out->counters;
+    ip.sf = out->sf; ip.score = out->score; ip.f0_idx = out->f0_idx; ip.mask = out->mask;
+    ip.work_cursor = reinterpret_cast<int32_t *>(ws + h->off_cursor);
+
+    NdftParams np{};
+    np.work = ip.work; np.csr_ev = out->csr_ev; np.counters = out->counters;
+    np.work_cursor = ip.work_cursor; np.max_active = c.max_active;
+    np.g_f0 = h->g_f0; np.g_d = h->g_d; np.g_h = h->g_h;
+    np.power = out->power; np.sf = out->sf; np.score = out->score; np.f0_idx = out->f0_idx;
+    np.mask = out->mask; np.comb_debug = out->comb_debug;
+    np.n_scored = out->counters + DDHF_CNT_N_SCORED;
+    np.sp = h->sp;
+
+    CclParams cp{};
+    cp.mask = out->mask; cp.width = c.width; cp.height = c.height; cp.np = h->np;
+    cp.a_min = c.a_min; cp.max_boxes = c.max_boxes;
+    cp.parent = out->labels ? out->labels : reinterpret_cast<int32_t *>(ws + h->off_parent);
+    cp.slot = reinterpret_cast<int32_t *>(ws + h->off_slot);
+    int32_t *ct = reinterpret_cast<int32_t *>(ws + h->off_ctiles);
+    cp.tile_sum = ct; cp.tile_off = ct + 1024;
+    cp.comp = reinterpret_cast<int32_t *>(ws + h->off_comp);
+    cp.comp_cap = h->comp_cap;
+    cp.comp_label = reinterpret_cast<int32_t *>(ws + h->off_comp_label);
+    cp.boxes = out->boxes; cp.counters = out->counters;
+
+    int launches = 0;
+    if (timing) cudaEventRecord(h->ev[0], st);
+    launches += launch_ingest(ip, st);
+    if (timing) cudaEventRecord(h->ev[1], st);
+    launches += launch_ndft(np, c.n_freq, h->sm_count, st);
+    if (timing) cudaEventRecord(h->ev[2], st);
+    launches += launch_ccl(cp, st);
+    if (timing) { cudaEventRecord(h->ev[3], st); h->timed_once = true; }
+    h->launches = launches;
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return fail(h, DDHF_E_CUDA, std::string("ddhf_window: ") + cudaGetErrorString(e));
+    return DDHF_OK;
+}
+
+extern "C" int ddhf_stage_ms(ddhf_handle *h, float *ms)
+{
+    if (!h || !ms) return DDHF_E_INVAL;
+    if (!(h->cfg.flags & DDHF_FLAG_TIMING) || !h->timed_once)
+        return fail(h, DDHF_E_INVAL, "ddhf_stage_ms: handle was not created with DDHF_FLAG_TIMING or no window ran");
+    if (cudaEventSynchronize(h->ev[3]) != cudaSuccess)
+        return fail(h, DDHF_E_CUDA, std::string("ddhf_stage_ms: ") + cudaGetErrorString(cudaGetLastError()));
+    cudaEventElapsedTime(&ms[0], h->ev[0], h->ev[1]);
+    cudaEventElapsedTime(&ms[1], h->ev[1], h->ev[2]);
+    cudaEventElapsedTime(&ms[2], h->ev[2], h->ev[3]);
+    cudaEventElapsedTime(&ms[3], h->ev[0], h->ev[3]);
+    return DDHF_OK;
+}
+
+#define HB_CHECK(call)                                                                         \
+    do {                                                                                       \
+        const cudaError_t e_ = (call);                                                         \
+        if (e_ != cudaSuccess)                                                                 \
+            return fail(h, DDHF_E_CUDA, std::string("ddhf_window_host: ") + cudaGetErrorString(e_)); \
+    } while (0)
+
+extern "C" int ddhf_window_host(ddhf_handle *h, const ddhf_event *h_events, int64_t n, int64_t t0_us,
+                                int64_t window_us, const ddhf_host_outputs *out, void *cuda_stream)
+{
+    if (!h) return DDHF_E_INVAL;
+    if (!out || (n > 0 && !h_events)) return fail(h, DDHF_E_INVAL, "ddhf_window_host: NULL argument");
+    if (n > h->cfg.max_events) return fail(h, DDHF_E_CAPACITY, "ddhf_window_host: n > max_events");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const ddhf_config &c = h->cfg;
+    const size_t np = h->np;
+    if (!h->hb_ready) {
+        HB_CHECK(cudaMalloc(&h->hb_events, sizeof(ddhf_event) * static_cast<size_t>(c.max_events)));
+        HB_CHECK(cudaMalloc(&h->hb_ws, h->ws_bytes));
+        HB_CHECK(cudaMalloc(&h->hb_out.row_ptr, sizeof(int32_t) * (np + 1)));
+        HB_CHECK(cudaMalloc(&h->hb_out.csr_ev, sizeof(uint32_t) * static_cast<size_t>(c.max_events)));
+        HB_CHECK(cudaMalloc(&h->hb_out.active_idx, sizeof(int32_t) * static_cast<size_t>(c.max_active)));
+        HB_CHECK(cudaMalloc(&h->hb_out.sf, sizeof(float) * np));
+        HB_CHECK(cudaMalloc(&h->hb_out.score, sizeof(float) * np));
+        HB_CHECK(cudaMalloc(&h->hb_out.f0_idx, sizeof(int32_t) * np));
+        HB_CHECK(cudaMalloc(&h->hb_out.mask, np));
+        HB_CHECK(cudaMalloc(&h->hb_out.labels, sizeof(int32_t) * np));
+        HB_CHECK(cudaMalloc(&h->hb_out.boxes, sizeof(ddhf_box) * static_cast<size_t>(c.max_boxes)));
+        HB_CHECK(cudaMalloc(&h->hb_out.counters, sizeof(int32_t) * DDHF_N_COUNTERS));
+        h->hb_out.power = nullptr;
+        h->hb_out.comb_debug = nullptr;
+        h->hb_ready = true;
+    }
+    if (out->power && !h->hb_out.power)
+        HB_CHECK(cudaMalloc(&h->hb_out.power, sizeof(float) * static_cast<size_t>(c.max_active) * c.n_freq));
+    ddhf_outputs dev = h->hb_out;
+    if (!out->power) dev.power = nullptr;
+
+    if (n > 0) HB_CHECK(cudaMemcpyAsync(h->hb_events, h_events, sizeof(ddhf_event) * static_cast<size_t>(n),
+                                        cudaMemcpyHostToDevice, st));
+    const int rc = ddhf_window(h, h->hb_events, n, t0_us, window_us, h->hb_ws, &dev, st);
+    if (rc != DDHF_OK) return rc;
+
+    int32_t cnt[DDHF_N_COUNTERS];
+    HB_CHECK(cudaMemcpyAsync(cnt, dev.counters, sizeof(cnt), cudaMemcpyDeviceToHost, st));
+    if (out->mask) HB_CHECK(cudaMemcpyAsync(out->mask, dev.mask, np, cudaMemcpyDeviceToHost, st));
+    if (out->sf) HB_CHECK(cudaMemcpyAsync(out->sf, dev.sf, sizeof(float) * np, cudaMemcpyDeviceToHost, st));
+    if (out->score) HB_CHECK(cudaMemcpyAsync(out->score, dev.score, sizeof(float) * np, cudaMemcpyDeviceToHost, st));
+    if (out->f0_idx) HB_CHECK(cudaMemcpyAsync(out->f0_idx, dev.f0_idx, sizeof(int32_t) * np, cudaMemcpyDeviceToHost, st));
+    if (out->labels) HB_CHECK(cudaMemcpyAsync(out->labels, dev.labels, sizeof(int32_t) * np, cudaMemcpyDeviceToHost, st));
+    if (out->row_ptr) HB_CHECK(cudaMemcpyAsync(out->row_ptr, dev.row_ptr, sizeof(int32_t) * (np + 1), cudaMemcpyDeviceToHost, st));
+    HB_CHECK(cudaStreamSynchronize(st));
+    const size_t n_in = static_cast<size_t>(cnt[DDHF_CNT_N_IN]);
+    const size_t n_act = static_cast<size_t>(cnt[DDHF_CNT_N_ACTIVE] < c.max_active ? cnt[DDHF_CNT_N_ACTIVE] : c.max_active);
+    const size_t n_box = static_cast<size_t>(cnt[DDHF_CNT_N_BOXES]);
+    if (out->counters) memcpy(out->counters, cnt, sizeof(cnt));
+    if (out->csr_ev && n_in) HB_CHECK(cudaMemcpyAsync(out->csr_ev, dev.csr_ev, sizeof(uint32_t) * n_in, cudaMemcpyDeviceToHost, st));
+    if (out->active_idx && n_act) HB_CHECK(cudaMemcpyAsync(out->active_idx, dev.active_idx, sizeof(int32_t) * n_act, cudaMemcpyDeviceToHost, st));
+    if (out->power && n_act) HB_CHECK(cudaMemcpyAsync(out->power, dev.power, sizeof(float) * n_act * c.n_freq, cudaMemcpyDeviceToHost, st));
+    if (out->boxes && n_box) HB_CHECK(cudaMemcpyAsync(out->boxes, dev.boxes, sizeof(ddhf_box) * n_box, cudaMemcpyDeviceToHost, st));
+    HB_CHECK(cudaStreamSynchronize(st));
+    return DDHF_OK;
+}
+
+extern "C" int ddhf_fma_peak_probe(float ms_target, float *tflops_out, void *cuda_stream)
+{
+    if (!tflops_out) return DDHF_E_INVAL;
+    return fma_probe(ms_target, tflops_out, static_cast<cudaStream_t>(cuda_stream));
+}
+
+extern "C" int ddhf_destroy(ddhf_handle *h)
+{
+    if (!h) return DDHF_OK;
+    if (h->d_cand) cudaFree(h->d_cand);
+    for (int i = 0; i < 4; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
+    if (h->hb_events) cudaFree(h->hb_events);
+    if (h->hb_ws) cudaFree(h->hb_ws);
+    void *bufs[] = {h->hb_out.row_ptr, h->hb_out.csr_ev, h->hb_out.active_idx, h->hb_out.power,
+                    h->hb_out.sf, h->hb_out.score, h->hb_out.f0_idx, h->hb_out.mask,
+                    h->hb_out.labels, h->hb_out.boxes, h->hb_out.counters};
+    for (void *b : bufs) if (b) cudaFree(b);
+    delete h;
+    return DDHF_OK;
+}

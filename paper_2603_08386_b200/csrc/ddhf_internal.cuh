@@ -1,0 +1,109 @@
+// ddhf_internal.cuh -- shared declarations of the DDHF CUDA kernel sets (sm_100a).
+// Product code: shares nothing with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/ddhf.h"
+
+namespace ddhf {
+
+constexpr int kMaxHarm = 16;       // n_harm limit
+constexpr int kMaxF0 = 256;        // n_f0 limit
+constexpr int kNumClasses = 12;    // work-list size classes (by log2 of the row length)
+constexpr int kScanTile = 4096;    // elements per scan tile (1024 threads x 4)
+
+// One unit of NDFT work: an active pixel's CSR row.
+struct __align__(16) WorkItem {
+    int32_t row_begin;   // first slot in csr_ev
+    int32_t n;           // events in the row
+    int32_t pix;         // linear pixel index
+    int32_t arow;        // row of the compact outputs (index into active_idx)
+};
+
+// Per-candidate comb tables, built on the host at create time (readings R7-R10).
+struct CandTable {
+    int16_t m_valid;             // valid harmonics (0 = candidate skipped)
+    int16_t n_int;               // disjoint intervals of the union of the windows
+    int16_t rank;                // 0-based rank of the lower median in the complement
+    int16_t n_excl;              // bins in the union
+    int16_t kc[kMaxHarm];        // centre bin of harmonic m (index m-1)
+    int16_t lo[kMaxHarm];        // union intervals, inclusive
+    int16_t hi[kMaxHarm];
+};
+
+struct ScoreParams {
+    int32_t n_freq, k_lo, n_f0, half_bw;
+    int32_t r0, r1;              // full-spectrum rank band that holds every complement median
+    float tau_sf, tau_comb, sf_eps;
+    int32_t score_all;
+    const CandTable *cand;       // DEVICE [n_f0]
+};
+
+struct NdftParams {
+    const WorkItem *work;        // DEVICE [n_active] ordered by descending size class
+    const uint32_t *csr_ev;
+    const int32_t *counters;     // n_active is read from here (device side)
+    int32_t *work_cursor;        // dynamic work queue head
+    int32_t max_active;
+    uint64_t g_f0, g_d, g_h;     // 2^64 * f * 1e-6 for: centre base, df, 16*df
+    float *power;                // optional compact spectra
+    float *sf, *score;
+    int32_t *f0_idx;
+    uint8_t *mask;
+    float *comb_debug;
+    int32_t *n_scored;
+    ScoreParams sp;
+};
+
+struct IngestParams {
+    const ddhf_event *events;
+    int64_t n;
+    int64_t t0, t1;              // window [t0, t1)
+    int32_t width, height, np;
+    int32_t n_min, max_active;
+    int32_t *cnt;                // [np] histogram, later reused as scatter cursor
+    int32_t *row_ptr;            // [np+1]
+    uint32_t *csr_ev;
+    uint64_t *pairs;             // [max_events] (input index << 32 | csr value), unsorted rows
+    int32_t *active_idx;
+    WorkItem *work;
+    int32_t *tile_sum, *tile_act;   // [n_tiles]
+    int32_t *tile_off, *tile_aoff;  // [n_tiles]
+    int32_t *class_cnt;             // [kNumClasses] counts, then bases
+    int32_t *class_cur;             // [kNumClasses] cursors
+    int32_t *counters;
+    float *sf, *score;           // per-pixel maps initialised for inactive pixels
+    int32_t *f0_idx;
+    uint8_t *mask;
+    int32_t *work_cursor;
+};
+
+struct CclParams {
+    const uint8_t *mask;
+    int32_t width, height, np;
+    int32_t a_min, max_boxes;
+    int32_t *parent;             // [np] = labels output or workspace
+    int32_t *slot;               // [np] root pixel -> component slot
+    int32_t *tile_sum, *tile_off;
+    int32_t *comp;               // [np/4+1][5] x0,y0,x1,y1,n per component slot (capped)
+    int32_t comp_cap;
+    int32_t *comp_label;         // [comp_cap]
+    int32_t *keep_off;           // [comp_cap] scan of the A_min filter
+    ddhf_box *boxes;
+    int32_t *counters;
+};
+
+// kernel-set entry points (host functions that enqueue on `st`); each returns the number
+// of kernels it launched
+int launch_ingest(const IngestParams &p, cudaStream_t st);
+int launch_ndft(const NdftParams &p, int n_freq, int sm_count, cudaStream_t st);
+int launch_ccl(const CclParams &p, cudaStream_t st);
+int ndft_bins_per_lane(int n_freq);          // 8, 16, 32 or 64
+int ndft_tn(int n_freq);                     // offset pairs per centre for that kernel
+size_t ndft_smem_bytes(int n_freq);
+int ndft_band_size(int n_freq, int r0, int r1);   // sort capacity needed, 0 if unsupported
+cudaError_t ndft_configure();                // opt in to large dynamic shared memory
+
+}  // namespace ddhf

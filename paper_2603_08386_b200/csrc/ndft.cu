@@ -1,0 +1,586 @@
+// ndft.cu -- a4-a7: per-pixel NDFT power spectrum with the scoring fused into its epilogue.
+//
+//   a4  X_j = sum_k w_k exp(-2 pi i f_j t_k),  P_j = |X_j|^2          (eq. 6)
+//   a5  SF = geometric mean / arithmetic mean of P                  (eq. 7)
+//   a6  SNR_M(w) = N(w) / median(P outside the harmonic windows)    (eq. 8-10)
+//   a7  mask = SF <= tau_sf and max_w SNR_M >= tau_comb              (L107, eq. 11)
+//
+// Design (B200, plain FP32 pipes -- the per-pixel Vandermonde has no operand shared between
+// pixels, so this is ALU work, not a tensor-core contraction):
+//
+// * One warp owns one pixel at a time and all of its bins; lane l holds the bins
+//   j = l + 32 i, i < NBL.  Warps pull pixels from a device-side queue ordered by
+//   descending row length, so the heavy tail (config 4) is spread over the grid.
+// * The direct sum is factorised exactly, not approximated: with the bins of a lane split
+//   into TM groups of 2 TN bins around a centre frequency, f_j = f_c +- (m + 1/2) 32 df and
+//       w e^{-i th_c} e^{-+i ph_m}
+//   needs only the four real products a_r b_r, a_r b_i, a_i b_r, a_i b_i of the centre
+//   phasor a (per lane, per event) and the offset phasor b (shared by all lanes, per event,
+//   read as a shared-memory broadcast).  Accumulating those four products costs 4 FMA for 2
+//   bins = 2 FMA per (pixel, bin, event) term, issued as packed FFMA2 (fma.rn.f32x2).  There
+//   is no recurrence along frequency or time, hence no drift to resync.
+// * Phases are exact 32-bit fixed point "turns": hi32(G * t) with G = 2^64 f 1e-6, so a
+//   5 kHz x 0.1 s = 500-cycle phase keeps 2^-32 turn resolution before it reaches the SFU.
+// * The spectrum never goes back to HBM for scoring: P stays in registers and in the warp's
+//   shared-memory slice; the optional compact spectrum output is a streaming store.
+// * The complement median of every candidate is an order statistic of the full spectrum
+//   in a narrow rank band [r0, r1] known at create time.  The band is isolated by a few
+//   counting passes over the register-resident spectrum, sorted once per pixel in registers
+//   (bitonic), and each candidate then only corrects the rank for its own excluded bins
+//   (prefix counts from warp ballots + a bitmask of excluded in-band positions).
+#include "ddhf_internal.cuh"
+
+namespace ddhf {
+
+namespace {
+
+constexpr int kWarps = 4;          // warps per CTA
+constexpr int kEC = 16;            // events per table chunk
+constexpr unsigned kFull = 0xffffffffu;
+constexpr uint32_t kInvalidKey = 0x7fffffffu;
+
+template <int TM, int TN, int BS>
+struct Layout {
+    static constexpr int NBL = TM * 2 * TN;                 // bins per lane
+    static constexpr int NB = NBL * 32;                     // padded spectrum length
+    static constexpr int P_WORDS = NB + NBL;                // P_s[j + (j >> 5)]
+    static constexpr int TAB_WORDS = kEC * TN * 2 + kEC * 4;
+    // scoring scratch (aliases the phasor table)
+    static constexpr int BAL_WORDS = 4 * (NBL + 1);         // belw, inbw, belc, inbc
+    static constexpr int BAND_WORDS = BS;                   // bandv
+    static constexpr int SORT_WORDS = BS;                   // sortv
+    static constexpr int POS_WORDS = BS / 2;                // posb (u16)
+    static constexpr int MASK_WORDS = BS;                   // maskw[BS/32][32]
+    static constexpr int SCORE_WORDS = BAL_WORDS + BAND_WORDS + SORT_WORDS + POS_WORDS + MASK_WORDS;
+    static constexpr int SCRATCH_WORDS = (SCORE_WORDS > TAB_WORDS ? SCORE_WORDS : TAB_WORDS);
+    static constexpr int WARP_WORDS = ((P_WORDS + SCRATCH_WORDS + 3) / 4) * 4;
+    static constexpr size_t SMEM_BYTES = static_cast<size_t>(WARP_WORDS) * 4 * kWarps;
+};
+
+__device__ __forceinline__ uint32_t phase_u32(uint64_t g, uint32_t t)
+{
+    // hi 32 bits of (g * t mod 2^64): the phase f*t in turns, 2^-32 resolution
+    return static_cast<uint32_t>(g >> 32) * t + __umulhi(static_cast<uint32_t>(g), t);
+}
+
+// (sin, cos) of 2 pi (turns - 1/2), turns = ph / 2^32.  The half-turn offset only flips the
+// sign of both components; every phasor of the kernel carries it, and centre x offset
+// phasors are always multiplied, so it cancels.  Argument of the SFU is in [-pi, pi).
+__device__ __forceinline__ void sincos_u32(uint32_t ph, float &s, float &c)
+{
+    const float x = __uint_as_float((ph >> 9) | 0x3f800000u) - 1.5f;
+    const float r = x * 6.283185307179586f;
+    s = __sinf(r);
+    c = __cosf(r);
+}
+
+__device__ __forceinline__ int pad(int j) { return j + (j >> 5); }
+
+template <int E>
+__device__ __forceinline__ void bitonic_sort_regs(float (&x)[E], int lane)
+{
+    constexpr int N = E * 32;
+#pragma unroll
+    for (int k = 2; k <= N; k <<= 1) {
+#pragma unroll
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            if (j < E) {
+#pragma unroll
+                for (int r = 0; r < E; ++r) {
+                    if ((r & j) == 0) {
+                        const bool asc = (k < E) ? ((r & k) == 0)
+                                                 : (k == N ? true : ((lane & (k / E)) == 0));
+                        const float a = x[r], b = x[r | j];
+                        const float lo = fminf(a, b), hi = fmaxf(a, b);
+                        x[r] = asc ? lo : hi;
+                        x[r | j] = asc ? hi : lo;
+                    }
+                }
+            } else {
+                const int lm = j / E;
+                const bool asc = (k == N) ? true : ((lane & (k / E)) == 0);
+                const bool lower = (lane & lm) == 0;
+                const bool take_min = (lower == asc);
+#pragma unroll
+                for (int r = 0; r < E; ++r) {
+                    const float o = __shfl_xor_sync(kFull, x[r], lm);
+                    x[r] = take_min ? fminf(x[r], o) : fmaxf(x[r], o);
+                }
+            }
+        }
+    }
+}
+
+// ----------------------------------------------------------------------------------------
+// a6: comb score of one pixel.  preg: the lane's NBL powers (bins lane + 32 i); P_s: the same
+// spectrum in shared memory (padded); returns (score, f0 index) on every lane.
+// ----------------------------------------------------------------------------------------
+template <int TM, int TN, int BS>
+__device__ __forceinline__ void comb_score(float (&preg)[TM * 2 * TN], const float *P_s, uint32_t *scr,
+                                           const ScoreParams &sp, float mean_p, int lane,
+                                           float &score_out, int &f0_out, float *dbg)
+{
+    using L = Layout<TM, TN, BS>;
+    constexpr int NBL = L::NBL;
+    constexpr int E = BS / 32;
+    uint32_t *belw = scr;
+    uint32_t *inbw = belw + (NBL + 1);
+    uint32_t *belc = inbw + (NBL + 1);
+    uint32_t *inbc = belc + (NBL + 1);
+    float *bandv = reinterpret_cast<float *>(inbc + (NBL + 1));
+    float *sortv = bandv + BS;
+    unsigned short *posb = reinterpret_cast<unsigned short *>(sortv + BS);
+    uint32_t *maskw = reinterpret_cast<uint32_t *>(sortv + BS) + BS / 2;
+
+    const int nb = sp.n_freq - sp.k_lo;
+    const int r0 = sp.r0, r1 = sp.r1;
+    const int slack = (BS - (r1 - r0 + 1)) / 2;
+
+    // invalid bins (below k_lo, or padding past n_freq) never take part in the order statistics
+#pragma unroll
+    for (int i = 0; i < NBL; ++i) {
+        const int j = i * 32 + lane;
+        if (j < sp.k_lo || j >= sp.n_freq) preg[i] = __uint_as_float(kInvalidKey);
+    }
+
+    // ---- A: band limits by counting passes over the register-resident spectrum ----------
+    // find Lkey with  r0 - slack <= #{key < Lkey} <= r0   and Ukey with
+    // r1 + 1 <= #{key < Ukey} <= r1 + 1 + slack; on heavy ties the search converges to the
+    // exact order statistic and the tied bins are split by their order in the spectrum.
+    uint32_t loL = 0u, hiL = 0x7f800001u, loU = 0u, hiU = 0x7f800001u;
+    int cntLo_L = 0, cntLo_U = 0;          // #{key < loL}, #{key < loU}
+    int cntHi_U = nb;                      // #{key < hiU}
+    bool doneL = false, doneU = false, exactL = false, exactU = false;
+    // first pivots: exponential-spectrum guess around the mean power
+    uint32_t pivL, pivU;
+    {
+        const float qL = fminf(fmaxf((r0 - 0.5f * slack) / nb, 0.01f), 0.98f);
+        const float qU = fminf(fmaxf((r1 + 1 + 0.5f * slack) / nb, 0.02f), 0.99f);
+        pivL = __float_as_uint(fmaxf(-mean_p * __logf(1.f - qL), 0.f));
+        pivU = __float_as_uint(fmaxf(-mean_p * __logf(1.f - qU), 0.f));
+        pivL = min(max(pivL, 1u), 0x7f800000u);
+        pivU = min(max(pivU, 1u), 0x7f800000u);
+    }
+    int cntL = 0, cntU = 0;
+    for (int it = 0; it < 80 && !(doneL && doneU); ++it) {
+        int cl = 0, cu = 0;
+#pragma unroll
+        for (int i = 0; i < NBL; ++i) {
+            const uint32_t key = __float_as_uint(preg[i]);
+            cl += (key < pivL);
+            cu += (key < pivU);
+        }
+        cl = __reduce_add_sync(kFull, cl);
+        cu = __reduce_add_sync(kFull, cu);
+        if (!doneL) {
+            if (cl > r0) {
+                hiL = pivL;
+            } else {
+                loL = pivL;
+                cntLo_L = cl;
+                if (cl >= r0 - slack) { doneL = true; cntL = cl; }
+            }
+            if (!doneL) {
+                if (hiL - loL <= 1u) { doneL = true; exactL = true; cntL = cntLo_L; }
+                else pivL = loL + ((hiL - loL) >> 1);
+            }
+        }
+        if (!doneU) {
+            if (cu >= r1 + 1) {
+                hiU = pivU;
+                cntHi_U = cu;
+                if (cu <= r1 + 1 + slack) { doneU = true; cntU = cu; }
+            } else {
+                loU = pivU;
+                cntLo_U = cu;
+            }
+            if (!doneU) {
+                if (hiU - loU <= 1u) { doneU = true; exactU = true; cntU = cntLo_U; }
+                else pivU = loU + ((hiU - loU) >> 1);
+            }
+        }
+    }
+    (void)cntHi_U;
+    const uint32_t Lkey = exactL ? loL : pivL;
+    const uint32_t Ukey = exactU ? loU : pivU;
+    const int tL = exactL ? (r0 - cntL) : 0;           // tied bins at Lkey that count as "below"
+    const int tU = exactU ? (r1 + 1 - cntU) : 0;       // tied bins at Ukey that are still in band
+    const int cntL_eff = cntL + tL;
+    const int cntU_eff = cntU + tU;
+    const int nband = cntU_eff - cntL_eff;
+
+    // ---- B: below / in-band flags as ballots (bit l of word i <-> bin 32 i + l) ----------
+    {
+        const uint32_t lt = (1u << lane) - 1u;
+        int runL = 0, runU = 0;
+        const bool ties = (tL | tU) != 0;
+        uint32_t my_bel0 = 0, my_inb0 = 0, my_bel1 = 0, my_inb1 = 0;   // words lane and lane+32
+#pragma unroll
+        for (int i = 0; i < NBL; ++i) {
+            const uint32_t key = __float_as_uint(preg[i]);
+            bool below = key < Lkey, leu = key < Ukey;
+            if (ties) {
+                const uint32_t mL = __ballot_sync(kFull, key == Lkey);
+                const uint32_t mU = __ballot_sync(kFull, key == Ukey);
+                const int trL = runL + __popc(mL & lt), trU = runU + __popc(mU & lt);
+                runL += __popc(mL);
+                runU += __popc(mU);
+                below = below || (key == Lkey && trL < tL);
+                leu = leu || (key == Ukey && trU < tU);
+            }
+            const uint32_t wb = __ballot_sync(kFull, below);
+            const uint32_t wi = __ballot_sync(kFull, leu && !below);
+            if ((i & 31) == lane) {
+                if (i < 32) { my_bel0 = wb; my_inb0 = wi; } else { my_bel1 = wb; my_inb1 = wi; }
+            }
+        }
+        // exclusive prefix popcounts over the words
+        int cb0 = __popc(my_bel0), ci0 = __popc(my_inb0), cb1 = __popc(my_bel1), ci1 = __popc(my_inb1);
+        int sb0 = cb0, si0 = ci0, sb1 = cb1, si1 = ci1;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int a = __shfl_up_sync(kFull, sb0, o), b = __shfl_up_sync(kFull, si0, o);
+            const int c = __shfl_up_sync(kFull, sb1, o), d = __shfl_up_sync(kFull, si1, o);
+            if (lane >= o) { sb0 += a; si0 += b; sb1 += c; si1 += d; }
+        }
+        const int totb0 = __shfl_sync(kFull, sb0, 31), toti0 = __shfl_sync(kFull, si0, 31);
+        if (lane < NBL) {
+            belw[lane] = my_bel0; inbw[lane] = my_inb0;
+            belc[lane] = sb0 - cb0; inbc[lane] = si0 - ci0;
+        }
+        if (NBL > 32 && lane + 32 < NBL) {
+            belw[lane + 32] = my_bel1; inbw[lane + 32] = my_inb1;
+            belc[lane + 32] = totb0 + sb1 - cb1; inbc[lane + 32] = toti0 + si1 - ci1;
+        }
+        if (lane == 0) {
+            belw[NBL] = 0; inbw[NBL] = 0;
+            belc[NBL] = cntL_eff; inbc[NBL] = nband;
+        }
+    }
+    __syncwarp();
+
+    // ---- C: compact the in-band powers in bin order ---------------------------------------
+    {
+        const uint32_t lt = (1u << lane) - 1u;
+#pragma unroll
+        for (int i = 0; i < NBL; ++i) {
+            const uint32_t w = inbw[i];
+            if ((w >> lane) & 1u) {
+                const int ib = inbc[i] + __popc(w & lt);
+                if (ib < BS) bandv[ib] = preg[i];
+            }
+        }
+    }
+    __syncwarp();
+
+    // ---- D: sort the band (ascending) in registers -----------------------------------------
+    {
+        float x[E];
+#pragma unroll
+        for (int r = 0; r < E; ++r) {
+            const int idx = lane * E + r;
+            x[r] = (idx < nband) ? bandv[idx] : __int_as_float(0x7f800000);
+        }
+        bitonic_sort_regs<E>(x, lane);
+#pragma unroll
+        for (int r = 0; r < E; ++r) sortv[lane * E + r] = x[r];
+    }
+    __syncwarp();
+
+    // ---- E: sorted position of every band element (unique; ties ordered by bin) -------------
+    for (int ib = lane; ib < nband; ib += 32) {
+        const float v = bandv[ib];
+        int lo = 0, hi = nband;                 // first index with sortv >= v
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            if (sortv[mid] < v) lo = mid + 1; else hi = mid;
+        }
+        int pos = lo;
+        if (lo + 1 < nband && sortv[lo + 1] == v) {      // tied values: earlier bins first
+            for (int q = 0; q < ib; ++q) pos += (bandv[q] == v);
+        }
+        posb[ib] = static_cast<unsigned short>(pos);
+    }
+    __syncwarp();
+
+    // ---- F: one candidate per lane ------------------------------------------------------------
+    float best = 0.f;
+    int best_c = 0x7fffffff;
+    const int d = sp.half_bw;
+    for (int c0 = 0; c0 < sp.n_f0; c0 += 32) {
+        const int c = c0 + lane;
+        float snr = 0.f, num = 0.f, med = 0.f;
+        bool valid = false;
+        if (c < sp.n_f0) {
+            const CandTable *ct = sp.cand + c;
+            const int mv = ct->m_valid;
+            if (mv > 0) {
+                valid = true;
+                // eq. 8: mean over valid harmonics of the window maximum
+                for (int m = 0; m < mv; ++m) {
+                    const int kc = ct->kc[m];
+                    float mx = 0.f;
+                    for (int k = kc - d; k <= kc + d; ++k) mx = fmaxf(mx, P_s[pad(k)]);
+                    num += mx;
+                }
+                num = num / static_cast<float>(mv);
+                // eq. 9-10: lower median of the complement
+#pragma unroll
+                for (int w = 0; w < BS / 32; ++w) maskw[w * 32 + lane] = 0u;
+                int e_low = 0;
+                const int ni = ct->n_int;
+                for (int q = 0; q < ni; ++q) {
+                    const int lo = ct->lo[q], hi1 = ct->hi[q] + 1;
+                    const int wl = lo >> 5, wh = hi1 >> 5;
+                    const uint32_t ml = (1u << (lo & 31)) - 1u, mh = (1u << (hi1 & 31)) - 1u;
+                    e_low += static_cast<int>(belc[wh] + __popc(belw[wh] & mh)) -
+                             static_cast<int>(belc[wl] + __popc(belw[wl] & ml));
+                    const int ib0 = inbc[wl] + __popc(inbw[wl] & ml);
+                    const int ib1 = inbc[wh] + __popc(inbw[wh] & mh);
+                    for (int ib = ib0; ib < ib1; ++ib) {
+                        const int pos = posb[ib];
+                        maskw[(pos >> 5) * 32 + lane] |= 1u << (pos & 31);
+                    }
+                }
+                int j = static_cast<int>(ct->rank) - (cntL_eff - e_low);   // rank inside the band's complement
+                j = max(j, 0);
+                int a = nband - 1;
+#pragma unroll 1
+                for (int w = 0; w < BS / 32; ++w) {
+                    uint32_t z = ~maskw[w * 32 + lane];
+                    const int nz = __popc(z);
+                    if (j < nz) {
+                        for (int q = 0; q < j; ++q) z &= z - 1u;            // drop j lowest set bits
+                        a = w * 32 + (__ffs(z) - 1);
+                        break;
+                    }
+                    j -= nz;
+                }
+                a = min(a, max(nband - 1, 0));
+                med = sortv[a];
+                snr = num / fmaxf(med, sp.sf_eps);
+            }
+        }
+        if (dbg != nullptr && c < sp.n_f0) {
+            dbg[c * 3 + 0] = snr;
+            dbg[c * 3 + 1] = num;
+            dbg[c * 3 + 2] = med;
+        }
+        if (valid && (best_c == 0x7fffffff || snr > best)) { best = snr; best_c = c; }
+        __syncwarp();
+    }
+    // eq. 11: max over candidates, first maximum wins
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const float ob = __shfl_xor_sync(kFull, best, o);
+        const int oc = __shfl_xor_sync(kFull, best_c, o);
+        const bool take = (oc != 0x7fffffff) && (best_c == 0x7fffffff || ob > best || (ob == best && oc < best_c));
+        if (take) { best = ob; best_c = oc; }
+    }
+    score_out = (best_c == 0x7fffffff) ? 0.f : best;
+    f0_out = (best_c == 0x7fffffff) ? -1 : best_c;
+}
+
+// ----------------------------------------------------------------------------------------
+// The fused kernel.
+// ----------------------------------------------------------------------------------------
+template <int TM, int TN, int BS>
+__global__ void __launch_bounds__(kWarps * 32, 3) k_ndft_score(NdftParams p)
+{
+    using L = Layout<TM, TN, BS>;
+    constexpr int NBL = L::NBL;
+    extern __shared__ __align__(16) uint32_t smem_raw[];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    uint32_t *wsm = smem_raw + wid * L::WARP_WORDS;
+    float *P_s = reinterpret_cast<float *>(wsm);
+    uint32_t *scr = wsm + L::P_WORDS;
+    float2 *btab = reinterpret_cast<float2 *>(scr);                 // [kEC][TN]
+    uint4 *phs = reinterpret_cast<uint4 *>(scr + kEC * TN * 2);     // [kEC]
+
+    const int n_items = p.counters[DDHF_CNT_N_ACTIVE];
+    const ScoreParams &sp = p.sp;
+    constexpr int EPP = 32 / TN;       // events per table pass
+
+    while (true) {
+        int idx = 0;
+        if (lane == 0) idx = atomicAdd(p.work_cursor, 1);
+        idx = __shfl_sync(kFull, idx, 0);
+        if (idx >= n_items) break;
+        const WorkItem it = p.work[idx];
+
+        float2 acc1[TM][TN], acc2[TM][TN];     // (S1, S4) and (S3, S2)
+#pragma unroll
+        for (int g = 0; g < TM; ++g)
+#pragma unroll
+            for (int m = 0; m < TN; ++m) {
+                acc1[g][m] = make_float2(0.f, 0.f);
+                acc2[g][m] = make_float2(0.f, 0.f);
+            }
+
+        for (int base = 0; base < it.n; base += kEC) {
+            const int nc = min(kEC, it.n - base);
+            // ---- per-event phase words and the offset-phasor table of this chunk ----------
+            uint32_t v = 0, hph = 0;
+            if (lane < nc) {
+                v = __ldg(p.csr_ev + it.row_begin + base + lane);
+                const uint32_t t = v >> 1;
+                hph = phase_u32(p.g_h, t);
+                phs[lane] = make_uint4(phase_u32(p.g_f0, t), phase_u32(p.g_d, t), hph, 0u);
+            }
+#pragma unroll
+            for (int ps = 0; ps < kEC / EPP; ++ps) {
+                const int e = ps * EPP + lane / TN, m = lane % TN;
+                const uint32_t ve = __shfl_sync(kFull, v, e);
+                const uint32_t he = __shfl_sync(kFull, hph, e);
+                float s, c;
+                sincos_u32(he * static_cast<uint32_t>(2 * m + 1), s, c);
+                // b = w (cos, -sin) up to the common sign; w = +1 if bit 0 else -1
+                const float w = (ve & 1u) ? 1.f : -1.f;
+                btab[e * TN + m] = (e < nc) ? make_float2(w * c, -w * s) : make_float2(0.f, 0.f);
+            }
+            __syncwarp();
+            // ---- accumulate: 4 real products per (centre, offset pair, event) --------------
+#pragma unroll 1
+            for (int k = 0; k < nc; ++k) {
+                const uint4 ph = phs[k];
+                float2 ar[TM], ai[TM];
+#pragma unroll
+                for (int g = 0; g < TM; ++g) {
+                    const uint32_t pc = ph.x + static_cast<uint32_t>(lane) * ph.y +
+                                        static_cast<uint32_t>(g * 4 * TN) * ph.z;
+                    float s, c;
+                    sincos_u32(pc, s, c);
+                    ar[g] = make_float2(c, c);
+                    ai[g] = make_float2(-s, -s);
+                }
+                const float4 *brow = reinterpret_cast<const float4 *>(btab + k * TN);
+#pragma unroll
+                for (int m2 = 0; m2 < TN / 2; ++m2) {
+                    const float4 bb = brow[m2];
+                    const float2 b0 = make_float2(bb.x, bb.y), b1 = make_float2(bb.z, bb.w);
+#pragma unroll
+                    for (int g = 0; g < TM; ++g) {
+                        acc1[g][2 * m2] = __ffma2_rn(ar[g], b0, acc1[g][2 * m2]);
+                        acc2[g][2 * m2] = __ffma2_rn(ai[g], b0, acc2[g][2 * m2]);
+                        acc1[g][2 * m2 + 1] = __ffma2_rn(ar[g], b1, acc1[g][2 * m2 + 1]);
+                        acc2[g][2 * m2 + 1] = __ffma2_rn(ai[g], b1, acc2[g][2 * m2 + 1]);
+                    }
+                }
+            }
+            __syncwarp();
+        }
+
+        // ---- epilogue: powers, spectrum store, spectral flatness ---------------------------
+        float preg[NBL];
+#pragma unroll
+        for (int g = 0; g < TM; ++g)
+#pragma unroll
+            for (int m = 0; m < TN; ++m) {
+                const float s1 = acc1[g][m].x, s4 = acc1[g][m].y, s3 = acc2[g][m].x, s2 = acc2[g][m].y;
+                const float rp = s1 - s2, ip = s4 + s3;       // bin centre + (m + 1/2) 32 df
+                const float rm = s1 + s2, im = s3 - s4;       // bin centre - (m + 1/2) 32 df
+                preg[g * 2 * TN + TN + m] = rp * rp + ip * ip;
+                preg[g * 2 * TN + TN - 1 - m] = rm * rm + im * im;
+            }
+        const bool has_row = it.arow < p.max_active;
+        float slog = 0.f, ssum = 0.f;
+#pragma unroll
+        for (int i = 0; i < NBL; ++i) {
+            const int j = i * 32 + lane;
+            P_s[i * 33 + lane] = preg[i];                       // == pad(j)
+            if (j < sp.n_freq) {
+                if (p.power != nullptr && has_row)
+                    __stcs(p.power + static_cast<size_t>(it.arow) * sp.n_freq + j, preg[i]);
+                if (j >= sp.k_lo) {
+                    const float pt = fmaxf(preg[i], sp.sf_eps);
+                    slog += __log2f(pt);
+                    ssum += pt;
+                }
+            }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            slog += __shfl_xor_sync(kFull, slog, o);
+            ssum += __shfl_xor_sync(kFull, ssum, o);
+        }
+        const float inv_nb = 1.f / static_cast<float>(sp.n_freq - sp.k_lo);
+        const float mean_p = ssum * inv_nb;
+        const float sfv = exp2f(slog * inv_nb) / mean_p;         // eq. 7
+        const bool sf_ok = sfv <= sp.tau_sf;                     // discard if SF > tau_sf (L107)
+        __syncwarp();
+
+        float score = 0.f;
+        int f0 = -1;
+        if (sp.score_all || sf_ok) {
+            float *dbg = (p.comb_debug != nullptr && has_row)
+                             ? p.comb_debug + static_cast<size_t>(it.arow) * sp.n_f0 * 3 : nullptr;
+            comb_score<TM, TN, BS>(preg, P_s, scr, sp, mean_p, lane, score, f0, dbg);
+            if (lane == 0) atomicAdd(p.n_scored, 1);
+        }
+        if (lane == 0) {
+            p.sf[it.pix] = sfv;
+            p.score[it.pix] = score;
+            p.f0_idx[it.pix] = f0;
+            p.mask[it.pix] = (sf_ok && f0 >= 0 && score >= sp.tau_comb) ? 1 : 0;   // eq. 11
+        }
+        __syncwarp();
+    }
+}
+
+template <int TM, int TN, int BS>
+int launch_one(const NdftParams &p, int sm_count, cudaStream_t st)
+{
+    using L = Layout<TM, TN, BS>;
+    static bool configured = false;
+    static int blocks_per_sm = 1;
+    if (!configured) {
+        cudaFuncSetAttribute(k_ndft_score<TM, TN, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             static_cast<int>(L::SMEM_BYTES));
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, k_ndft_score<TM, TN, BS>,
+                                                      kWarps * 32, L::SMEM_BYTES);
+        if (blocks_per_sm < 1) blocks_per_sm = 1;
+        configured = true;
+    }
+    k_ndft_score<TM, TN, BS><<<sm_count * blocks_per_sm, kWarps * 32, L::SMEM_BYTES, st>>>(p);
+    return 1;
+}
+
+}  // namespace
+
+int ndft_bins_per_lane(int n_freq)
+{
+    if (n_freq <= 256) return 8;
+    if (n_freq <= 512) return 16;
+    if (n_freq <= 1024) return 32;
+    return 64;
+}
+
+int ndft_tn(int n_freq)
+{
+    const int nbl = ndft_bins_per_lane(n_freq);
+    return nbl >= 32 ? 16 : nbl / 2;
+}
+
+int ndft_band_size(int n_freq, int r0, int r1)
+{
+    const int need = r1 - r0 + 1;
+    const int nb = ndft_bins_per_lane(n_freq) * 32;
+    if (need + 16 <= 256 || nb <= 256) return (need <= 256) ? 256 : 0;
+    if (need + 32 <= 512 || nb <= 512) return (need <= 512) ? 512 : 0;
+    if (nb >= 2048 && need <= 1024) return 1024;
+    return 0;
+}
+
+int launch_ndft(const NdftParams &p, int n_freq, int sm_count, cudaStream_t st)
+{
+    const int nbl = ndft_bins_per_lane(n_freq);
+    const int bs = ndft_band_size(n_freq, p.sp.r0, p.sp.r1);
+    if (nbl == 8) return launch_one<1, 4, 256>(p, sm_count, st);
+    if (nbl == 16) return bs == 256 ? launch_one<1, 8, 256>(p, sm_count, st) : launch_one<1, 8, 512>(p, sm_count, st);
+    if (nbl == 32) return bs == 256 ? launch_one<1, 16, 256>(p, sm_count, st) : launch_one<1, 16, 512>(p, sm_count, st);
+    if (bs == 256) return launch_one<2, 16, 256>(p, sm_count, st);
+    if (bs == 512) return launch_one<2, 16, 512>(p, sm_count, st);
+    return launch_one<2, 16, 1024>(p, sm_count, st);
+}
+
+}  // namespace ddhf

@@ -1,0 +1,111 @@
+"""Helpers shared by the GPU parity tests: run the CUDA path through the C ABI binding and
+compare it with the float64 oracle, stage by stage.
+
+Tolerances (north_star):
+  CSR                 bit-exact
+  power               |P_gpu - P_oracle| <= 1e-3 * max_j P_oracle  per pixel
+  SF, score           relative 1e-3 (they are ratios of sums / order statistics of P)
+  mask / f0 / boxes   bit-exact, except pixels whose SF or score lies within 1e-3 relative of
+                      its threshold (excluded) and f0 ties (top-2 SNR within 1e-3 relative)
+"""
+from __future__ import annotations
+
+import numpy as np
+
+POWER_TOL = 1e-3
+REL_TOL = 1e-3
+
+
+def run_gpu(params, events, t0, window_us, *, score_all=False, want_power=True, want_debug=False,
+            max_active=None, max_boxes=4096, max_events=None, timing=False):
+    from paper_2603_08386_b200 import binding
+    det = binding.Detector(params, max_events=max_events or max(len(events), 1),
+                           max_active=max_active, max_boxes=max_boxes, score_all=score_all,
+                           want_power=want_power, want_debug=want_debug, timing=timing)
+    d_ev = det.upload(events) if len(events) else None
+    det.window(d_ev, len(events), t0, window_us)
+    res = det.results()
+    if timing:
+        res["stage_ms"] = det.stage_ms()
+    res["launches"] = binding.ddhf_launches_per_window(det.h)
+    det.close()
+    return res
+
+
+def check_csr(gpu, orc):
+    assert gpu["n_in"] == orc["n_in"], (gpu["n_in"], orc["n_in"])
+    assert gpu["n_dropped"] == orc["n_dropped"]
+    assert np.array_equal(gpu["row_ptr"], orc["row_ptr"]), "row_ptr differs"
+    assert np.array_equal(gpu["csr_ev"], orc["csr_ev"]), "csr_ev differs"
+    assert gpu["n_active"] == orc["n_active"]
+    assert np.array_equal(gpu["active_idx"], orc["active_idx"]), "active_idx differs"
+
+
+def power_error(gpu_power, orc_power):
+    """max over pixels of max_j |P_gpu - P_orc| / peak_orc."""
+    if len(orc_power) == 0:
+        return 0.0
+    peak = orc_power.max(axis=1)
+    err = np.abs(gpu_power.astype(np.float64) - orc_power).max(axis=1) / np.maximum(peak, 1e-300)
+    return float(err.max())
+
+
+def near(value, thr, rel=REL_TOL):
+    return np.abs(value - thr) <= rel * abs(thr)
+
+
+def check_maps(gpu, orc, params, *, score_all, oracle_mod=None, orc_power=None):
+    """SF, score, f0_idx and mask on all pixels.  Returns the boolean map of pixels that are
+    within tolerance of a threshold (excluded from the exact comparisons)."""
+    act = np.zeros(gpu["sf"].size, bool)
+    act[orc["active_idx"]] = True
+    act = act.reshape(gpu["sf"].shape)
+    # inactive pixels
+    assert np.isnan(gpu["sf"][~act]).all()
+    assert (gpu["score"][~act] == 0).all() and (gpu["f0_idx"][~act] == -1).all()
+    assert (gpu["mask"][~act] == 0).all()
+    # SF
+    sf_g, sf_o = gpu["sf"][act].astype(np.float64), orc["sf"][act]
+    sf_err = np.abs(sf_g - sf_o) / np.maximum(np.abs(sf_o), 1e-30)
+    assert sf_err.max(initial=0) <= REL_TOL, f"SF rel err {sf_err.max()}"
+    edge_sf = near(orc["sf"], params["tau_sf"]) & act
+    # score is evaluated where score_all or SF <= tau_sf
+    scored_o = act & (np.ones_like(act) if score_all else (orc["sf"] <= params["tau_sf"]))
+    cmp_px = scored_o & ~edge_sf
+    s_g, s_o = gpu["score"][cmp_px].astype(np.float64), orc["score"][cmp_px]
+    s_err = np.abs(s_g - s_o) / np.maximum(np.abs(s_o), 1e-30)
+    s_err[(s_o == 0) & (s_g == 0)] = 0
+    assert s_err.max(initial=0) <= REL_TOL, f"score rel err {s_err.max()} at {np.argmax(s_err)}"
+    if not score_all:
+        skipped = act & ~scored_o & ~edge_sf
+        assert (gpu["score"][skipped] == 0).all() and (gpu["f0_idx"][skipped] == -1).all()
+    # f0 index: equal unless the oracle's two best candidates tie within tolerance
+    diff = cmp_px & (gpu["f0_idx"] != orc["f0_idx"])
+    if diff.any():
+        assert oracle_mod is not None and orc_power is not None, \
+            f"{diff.sum()} f0_idx mismatches and no spectra to check ties"
+        row_of = {int(p): r for r, p in enumerate(orc["active_idx"])}
+        W = gpu["sf"].shape[1]
+        for y, x in zip(*np.nonzero(diff)):
+            r = row_of[int(y) * W + int(x)]
+            if r >= len(orc_power):
+                continue
+            _, _, snr, _, _ = oracle_mod.comb_score(orc_power[r], params)
+            g, o = gpu["f0_idx"][y, x], orc["f0_idx"][y, x]
+            assert g >= 0 and abs(snr[g] - snr[o]) <= REL_TOL * snr[o], \
+                f"f0_idx {g} vs {o} at ({x},{y}): snr {snr[g]} vs {snr[o]}"
+    # mask
+    edge = edge_sf | (near(orc["score"], params["tau_comb"]) & scored_o)
+    bad = (gpu["mask"] != orc["mask"]) & ~edge
+    assert not bad.any(), f"{bad.sum()} mask mismatches outside tolerance"
+    return edge
+
+
+def check_boxes_against_oracle_ccl(gpu, oracle_mod, a_min, max_boxes=4096):
+    """GPU CCL/boxes vs the oracle's CCL run on the GPU's own mask (exact)."""
+    labels, boxes, total = oracle_mod.ccl_boxes(gpu["mask"], a_min, max_boxes=max_boxes)
+    if "labels" in gpu:
+        assert np.array_equal(gpu["labels"], labels), "labels differ"
+    assert gpu["n_boxes_total"] == total and gpu["n_boxes"] == len(boxes)
+    for k in ("x0", "y0", "x1", "y1", "n_pix", "label"):
+        assert np.array_equal(gpu["boxes"][k], boxes[k]), f"boxes.{k} differ"

@@ -1,0 +1,201 @@
+"""GPU edge cases of the C ABI: empty and degenerate inputs, capacity limits, error codes,
+determinism, the host-buffer (end-to-end) entry point."""
+import ctypes as C
+
+import numpy as np
+import pytest
+
+from paper_2603_08386_b200 import workloads as wl
+
+import gpu_util as gu
+
+pytestmark = pytest.mark.gpu
+
+SMALL = dict(wl.preset(1), width=48, height=40)
+
+
+def test_empty_window(oracle):
+    ev = np.zeros(0, dtype=wl.EVENT_DTYPE)
+    gpu = gu.run_gpu(SMALL, ev, 0, 20_000)
+    assert gpu["n_in"] == 0 and gpu["n_active"] == 0 and gpu["n_boxes"] == 0
+    assert (gpu["row_ptr"] == 0).all() and gpu["mask"].sum() == 0 and np.isnan(gpu["sf"]).all()
+
+
+def test_all_events_dropped(oracle):
+    ev = wl.random_window(3, 48, 40, 1000, 20_000)
+    ev["t"] += 1_000_000                      # all after the window
+    gpu = gu.run_gpu(SMALL, ev, 0, 20_000)
+    assert gpu["n_in"] == 0 and gpu["n_dropped"] == 1000 and gpu["n_active"] == 0
+
+
+def test_unsorted_input_and_bad_coordinates(oracle):
+    ev = wl.random_window(4, 48, 40, 20_000, 20_000, hot_fraction=0.3, out_of_range=0.15,
+                          time_sorted=False)
+    prm = dict(SMALL, n_min=2)
+    orc = oracle.window(prm, ev, 0, 20_000, score_all=True)
+    gpu = gu.run_gpu(prm, ev, 0, 20_000, score_all=True)
+    gu.check_csr(gpu, orc)
+    assert gpu["n_dropped"] > 1000
+    assert gu.power_error(gpu["power"], orc["power"]) <= gu.POWER_TOL
+    gu.check_maps(gpu, orc, prm, score_all=True, oracle_mod=oracle, orc_power=orc["power"])
+
+
+def test_nonzero_t0_and_negative_times(oracle):
+    ev = wl.random_window(5, 48, 40, 8000, 30_000)
+    ev["t"] -= 10_000                          # stream spans [-10 ms, 20 ms)
+    prm = dict(SMALL, n_min=2)
+    for t0 in (-10_000, -3_333, 5_000):
+        orc = oracle.window(prm, ev, t0, 15_000, score_all=True)
+        gpu = gu.run_gpu(prm, ev, t0, 15_000, score_all=True)
+        gu.check_csr(gpu, orc)
+        assert gu.power_error(gpu["power"], orc["power"]) <= gu.POWER_TOL
+
+
+def test_single_hot_pixel_long_row(oracle):
+    """All events on one pixel: one very long row (row sort, chunk loop, size class > 8)."""
+    n = 6000
+    rng = np.random.default_rng(7)
+    ev = np.zeros(n, dtype=wl.EVENT_DTYPE)
+    ev["x"], ev["y"] = 5, 7
+    ev["t"] = np.sort(rng.integers(0, 20_000, size=n))
+    ev["p"] = rng.integers(0, 2, size=n) * 2 - 1
+    orc = oracle.window(SMALL, ev, 0, 20_000, score_all=True)
+    gpu = gu.run_gpu(SMALL, ev, 0, 20_000, score_all=True)
+    gu.check_csr(gpu, orc)
+    assert gpu["n_active"] == 1
+    assert gu.power_error(gpu["power"], orc["power"]) <= gu.POWER_TOL
+    gu.check_maps(gpu, orc, SMALL, score_all=True, oracle_mod=oracle, orc_power=orc["power"])
+
+
+def test_single_event_pixels_flat_spectrum(oracle):
+    """n_min = 1: one-event pixels have P = w^2 = 1 in every bin (massive ties in the median)."""
+    ev = wl.random_window(8, 48, 40, 600, 20_000)
+    prm = dict(SMALL, n_min=1)
+    orc = oracle.window(prm, ev, 0, 20_000, score_all=True)
+    gpu = gu.run_gpu(prm, ev, 0, 20_000, score_all=True)
+    gu.check_csr(gpu, orc)
+    single = np.flatnonzero(np.diff(orc["row_ptr"])[orc["active_idx"]] == 1)
+    assert len(single) > 100
+    assert np.allclose(gpu["power"][single], 1.0, atol=1e-5)
+    assert np.allclose(gpu["sf"].ravel()[orc["active_idx"][single]], 1.0, atol=1e-5)
+    assert np.allclose(gpu["score"].ravel()[orc["active_idx"][single]], 1.0, atol=1e-4)
+    gu.check_maps(gpu, orc, prm, score_all=True, oracle_mod=oracle, orc_power=orc["power"])
+
+
+@pytest.mark.parametrize("nf,klo,fmin", [(8, 0, 50.0), (33, 1, 0.0), (256, 0, 12.5), (257, 1, 0.0),
+                                         (512, 2, 0.0), (513, 1, 3.0), (1025, 1, 0.0), (2048, 0, 1.0)])
+def test_grid_shapes(oracle, nf, klo, fmin):
+    """Ragged n_freq (not a multiple of 32), every kernel instantiation, k_lo and f_min != 0."""
+    ev = wl.random_window(9 + nf, 32, 24, 4000, 20_000, hot_fraction=0.2)
+    df = 2000.0 / nf
+    prm = dict(SMALL, width=32, height=24, n_freq=nf, df_hz=df, k_lo=klo, f_min_hz=fmin, n_min=3,
+               f0_min_hz=max(100.0, 12 * df), f0_step_hz=10.0, n_f0=40 if nf > 64 else 3,
+               n_harm=4 if nf > 64 else 1, h_min=2 if nf > 64 else 1,
+               half_bw_bins=2 if nf > 64 else 0)
+    orc = oracle.window(prm, ev, 0, 20_000, score_all=True)
+    gpu = gu.run_gpu(prm, ev, 0, 20_000, score_all=True)
+    gu.check_csr(gpu, orc)
+    assert gu.power_error(gpu["power"], orc["power"]) <= gu.POWER_TOL
+    gu.check_maps(gpu, orc, prm, score_all=True, oracle_mod=oracle, orc_power=orc["power"])
+
+
+def test_capacity_truncation(oracle):
+    w = wl.make(1)
+    prm = dict(w.params, n_min=1, a_min=1, tau_sf=1.0, tau_comb=0.0)    # everything is a detection
+    orc = oracle.window(prm, w.events, 0, w.window_us, score_all=True, max_boxes=1 << 16)
+    gpu = gu.run_gpu(prm, w.events, 0, w.window_us, score_all=True, max_active=100, max_boxes=5)
+    assert gpu["overflow"] == 3
+    assert gpu["n_active"] == orc["n_active"] > 100
+    assert np.array_equal(gpu["active_idx"], orc["active_idx"][:100])        # lowest indices kept
+    assert gu.power_error(gpu["power"], orc["power"][:100]) <= gu.POWER_TOL
+    # per-pixel maps stay complete even though the compact outputs are truncated
+    gu.check_maps(gpu, orc, prm, score_all=True, oracle_mod=oracle, orc_power=orc["power"])
+    assert gpu["n_boxes"] == 5 and gpu["n_boxes_total"] == orc["n_boxes_total"]
+    assert np.array_equal(gpu["boxes"]["label"], orc["boxes"]["label"][:5])
+
+
+def test_error_codes():
+    from paper_2603_08386_b200 import binding
+    bad = [dict(n_freq=4), dict(n_freq=4096), dict(df_hz=0.0), dict(n_f0=0), dict(n_harm=17),
+           dict(k_lo=-1), dict(width=0), dict(sf_eps=0.0),
+           # harmonic windows that exclude more bins than the band sorter holds
+           dict(n_freq=2048, df_hz=1.0, n_harm=16, half_bw_bins=40, h_min=1, f0_min_hz=100.0)]
+    for b in bad:
+        with pytest.raises(binding.DdhfError) as e:
+            binding.ddhf_create(binding.make_config(dict(SMALL, **b), max_events=10))
+        assert e.value.code == binding.DDHF_E_INVAL, b
+    det = binding.Detector(SMALL, max_events=10)
+    ev = det.upload(wl.random_window(1, 48, 40, 20, 20_000))
+    with pytest.raises(binding.DdhfError) as e:
+        det.window(ev, 20, 0, 20_000)
+    assert e.value.code == binding.DDHF_E_CAPACITY
+    with pytest.raises(binding.DdhfError) as e:
+        det.window(ev, 10, 0, 0)
+    assert e.value.code == binding.DDHF_E_INVAL
+    with pytest.raises(binding.DdhfError) as e:
+        det.window(ev, 10, 0, 1 << 31)
+    assert e.value.code == binding.DDHF_E_INVAL
+    det.close()
+
+
+def test_deterministic_and_stateless():
+    """Two runs (with another window in between) give bit-identical outputs."""
+    w = wl.make(2)
+    from paper_2603_08386_b200 import binding
+    det = binding.Detector(w.params, max_events=len(w.events), want_power=True)
+    d_ev = det.upload(w.events)
+    det.window(d_ev, len(w.events), 0, w.window_us)
+    a = det.results()
+    det.window(d_ev, len(w.events) // 2, 0, w.window_us // 2)
+    det.results()
+    det.window(d_ev, len(w.events), 0, w.window_us)
+    b = det.results()
+    det.close()
+    for k in ("row_ptr", "csr_ev", "active_idx", "power", "sf", "score", "f0_idx", "mask", "labels", "boxes"):
+        same = (np.array_equal(a[k], b[k], equal_nan=True) if a[k].dtype.kind == "f"
+                else np.array_equal(a[k], b[k]))
+        assert same, k
+
+
+def test_host_buffer_entry_point_matches_device_path():
+    """ddhf_window_host (H2D + kernels + D2H inside the call) == ddhf_window on device buffers."""
+    import torch
+    from paper_2603_08386_b200 import binding
+    w = wl.make(2)
+    ref = gu.run_gpu(w.params, w.events, 0, w.window_us, want_power=True)
+    cfg = binding.make_config(w.params, max_events=len(w.events), flags=binding.DDHF_FLAG_TIMING)
+    h = binding.ddhf_create(cfg)
+    NP = w.width * w.height
+    ev = torch.from_numpy(np.ascontiguousarray(w.events).view(np.uint8).copy()).pin_memory()
+    host = dict(
+        row_ptr=np.zeros(NP + 1, np.int32), csr_ev=np.zeros(len(w.events), np.uint32),
+        active_idx=np.zeros(NP, np.int32), power=np.zeros((NP, cfg.n_freq), np.float32),
+        sf=np.zeros(NP, np.float32), score=np.zeros(NP, np.float32), f0_idx=np.zeros(NP, np.int32),
+        mask=np.zeros(NP, np.uint8), labels=np.zeros(NP, np.int32),
+        boxes=np.zeros(cfg.max_boxes, binding.BOX_DTYPE), counters=np.zeros(8, np.int32))
+    out = binding.DdhfHostOutputs()
+    for k, v in host.items():
+        setattr(out, k, v.ctypes.data)
+    for _ in range(2):                       # second call reuses the handle's buffers
+        binding.ddhf_window_host(h, ev.data_ptr(), len(w.events), 0, w.window_us, out, 0)
+    ms = binding.ddhf_stage_ms(h)
+    assert all(m >= 0 for m in ms) and abs(ms[3] - sum(ms[:3])) < 0.05 * ms[3] + 0.01
+    assert binding.ddhf_launches_per_window(h) >= 10
+    binding.ddhf_destroy(h)
+    n_in, n_act, n_box = (int(host["counters"][i]) for i in (0, 2, 3))
+    assert n_in == ref["n_in"] and n_act == ref["n_active"] and n_box == ref["n_boxes"]
+    assert np.array_equal(host["row_ptr"], ref["row_ptr"])
+    assert np.array_equal(host["csr_ev"][:n_in], ref["csr_ev"])
+    assert np.array_equal(host["active_idx"][:n_act], ref["active_idx"])
+    assert np.array_equal(host["power"][:n_act], ref["power"])
+    assert np.array_equal(host["mask"].reshape(ref["mask"].shape), ref["mask"])
+    assert np.array_equal(host["score"].reshape(ref["mask"].shape), ref["score"])
+    assert np.array_equal(host["labels"].reshape(ref["mask"].shape), ref["labels"])
+    assert np.array_equal(host["boxes"][:n_box], ref["boxes"])
+
+
+def test_fma_probe_reports_plausible_peak():
+    from paper_2603_08386_b200 import binding
+    scalar, packed = binding.ddhf_fma_peak_probe(5.0)
+    print(f"FMA probe: scalar {scalar:.1f} TFLOP/s, packed {packed:.1f} TFLOP/s")
+    assert 20.0 < max(scalar, packed) < 90.0

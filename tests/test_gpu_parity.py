@@ -1,0 +1,189 @@
+"""GPU parity: the CUDA path (through the C ABI) against the float64 oracle, element by
+element on the same seeded inputs.  Run with `pytest -m gpu` on a B200."""
+import numpy as np
+import pytest
+
+from paper_2603_08386_b200 import workloads as wl
+
+import gpu_util as gu
+
+pytestmark = pytest.mark.gpu
+
+
+def _full_compare(oracle, w, params, *, score_all, events=None, t0=None):
+    ev = w.events if events is None else events
+    t0 = w.t0_us if t0 is None else t0
+    orc = oracle.window(params, ev, t0, w.window_us, score_all=score_all, want_power=True)
+    gpu = gu.run_gpu(params, ev, t0, w.window_us, score_all=score_all, want_power=True,
+                     want_debug=True)
+    gu.check_csr(gpu, orc)
+    err = gu.power_error(gpu["power"], orc["power"])
+    assert err <= gu.POWER_TOL, f"power error / peak = {err}"
+    gu.check_maps(gpu, orc, params, score_all=score_all, oracle_mod=oracle, orc_power=orc["power"])
+    gu.check_boxes_against_oracle_ccl(gpu, oracle, params["a_min"])
+    if np.array_equal(gpu["mask"], orc["mask"]):
+        assert np.array_equal(gpu["boxes"], orc["boxes"].view(gpu["boxes"].dtype))
+    return gpu, orc, err
+
+
+@pytest.mark.parametrize("n_min", [1, 6])
+@pytest.mark.parametrize("score_all", [False, True])
+def test_config1_full(oracle, n_min, score_all):
+    w = wl.make(1)
+    prm = dict(w.params, n_min=n_min)
+    gpu, orc, err = _full_compare(oracle, w, prm, score_all=score_all)
+    assert gpu["mask"].sum() >= 40            # the rotor patch is found
+    print(f"cfg1 n_min={n_min} score_all={score_all}: power err/peak {err:.2e}, "
+          f"active {gpu['n_active']}, scored {gpu['n_scored']}, mask {gpu['mask'].sum()}")
+
+
+@pytest.mark.parametrize("n_min,score_all", [(6, False), (6, True), (1, False), (3, True)])
+def test_config2_full(oracle, n_min, score_all):
+    w = wl.make(2)
+    prm = dict(w.params, n_min=n_min)
+    gpu, orc, err = _full_compare(oracle, w, prm, score_all=score_all)
+    print(f"cfg2 n_min={n_min} score_all={score_all}: power err/peak {err:.2e}, "
+          f"active {gpu['n_active']}, scored {gpu['n_scored']}, mask {gpu['mask'].sum()}")
+
+
+def test_comb_per_candidate_debug(oracle):
+    """Per-candidate SNR_M, numerator and complement median (eq. 8-10) against the oracle."""
+    w = wl.make(2)
+    prm = dict(w.params, n_min=4)
+    orc = oracle.window(prm, w.events, 0, w.window_us, score_all=True)
+    gpu = gu.run_gpu(prm, w.events, 0, w.window_us, score_all=True, want_debug=True)
+    worst = 0.0
+    for r in range(gpu["n_active"]):
+        s, fi, snr, num, med = oracle.comb_score(orc["power"][r], prm)
+        d = gpu["comb_debug"][r].astype(np.float64)
+        for k, ref in enumerate((snr, num, med)):
+            e = np.abs(d[:, k] - ref) / np.maximum(np.abs(ref), 1e-30)
+            e[(ref == 0) & (d[:, k] == 0)] = 0
+            worst = max(worst, e.max())
+            assert e.max() <= gu.REL_TOL, f"row {r} field {k} cand {np.argmax(e)}: {d[np.argmax(e), k]} vs {ref[np.argmax(e)]}"
+    print(f"per-candidate worst rel err {worst:.2e}")
+
+
+def test_paper_table2_thresholds(oracle):
+    """Table 2 finals (tau_sf 0.89, tau_comb 1.5, M 4, dk 3, h_min 4, n_min 6, A_min 147)."""
+    w = wl.make(2)
+    t2 = wl.paper_table2()
+    prm = dict(w.params, tau_sf=t2["tau_sf"], tau_comb=t2["tau_comb"], n_harm=t2["n_harm"],
+               half_bw_bins=t2["half_bw_bins"], h_min=t2["h_min"], n_min=t2["n_min"], a_min=t2["a_min"])
+    _full_compare(oracle, w, prm, score_all=False)
+
+
+def test_paper_native_grid(oracle):
+    """The paper's own operating point: 33.3 ms window, integer modes df = 1/T (L137, L139)."""
+    w = wl.make(2)
+    T = 33_333
+    prm = dict(w.params, df_hz=1e6 / T, n_freq=128, n_harm=4, half_bw_bins=3, h_min=4, n_min=6,
+               f0_min_hz=90.0, f0_step_hz=30.0, n_f0=12)
+    orc = oracle.window(prm, w.events, 0, T, score_all=True)
+    gpu = gu.run_gpu(prm, w.events, 0, T, score_all=True, want_power=True)
+    gu.check_csr(gpu, orc)
+    assert gu.power_error(gpu["power"], orc["power"]) <= gu.POWER_TOL
+    gu.check_maps(gpu, orc, prm, score_all=True, oracle_mod=oracle, orc_power=orc["power"])
+
+
+def test_config4_quarter_scale(oracle):
+    """Config-4 scene on a 320x180 sensor: heavy-tailed rows, several size classes."""
+    w = wl.make(4, scale=0.25)
+    gpu, orc, err = _full_compare(oracle, w, w.params, score_all=False)
+    assert np.diff(orc["row_ptr"]).max() > 500          # a long row is present
+    print(f"cfg4/16: events {len(w.events)}, active {gpu['n_active']}, power err/peak {err:.2e}, "
+          f"scored {gpu['n_scored']}, mask {gpu['mask'].sum()}, boxes {gpu['n_boxes']}")
+
+
+def _sampled_compare(oracle, w, params, ev, t0, n_sample, score_all, seed=0):
+    """Full-size run on the GPU; CSR compared in full; spectra / SF / comb on sampled pixels
+    the oracle computes one by one; CCL against the oracle's CCL of the same mask."""
+    gpu = gu.run_gpu(params, ev, t0, w.window_us, score_all=score_all, want_power=True)
+    row_ptr, csr, dropped = oracle.bucket(ev, params["width"], params["height"], t0, w.window_us)
+    assert np.array_equal(gpu["row_ptr"], row_ptr) and np.array_equal(gpu["csr_ev"], csr)
+    assert gpu["n_dropped"] == dropped
+    cnt = np.diff(row_ptr)
+    act = np.flatnonzero(cnt >= params["n_min"])
+    assert np.array_equal(gpu["active_idx"], act)
+    rng = np.random.default_rng(seed)
+    rows = set(rng.choice(len(act), size=min(n_sample, len(act)), replace=False).tolist())
+    rows |= set(np.argsort(cnt[act])[-5:].tolist())                      # the longest rows
+    truth = w.truth.get("mask")
+    if truth is not None:
+        tp = np.flatnonzero(truth.ravel()[act])
+        rows |= set(rng.choice(tp, size=min(60, len(tp)), replace=False).tolist())
+    worst_p = worst_sf = worst_s = 0.0
+    W = params["width"]
+    for r in sorted(rows):
+        p = int(act[r])
+        seg = csr[row_ptr[p]:row_ptr[p + 1]]
+        P = oracle.ndft_power(seg >> 1, np.where(seg & 1, 1.0, -1.0), params["f_min_hz"],
+                              params["df_hz"], params["n_freq"])
+        worst_p = max(worst_p, np.abs(gpu["power"][r] - P).max() / P.max())
+        sf = oracle.spectral_flatness(P, params["k_lo"], params["sf_eps"])
+        y, x = divmod(p, W)
+        worst_sf = max(worst_sf, abs(gpu["sf"][y, x] - sf) / sf)
+        if gu.near(sf, params["tau_sf"]):
+            continue
+        if score_all or sf <= params["tau_sf"]:
+            s, fi, snr, _, _ = oracle.comb_score(P, params)
+            worst_s = max(worst_s, abs(gpu["score"][y, x] - s) / max(s, 1e-30))
+            g = int(gpu["f0_idx"][y, x])
+            assert g == fi or (g >= 0 and abs(snr[g] - snr[fi]) <= gu.REL_TOL * snr[fi])
+            if not gu.near(s, params["tau_comb"]):
+                assert gpu["mask"][y, x] == (sf <= params["tau_sf"] and fi >= 0 and s >= params["tau_comb"])
+        else:
+            assert gpu["score"][y, x] == 0 and gpu["f0_idx"][y, x] == -1 and gpu["mask"][y, x] == 0
+    assert worst_p <= gu.POWER_TOL, worst_p
+    assert worst_sf <= gu.REL_TOL, worst_sf
+    assert worst_s <= gu.REL_TOL, worst_s
+    gu.check_boxes_against_oracle_ccl(gpu, oracle, params["a_min"])
+    # properties that hold at any size
+    inactive = np.ones(params["width"] * params["height"], bool)
+    inactive[act] = False
+    assert np.isnan(gpu["sf"].ravel()[inactive]).all() and not np.isnan(gpu["sf"].ravel()[act]).any()
+    assert (gpu["mask"].ravel()[inactive] == 0).all()
+    dc = np.array([np.where(csr[row_ptr[p]:row_ptr[p + 1]] & 1, 1.0, -1.0).sum() ** 2 for p in act[:2000]])
+    if params["f_min_hz"] == 0:
+        assert np.allclose(gpu["power"][:2000, 0], dc, rtol=1e-4, atol=1e-3)      # P_0 = (sum w)^2
+    return gpu, worst_p, worst_sf, worst_s
+
+
+@pytest.mark.slow
+def test_config3_full_size_sampled(oracle):
+    w = wl.make(3)
+    gpu, wp, wsf, ws = _sampled_compare(oracle, w, w.params, w.events, 0, 400, score_all=False)
+    if w.truth.get("mask") is not None:
+        assert (gpu["mask"].astype(bool) & w.truth["mask"]).sum() >= 0.9 * w.truth["mask"].sum()
+    print(f"cfg3: events {len(w.events)}, active {gpu['n_active']}, scored {gpu['n_scored']}, "
+          f"power {wp:.2e}, sf {wsf:.2e}, score {ws:.2e}, boxes {gpu['n_boxes']}")
+
+
+@pytest.mark.slow
+def test_config4_full_size_sampled(oracle):
+    """BASELINE.json's 1280x720 / 10 M event window in the launch configuration bench.py times."""
+    w = wl.make(4)
+    gpu, wp, wsf, ws = _sampled_compare(oracle, w, w.params, w.events, 0, 300, score_all=False)
+    assert (gpu["mask"].astype(bool) & w.truth["mask"]).sum() >= 0.9 * w.truth["mask"].sum()
+    print(f"cfg4: events {len(w.events)}, active {gpu['n_active']}, scored {gpu['n_scored']}, "
+          f"power {wp:.2e}, sf {wsf:.2e}, score {ws:.2e}, boxes {gpu['n_boxes']}")
+
+
+@pytest.mark.slow
+def test_config5_streaming_windows(oracle):
+    """Sliding windows over one device-resident stream (pointer/length slices)."""
+    w = wl.make(5, n_windows=3)
+    from paper_2603_08386_b200 import binding
+    det = binding.Detector(w.params, max_events=len(w.events), want_power=True)
+    d_ev = det.upload(w.events)
+    for k in (0, 2):
+        lo, n, t0 = w.window_slice(k)
+        det.window(d_ev, n, t0, w.window_us, offset_events=lo)
+        gpu = det.results()
+        ev = w.events[lo:lo + n]
+        row_ptr, csr, dropped = oracle.bucket(ev, w.width, w.height, t0, w.window_us)
+        assert np.array_equal(gpu["row_ptr"], row_ptr) and np.array_equal(gpu["csr_ev"], csr)
+        assert dropped == 0 and gpu["n_dropped"] == 0
+    det.close()
+    lo, n, t0 = w.window_slice(1)
+    _sampled_compare(oracle, w, w.params, w.events[lo:lo + n], t0, 200, score_all=False, seed=1)
