@@ -1,0 +1,318 @@
+#!/usr/bin/env python
+"""bench.py -- DDHF hot path on B200: NDFT Gterms/s and ms per 1280x720 window.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4|cfg5] [--impl reference]
+
+A *step* is one pass of the whole hot path (a0-a8: ingest, NDFT power, spectral flatness, comb
+score, mask, CCL/boxes) over one synthetic window.  Default workload: BASELINE.json config 4
+(1280x720, 100 ms, ~10 M events, 5 % of the pixels hold 60 % of the events) -- the heaviest
+single 1280x720 window; `--workload cfg5` runs the streaming config (sliding 50 ms windows,
+10 ms hop, 50 Mev/s) with one step per window.
+
+Prints ONE JSON line (rank 0).  `value` = (pixel x frequency x event) terms of the active
+pixels per step / device time per step, inputs resident in HBM.  `e2e` = the same through
+ddhf_window_host(): pinned host events in, mask / boxes / counters back to the host, copies
+inside the timed region.  `roofline` is for the fused NDFT+scoring kernel (FP32 ALU bound,
+2 FMA = 4 flop per term); `cpu_baseline` is the float64 oracle timed on this box's host cores
+on a bounded crop of the same window.
+
+N > 1 (torchrun): every rank runs its own replica of the window (the path has no exchange
+step: pixels and windows are independent), scaling = weak, value = sum over ranks / max time.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+NOMINAL_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # 74.45: SMs x FP32 lanes x 2 flop x max SM clock
+FLOP_PER_TERM = 4.0                                        # one complex phasor accumulate = 2 FMA
+
+
+class ClockSampler(threading.Thread):
+    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index = index
+        self.samples: list[list[str]] = []
+        self.stop_flag = threading.Event()
+
+    def run(self):
+        while not self.stop_flag.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True,
+                                     timeout=5).stdout.strip()
+                if out:
+                    self.samples.append([s.strip() for s in out.split(",")])
+            except Exception:
+                pass
+            self.stop_flag.wait(0.1)
+
+    def summary(self) -> dict:
+        mhz = [float(s[0]) for s in self.samples if s and s[0].replace(".", "").isdigit()]
+        mx = [float(s[1]) for s in self.samples if len(s) > 1 and s[1].replace(".", "").isdigit()]
+        pw = [float(s[2]) for s in self.samples if len(s) > 2 and s[2].replace(".", "").isdigit()]
+        reasons = set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for s in self.samples:
+            for name, v in zip(names, s[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(mhz)) if mhz else None,
+                "sm_max_mhz": float(max(mx)) if mx else None,
+                "power_w_max": float(max(pw)) if pw else None,
+                "samples": len(self.samples), "reasons": sorted(reasons)}
+
+
+def load_workload(name: str):
+    from paper_2603_08386_b200 import workloads
+    if name == "cfg4":
+        return workloads.make(4)
+    if name == "cfg5":
+        return workloads.make(5, n_windows=100)
+    if name == "cfg3":
+        return workloads.make(3)
+    if name == "cfg4q":                       # quarter-scale config 4 (for quick checks)
+        return workloads.make(4, scale=0.5)
+    raise SystemExit(f"unknown workload {name}")
+
+
+def window_list(w, steps_needed: int):
+    """(first event, count, t0) for each step."""
+    if w.n_windows == 1:
+        return [(0, len(w.events), w.t0_us)] * steps_needed
+    wins = [w.window_slice(k) for k in range(w.n_windows)]
+    return [wins[i % len(wins)] for i in range(steps_needed)]
+
+
+def terms_of(res, n_freq: int, n_min: int) -> int:
+    cnt = np.diff(res["row_ptr"])
+    return int(cnt[cnt >= max(n_min, 1)].sum()) * n_freq
+
+
+def oracle_sample(w, crop=(320, 180)):
+    """Bounded sample of the workload for the CPU oracle: the top-left crop of the sensor."""
+    cw, ch = min(crop[0], w.width), min(crop[1], w.height)
+    lo, n, t0 = w.window_slice(0) if w.n_windows > 1 else (0, len(w.events), w.t0_us)
+    ev = w.events[lo:lo + n]
+    ev = ev[(ev["x"] < cw) & (ev["y"] < ch)]
+    prm = dict(w.params, width=cw, height=ch)
+    return prm, ev, t0, f"{cw}x{ch} crop (top-left) of the {w.width}x{w.height} window, {len(ev)} events"
+
+
+def time_oracle(w, steps: int, warmup: int):
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import ddhf_oracle
+    prm, ev, t0, what = oracle_sample(w)
+    times, terms = [], 0
+    for i in range(warmup + steps):
+        t = time.perf_counter()
+        out = ddhf_oracle.window(prm, ev, t0, w.window_us, want_power=False)
+        dt = time.perf_counter() - t
+        if i >= warmup:
+            times.append(dt)
+        terms = terms_of(out, prm["n_freq"], prm["n_min"])
+    return dict(value=terms / np.mean(times) / 1e9, unit="Gterms/s", cores=ddhf_oracle.num_threads(),
+                kind="oracle", sample=what, ms_per_step=float(np.mean(times) * 1e3), terms_per_step=terms)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg4")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--score-all", action="store_true", help="comb score on every active pixel (R14)")
+    ap.add_argument("--spectra", action="store_true", help="also write the compact power spectra to HBM")
+    args = ap.parse_args()
+    steps, warmup = max(args.steps, 1), max(args.warmup, 3 if args.impl == "ours" else 0)
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        # The oracle, as it stands, on this box's host cores.  Rank 0 only.
+        if rank != 0:
+            return
+        w = load_workload(args.workload)
+        r = time_oracle(w, min(steps, 3), min(warmup, 1))
+        line = {"impl": "reference", "metric": "ndft_gterms_per_s", "value": r["value"], "unit": "Gterms/s",
+                "n_gpus": args.gpus, "steps": min(steps, 3), "warmup": min(warmup, 1),
+                "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": f"{args.workload} ({r['sample']})", "terms_per_step": r["terms_per_step"]},
+                "cpu_baseline": {"value": r["value"], "unit": "Gterms/s", "cores": r["cores"],
+                                 "kind": "oracle", "sample": r["sample"]},
+                "e2e": {"value": r["value"], "unit": "Gterms/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+                "gpu_launches": 0}
+        print(json.dumps(line))
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2603_08386_b200 import binding
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the DDHF path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    w = load_workload(args.workload)
+    prm = w.params
+    det = binding.Detector(prm, max_events=len(w.events), score_all=args.score_all, timing=True,
+                           want_power=args.spectra, want_labels=False, device=f"cuda:{local_rank}",
+                           max_active=(prm["width"] * prm["height"]) if args.spectra else 1)
+    d_ev = det.upload(w.events)
+    wins = window_list(w, warmup + steps)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # one untimed pass to count the terms of every distinct window (device counters only tell
+    # events and pixels; the term count needs the row lengths)
+    terms_by_win = {}
+    for lo, n, t0 in dict.fromkeys(wins):
+        det.window(d_ev, n, t0, w.window_us, offset_events=lo)
+        res = det.results()
+        terms_by_win[(lo, n, t0)] = (terms_of(res, prm["n_freq"], prm["n_min"]), res)
+    launches_per_window = binding.ddhf_launches_per_window(det.h)
+
+    # ---- device-resident timing ---------------------------------------------------------------
+    for lo, n, t0 in wins[:warmup]:
+        det.window(d_ev, n, t0, w.window_us, offset_events=lo)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    ev0 = torch.cuda.Event(enable_timing=True)
+    ev1 = torch.cuda.Event(enable_timing=True)
+    per_step_ms, stage = [], []
+    ev0.record()
+    for lo, n, t0 in wins[warmup:]:
+        det.window(d_ev, n, t0, w.window_us, offset_events=lo)
+    ev1.record()
+    barrier()
+    total_ms = ev0.elapsed_time(ev1)
+    # per-step latency and per-stage split: a second timed pass with a sync per window
+    for lo, n, t0 in wins[warmup:]:
+        det.window(d_ev, n, t0, w.window_us, offset_events=lo)
+        ms = det.stage_ms()
+        stage.append(ms)
+        per_step_ms.append(ms[3])
+    sampler.stop_flag.set()
+    sampler.join()
+    stage = np.array(stage)
+    terms_total = sum(terms_by_win[k][0] for k in wins[warmup:])
+    if world > 1:
+        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+        tt = torch.tensor([terms_total], device=dev, dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.SUM)
+        terms_all = float(tt.item())
+    else:
+        terms_all = float(terms_total)
+    value = terms_all / (total_ms * 1e-3) / 1e9
+
+    # ---- end to end through the host-buffer entry point -------------------------------------------
+    NP = prm["width"] * prm["height"]
+    h_ev = torch.from_numpy(np.ascontiguousarray(w.events).view(np.uint8).copy()).pin_memory()
+    h_mask = torch.zeros(NP, dtype=torch.uint8).pin_memory()
+    h_boxes = torch.zeros(det.cfg.max_boxes * 6, dtype=torch.int32).pin_memory()
+    h_cnt = torch.zeros(8, dtype=torch.int32).pin_memory()
+    hout = binding.DdhfHostOutputs()
+    hout.mask, hout.boxes, hout.counters = h_mask.data_ptr(), h_boxes.data_ptr(), h_cnt.data_ptr()
+    st = torch.cuda.current_stream(dev).cuda_stream
+    e2e_steps = min(steps, 10)
+    for lo, n, t0 in wins[:2]:
+        binding.ddhf_window_host(det.h, h_ev.data_ptr() + 16 * lo, n, t0, w.window_us, hout, st)
+    barrier()
+    t_start = time.perf_counter()
+    h2d = 0
+    for lo, n, t0 in wins[warmup:warmup + e2e_steps]:
+        binding.ddhf_window_host(det.h, h_ev.data_ptr() + 16 * lo, n, t0, w.window_us, hout, st)
+        h2d += 16 * n
+    barrier()
+    e2e_s = time.perf_counter() - t_start
+    e2e_terms = sum(terms_by_win[k][0] for k in wins[warmup:warmup + e2e_steps])
+    if world > 1:
+        t = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+        e2e_terms *= world
+    d2h = NP + 32 + 24 * int(h_cnt[3])
+    e2e = {"value": e2e_terms / e2e_s / 1e9, "unit": "Gterms/s", "ms_per_step": e2e_s / e2e_steps * 1e3,
+           "h2d_bytes_per_step": h2d // e2e_steps, "d2h_bytes_per_step": d2h, "steps": e2e_steps}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (fused NDFT + scoring), measured live -------------------
+    ndft_ms = float(stage[:, 1].mean())
+    terms_per_step = terms_total / len(wins[warmup:])
+    achieved = terms_per_step * FLOP_PER_TERM / (ndft_ms * 1e-3) / 1e12
+    probe = binding.ddhf_fma_peak_probe(20.0)
+    roofline = {"bound": "alu", "kernel": "k_ndft_score", "achieved": achieved, "peak": NOMINAL_FP32_TFLOPS,
+                "unit": "TFLOP/s", "frac": achieved / NOMINAL_FP32_TFLOPS, "traffic": None,
+                "peak_kind": "nominal FP32 FMA: 148 SM x 128 lanes x 2 flop x 1.965 GHz (DESIGN.md section 5)",
+                "flop_per_term": FLOP_PER_TERM, "kernel_ms": ndft_ms,
+                "gterms_per_s_kernel": terms_per_step / (ndft_ms * 1e-3) / 1e9,
+                "measured_fma_peak_tflops": {"ffma": probe[0], "ffma2": probe[1]},
+                "frac_of_measured_fma_peak": achieved / max(probe)}
+    res0 = terms_by_win[wins[warmup]][1]
+    line = {
+        "metric": "ndft_gterms_per_s", "value": value, "unit": "Gterms/s", "n_gpus": world,
+        "steps": steps, "warmup": warmup, "ms_per_step": total_ms / steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"{args.workload}: {prm['width']}x{prm['height']} sensor, "
+                               f"{w.window_us / 1e3:.0f} ms window, {res0['n_in']} events, "
+                               f"{prm['n_freq']} bins, {prm['n_f0']} f0 candidates, H={prm['n_harm']}, "
+                               f"n_min={prm['n_min']}",
+                   "events_per_step": res0["n_in"], "active_pixels": res0["n_active"],
+                   "scored_pixels": res0["n_scored"], "terms_per_step": terms_per_step,
+                   "mask_pixels": int(res0["mask"].sum()), "boxes": res0["n_boxes"],
+                   "score_all": bool(args.score_all), "spectra_to_hbm": bool(args.spectra),
+                   "l2": "inputs larger than L2 (events %.0f MB + pairs + csr per step)" % (16 * res0["n_in"] / 1e6),
+                   "replicas": world},
+        "latency_ms": {"p50": float(np.percentile(per_step_ms, 50)), "p99": float(np.percentile(per_step_ms, 99)),
+                       "ingest": float(stage[:, 0].mean()), "ndft_score": ndft_ms, "ccl": float(stage[:, 2].mean())},
+        "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": launches_per_window * steps,
+        "roofline": roofline,
+        "paper_context": "DDHF 2.39 ms/frame, YOLOv11-n 12.40 ms/frame on an NVIDIA L40-8Q, 33.3 ms windows (PAPER.md L154-156)",
+    }
+    if not args.no_cpu_baseline:
+        r = time_oracle(w, 1, 0)
+        line["cpu_baseline"] = {"value": r["value"], "unit": "Gterms/s", "cores": r["cores"], "kind": "oracle",
+                                "sample": r["sample"], "ms": r["ms_per_step"]}
+    print(json.dumps(line))
+    det.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -101,7 +101,7 @@ def test_grid_shapes(oracle, nf, klo, fmin):
 
 def test_capacity_truncation(oracle):
     w = wl.make(1)
-    prm = dict(w.params, n_min=1, a_min=1, tau_sf=1.0, tau_comb=0.0)    # everything is a detection
+    prm = dict(w.params, n_min=1, a_min=1, tau_sf=2.0, tau_comb=0.0)    # every active pixel is a detection
     orc = oracle.window(prm, w.events, 0, w.window_us, score_all=True, max_boxes=1 << 16)
     gpu = gu.run_gpu(prm, w.events, 0, w.window_us, score_all=True, max_active=100, max_boxes=5)
     assert gpu["overflow"] == 3
