@@ -26,7 +26,7 @@ struct ddhf_handle {
     uint64_t g_f0 = 0, g_d = 0, g_h = 0;
     CandTable *d_cand = nullptr;
     // workspace offsets (bytes)
-    size_t off_cnt = 0, off_pairs = 0, off_work = 0, off_tiles = 0, off_class = 0, off_cursor = 0,
+    size_t off_cnt = 0, off_pairs = 0, off_work = 0, off_tiles = 0, off_class = 0, off_cursor = 0, off_long = 0,
            off_parent = 0, off_slot = 0, off_comp = 0, off_comp_label = 0, off_ctiles = 0, ws_bytes = 0;
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     bool timed_once = false;
@@ -166,6 +166,7 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
     h->off_tiles = o;      o = align_up(o + sizeof(int32_t) * 4 * 1024);
     h->off_class = o;      o = align_up(o + sizeof(int32_t) * 2 * kNumClasses);
     h->off_cursor = o;     o = align_up(o + 256);
+    h->off_long = o;       o = align_up(o + sizeof(int32_t) * h->np);
     h->off_parent = o;     o = align_up(o + sizeof(int32_t) * h->np);
     h->off_slot = o;       o = align_up(o + sizeof(int32_t) * h->np);
     h->off_comp = o;       o = align_up(o + sizeof(int32_t) * 5 * static_cast<size_t>(h->comp_cap));
@@ -217,6 +218,8 @@ extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n
     ip.counters = out->counters;
     ip.sf = out->sf; ip.score = out->score; ip.f0_idx = out->f0_idx; ip.mask = out->mask;
     ip.work_cursor = reinterpret_cast<int32_t *>(ws + h->off_cursor);
+    ip.n_long = ip.work_cursor + 1;
+    ip.long_rows = reinterpret_cast<int32_t *>(ws + h->off_long);
 
     NdftParams np{};
     np.work = ip.work; np.csr_ev = out->csr_ev; np.counters = out->counters;

@@ -17,10 +17,13 @@ constexpr int kTile = 4096;      // 1024 threads x 4
 
 __device__ __forceinline__ int uf_find(int *parent, int x)
 {
+    // find with path halving; parent[] only ever decreases, so concurrent halving is safe
     int p = *reinterpret_cast<volatile int *>(parent + x);
     while (p != x) {
+        const int gp = *reinterpret_cast<volatile int *>(parent + p);
+        if (gp != p) atomicMin(parent + x, gp);
         x = p;
-        p = *reinterpret_cast<volatile int *>(parent + x);
+        p = gp;
     }
     return x;
 }
@@ -38,10 +41,18 @@ __device__ __forceinline__ void uf_union(int *parent, int a, int b)
     }
 }
 
+// Every mask pixel starts as a child of the first pixel of its horizontal run inside the
+// warp's 32-pixel span (runs are cut at row starts), so the union-find trees start flat.
 __global__ void k_ccl_init(CclParams p)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i < p.np) p.parent[i] = p.mask[i] ? i : -1;
+    const int lane = threadIdx.x & 31;
+    const bool m = (i < p.np) && p.mask[i];
+    const unsigned bits = __ballot_sync(0xffffffffu, m);
+    const unsigned rs = __ballot_sync(0xffffffffu, (i % p.width) == 0);
+    const unsigned starts = bits & (~(bits << 1) | rs | 1u);
+    const unsigned upto = starts & (0xffffffffu >> (31 - lane));
+    if (i < p.np) p.parent[i] = m ? i - (lane - (31 - __clz(upto))) : -1;
 }
 
 __global__ void k_ccl_merge(CclParams p)
@@ -49,13 +60,16 @@ __global__ void k_ccl_merge(CclParams p)
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= p.np || !p.mask[i]) return;
     const int x = i % p.width, y = i / p.width;
-    // the four neighbours that precede i in raster order (W, NW, N, NE)
-    if (x > 0 && p.mask[i - 1]) uf_union(p.parent, i, i - 1);
+    // W: only where a run was cut at a span boundary
+    if (x > 0 && p.mask[i - 1] && (threadIdx.x & 31) == 0) uf_union(p.parent, i, i - 1);
     if (y > 0) {
         const int up = i - p.width;
-        if (x > 0 && p.mask[up - 1]) uf_union(p.parent, i, up - 1);
-        if (p.mask[up]) uf_union(p.parent, i, up);
-        if (x + 1 < p.width && p.mask[up + 1]) uf_union(p.parent, i, up + 1);
+        if (p.mask[up]) {
+            uf_union(p.parent, i, up);                    // N (NW and NE are then in N's run)
+        } else {
+            if (x > 0 && p.mask[up - 1]) uf_union(p.parent, i, up - 1);             // NW
+            if (x + 1 < p.width && p.mask[up + 1]) uf_union(p.parent, i, up + 1);   // NE
+        }
     }
 }
 

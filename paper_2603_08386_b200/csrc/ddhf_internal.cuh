@@ -78,6 +78,8 @@ struct IngestParams {
     int32_t *f0_idx;
     uint8_t *mask;
     int32_t *work_cursor;
+    int32_t *long_rows;          // [np] pixels whose row is longer than the short-row limit
+    int32_t *n_long;
 };
 
 struct CclParams {

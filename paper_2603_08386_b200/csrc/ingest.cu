@@ -18,8 +18,10 @@ namespace {
 
 constexpr int kEvThreads = 256;
 constexpr int kEvUnroll = 4;
-constexpr int kRowPix = 128;       // pixels per k_rowsort block
-constexpr int kRowCap = 4096;      // pairs staged in shared memory per k_rowsort block
+constexpr int kRowPix = 128;       // pixels per k_rowsort_short block
+constexpr int kRowCap = 4096;      // pairs staged in shared memory per block
+constexpr int kShortMax = 64;      // rows up to this length are ranked by counting
+constexpr int kLongBlocks = 148 * 6;
 
 struct Ev {
     int32_t pix;       // -1 if dropped
@@ -67,7 +69,7 @@ __global__ void k_init(IngestParams p)
             p.class_cnt[threadIdx.x] = 0;
             p.class_cur[threadIdx.x] = 0;
         }
-        if (threadIdx.x == 0) *p.work_cursor = 0;
+        if (threadIdx.x == 0) { *p.work_cursor = 0; *p.n_long = 0; }
     }
 }
 
@@ -205,29 +207,34 @@ __global__ void __launch_bounds__(1024) k_scan_apply(IngestParams p)
 {
     __shared__ int s_a[33], s_b[33];
     __shared__ int s_cls[kNumClasses], s_base[kNumClasses];
+    __shared__ int s_nlong, s_longbase;
     if (threadIdx.x < kNumClasses) s_cls[threadIdx.x] = 0;
+    if (threadIdx.x == 0) s_nlong = 0;
     __syncthreads();
     const int base = blockIdx.x * kScanTile + threadIdx.x * 4;
     int v[4];
     load4(p.cnt, base, p.np, v);
     const int nmin = max(p.n_min, 1);
     int sum = 0, act = 0;
-    int lrank[4];
+    int lrank[4], llong[4];
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         sum += v[j];
         lrank[j] = -1;
+        llong[j] = -1;
         if (v[j] >= nmin) {
             ++act;
             lrank[j] = atomicAdd(&s_cls[size_class(v[j])], 1);
         }
+        if (v[j] > kShortMax) llong[j] = atomicAdd(&s_nlong, 1);
     }
     int ta, tb;
-    block_scan2(sum, act, ta, tb, s_a, s_b);       // contains __syncthreads: s_cls is final
+    block_scan2(sum, act, ta, tb, s_a, s_b);       // contains __syncthreads: s_cls, s_nlong are final
     if (threadIdx.x < kNumClasses) {
         const int n = s_cls[threadIdx.x];
         s_base[threadIdx.x] = p.class_cnt[threadIdx.x] + (n ? atomicAdd(&p.class_cur[threadIdx.x], n) : 0);
     }
+    if (threadIdx.x == 32) s_longbase = s_nlong ? atomicAdd(p.n_long, s_nlong) : 0;
     __syncthreads();
     int off = p.tile_off[blockIdx.x] + sum;
     int aoff = p.tile_aoff[blockIdx.x] + act;
@@ -237,6 +244,7 @@ __global__ void __launch_bounds__(1024) k_scan_apply(IngestParams p)
         if (pix < p.np) {
             p.row_ptr[pix] = off;
             p.cnt[pix] = 0;
+            if (llong[j] >= 0) p.long_rows[s_longbase + llong[j]] = pix;
             if (lrank[j] >= 0) {
                 if (aoff < p.max_active) p.active_idx[aoff] = pix;
                 WorkItem it;
@@ -273,11 +281,13 @@ __global__ void __launch_bounds__(kEvThreads) k_scatter(IngestParams p)
     }
 }
 
-// ---- k_rowsort: restore input order inside every row (a3, R20) --------------------------
-// A block owns kRowPix consecutive pixels, i.e. one contiguous span of slots.  Every element
-// finds its row by binary search over the block's row starts and its rank inside the row by
-// counting the elements of the row with a smaller input index.
-__global__ void __launch_bounds__(256) k_rowsort(IngestParams p)
+// ---- row sort: restore input order inside every row (a3, R20) ---------------------------
+// Short rows (<= kShortMax events): a block owns kRowPix consecutive pixels, i.e. one
+// contiguous span of slots; every element finds its row by binary search over the block's
+// row starts and its rank inside the row by counting the elements of the row with a smaller
+// input index.  Long rows are listed by k_scan_apply and sorted one per block (bitonic sort
+// in shared memory) by k_rowsort_long.
+__global__ void __launch_bounds__(256) k_rowsort_short(IngestParams p)
 {
     __shared__ int s_rp[kRowPix + 1];
     __shared__ uint64_t s_pair[kRowCap];
@@ -293,13 +303,13 @@ __global__ void __launch_bounds__(256) k_rowsort(IngestParams p)
         __syncthreads();
     }
     for (int s = threadIdx.x; s < tot; s += blockDim.x) {
-        // row = last r with s_rp[r] - beg <= s
-        int lo = 0, hi = npx;
+        int lo = 0, hi = npx;                              // row = last r with s_rp[r] - beg <= s
         while (hi - lo > 1) {
             const int mid = (lo + hi) >> 1;
             if (s_rp[mid] - beg <= s) lo = mid; else hi = mid;
         }
         const int rb = s_rp[lo] - beg, re = s_rp[lo + 1] - beg;
+        if (re - rb > kShortMax) continue;                 // k_rowsort_long's
         int rank = 0;
         uint64_t mine;
         if (staged) {
@@ -310,6 +320,46 @@ __global__ void __launch_bounds__(256) k_rowsort(IngestParams p)
             for (int j = rb; j < re; ++j) rank += (p.pairs[beg + j] < mine);
         }
         p.csr_ev[beg + rb + rank] = static_cast<uint32_t>(mine);
+    }
+}
+
+__global__ void __launch_bounds__(256) k_rowsort_long(IngestParams p)
+{
+    __shared__ uint64_t s_key[kRowCap];
+    const int n_long = *p.n_long;
+    for (int r = blockIdx.x; r < n_long; r += gridDim.x) {
+        const int pix = p.long_rows[r];
+        const int beg = p.row_ptr[pix], n = p.row_ptr[pix + 1] - beg;
+        if (n <= kRowCap) {
+            int np2 = 1;
+            while (np2 < n) np2 <<= 1;
+            for (int i = threadIdx.x; i < np2; i += blockDim.x)
+                s_key[i] = (i < n) ? p.pairs[beg + i] : ~0ull;
+            __syncthreads();
+            for (int k = 2; k <= np2; k <<= 1) {
+                for (int j = k >> 1; j > 0; j >>= 1) {
+                    for (int t = threadIdx.x; t < (np2 >> 1); t += blockDim.x) {
+                        const int lo = ((t & ~(j - 1)) << 1) | (t & (j - 1));    // index with bit j clear
+                        const int hi = lo | j;
+                        const bool asc = (lo & k) == 0;
+                        const uint64_t a = s_key[lo], b = s_key[hi];
+                        if ((a > b) == asc) { s_key[lo] = b; s_key[hi] = a; }
+                    }
+                    __syncthreads();
+                }
+            }
+            for (int i = threadIdx.x; i < n; i += blockDim.x)
+                p.csr_ev[beg + i] = static_cast<uint32_t>(s_key[i]);
+            __syncthreads();
+        } else {
+            // very long row (thousands of events on one pixel): rank by counting from global memory
+            for (int s = threadIdx.x; s < n; s += blockDim.x) {
+                const uint64_t mine = p.pairs[beg + s];
+                int rank = 0;
+                for (int j = 0; j < n; ++j) rank += (p.pairs[beg + j] < mine);
+                p.csr_ev[beg + rank] = static_cast<uint32_t>(mine);
+            }
+        }
     }
 }
 
@@ -327,7 +377,8 @@ int launch_ingest(const IngestParams &p, cudaStream_t st)
     k_scan_apply<<<n_tiles, 1024, 0, st>>>(p); ++launches;
     if (ev_blocks > 0) {
         k_scatter<<<ev_blocks, kEvThreads, 0, st>>>(p); ++launches;
-        k_rowsort<<<(p.np + kRowPix - 1) / kRowPix, 256, 0, st>>>(p); ++launches;
+        k_rowsort_short<<<(p.np + kRowPix - 1) / kRowPix, 256, 0, st>>>(p); ++launches;
+        k_rowsort_long<<<kLongBlocks, 256, 0, st>>>(p); ++launches;
     }
     return launches;
 }

@@ -76,6 +76,13 @@ __device__ __forceinline__ void sincos_u32(uint32_t ph, float &s, float &c)
 
 __device__ __forceinline__ int pad(int j) { return j + (j >> 5); }
 
+__device__ __forceinline__ WorkItem make_item()
+{
+    WorkItem w;
+    w.row_begin = 0; w.n = 0; w.pix = 0; w.arow = 0;
+    return w;
+}
+
 template <int E>
 __device__ __forceinline__ void bitonic_sort_regs(float (&x)[E], int lane)
 {
@@ -400,13 +407,25 @@ __global__ void __launch_bounds__(kWarps * 32, 3) k_ndft_score(NdftParams p)
     const int n_items = p.counters[DDHF_CNT_N_ACTIVE];
     const ScoreParams &sp = p.sp;
     constexpr int EPP = 32 / TN;       // events per table pass
+    const bool full_grid = (sp.n_freq == L::NB) && (sp.k_lo <= 32);
+    const bool store_power = p.power != nullptr;
 
-    while (true) {
-        int idx = 0;
-        if (lane == 0) idx = atomicAdd(p.work_cursor, 1);
-        idx = __shfl_sync(kFull, idx, 0);
-        if (idx >= n_items) break;
-        const WorkItem it = p.work[idx];
+    // dynamic work queue with one item of look-ahead: the next index is fetched while the
+    // current pixel is being processed, so the atomic's latency is off the critical path
+    int idx = 0;
+    if (lane == 0) idx = atomicAdd(p.work_cursor, 1);
+    idx = __shfl_sync(kFull, idx, 0);
+    WorkItem it_next = make_item();
+    uint32_t v_first = 0u;
+    if (idx < n_items) {
+        it_next = p.work[idx];
+        if (lane < kEC && lane < it_next.n) v_first = __ldg(p.csr_ev + it_next.row_begin + lane);
+    }
+
+    while (idx < n_items) {
+        const WorkItem it = it_next;
+        int next_idx = 0;
+        if (lane == 0) next_idx = atomicAdd(p.work_cursor, 1);
 
         float2 acc1[TM][TN], acc2[TM][TN];     // (S1, S4) and (S3, S2)
 #pragma unroll
@@ -417,26 +436,31 @@ __global__ void __launch_bounds__(kWarps * 32, 3) k_ndft_score(NdftParams p)
                 acc2[g][m] = make_float2(0.f, 0.f);
             }
 
+        uint32_t v_next = v_first;
         for (int base = 0; base < it.n; base += kEC) {
             const int nc = min(kEC, it.n - base);
             // ---- per-event phase words and the offset-phasor table of this chunk ----------
-            uint32_t v = 0, hph = 0;
+            const uint32_t v = v_next;
+            if (base + kEC + lane < it.n && lane < kEC)           // prefetch the next chunk
+                v_next = __ldg(p.csr_ev + it.row_begin + base + kEC + lane);
+            uint32_t hph = 0;
             if (lane < nc) {
-                v = __ldg(p.csr_ev + it.row_begin + base + lane);
                 const uint32_t t = v >> 1;
                 hph = phase_u32(p.g_h, t);
                 phs[lane] = make_uint4(phase_u32(p.g_f0, t), phase_u32(p.g_d, t), hph, 0u);
             }
-#pragma unroll
-            for (int ps = 0; ps < kEC / EPP; ++ps) {
+            const int n_pass = (nc + EPP - 1) / EPP;
+#pragma unroll 1
+            for (int ps = 0; ps < n_pass; ++ps) {
                 const int e = ps * EPP + lane / TN, m = lane % TN;
                 const uint32_t ve = __shfl_sync(kFull, v, e);
                 const uint32_t he = __shfl_sync(kFull, hph, e);
                 float s, c;
                 sincos_u32(he * static_cast<uint32_t>(2 * m + 1), s, c);
                 // b = w (cos, -sin) up to the common sign; w = +1 if bit 0 else -1
-                const float w = (ve & 1u) ? 1.f : -1.f;
-                btab[e * TN + m] = (e < nc) ? make_float2(w * c, -w * s) : make_float2(0.f, 0.f);
+                const uint32_t sgn = (ve & 1u) ? 0u : 0x80000000u;
+                btab[e * TN + m] = make_float2(__uint_as_float(__float_as_uint(c) ^ sgn),
+                                               __uint_as_float(__float_as_uint(s) ^ sgn ^ 0x80000000u));
             }
             __syncwarp();
             // ---- accumulate: 4 real products per (centre, offset pair, event) --------------
@@ -470,7 +494,11 @@ __global__ void __launch_bounds__(kWarps * 32, 3) k_ndft_score(NdftParams p)
             __syncwarp();
         }
 
-        // ---- epilogue: powers, spectrum store, spectral flatness ---------------------------
+        // the next pixel's work item and first events are fetched under the epilogue
+        idx = __shfl_sync(kFull, next_idx, 0);
+        if (idx < n_items) it_next = p.work[idx];
+
+        // ---- epilogue: powers, optional spectrum store, spectral flatness -------------------
         float preg[NBL];
 #pragma unroll
         for (int g = 0; g < TM; ++g)
@@ -483,15 +511,32 @@ __global__ void __launch_bounds__(kWarps * 32, 3) k_ndft_score(NdftParams p)
                 preg[g * 2 * TN + TN - 1 - m] = rm * rm + im * im;
             }
         const bool has_row = it.arow < p.max_active;
-        float slog = 0.f, ssum = 0.f;
+        if (store_power && has_row) {
+            float *dst = p.power + static_cast<size_t>(it.arow) * sp.n_freq + lane;
 #pragma unroll
-        for (int i = 0; i < NBL; ++i) {
-            const int j = i * 32 + lane;
-            P_s[i * 33 + lane] = preg[i];                       // == pad(j)
-            if (j < sp.n_freq) {
-                if (p.power != nullptr && has_row)
-                    __stcs(p.power + static_cast<size_t>(it.arow) * sp.n_freq + j, preg[i]);
-                if (j >= sp.k_lo) {
+            for (int i = 0; i < NBL; ++i)
+                if (i * 32 + lane < sp.n_freq) __stcs(dst + i * 32, preg[i]);
+        }
+        float slog = 0.f, ssum = 0.f;
+        if (full_grid) {
+            // every bin is in range; only the first k_lo bins (register 0) are left out
+            {
+                const float pt = fmaxf(preg[0], sp.sf_eps);
+                const bool in = lane >= sp.k_lo;
+                slog = in ? __log2f(pt) : 0.f;
+                ssum = in ? pt : 0.f;
+            }
+#pragma unroll
+            for (int i = 1; i < NBL; ++i) {
+                const float pt = fmaxf(preg[i], sp.sf_eps);
+                slog += __log2f(pt);
+                ssum += pt;
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < NBL; ++i) {
+                const int j = i * 32 + lane;
+                if (j >= sp.k_lo && j < sp.n_freq) {
                     const float pt = fmaxf(preg[i], sp.sf_eps);
                     slog += __log2f(pt);
                     ssum += pt;
@@ -503,15 +548,20 @@ __global__ void __launch_bounds__(kWarps * 32, 3) k_ndft_score(NdftParams p)
             slog += __shfl_xor_sync(kFull, slog, o);
             ssum += __shfl_xor_sync(kFull, ssum, o);
         }
+        v_first = 0u;
+        if (idx < n_items && lane < kEC && lane < it_next.n)
+            v_first = __ldg(p.csr_ev + it_next.row_begin + lane);
         const float inv_nb = 1.f / static_cast<float>(sp.n_freq - sp.k_lo);
         const float mean_p = ssum * inv_nb;
         const float sfv = exp2f(slog * inv_nb) / mean_p;         // eq. 7
         const bool sf_ok = sfv <= sp.tau_sf;                     // discard if SF > tau_sf (L107)
-        __syncwarp();
 
         float score = 0.f;
         int f0 = -1;
         if (sp.score_all || sf_ok) {
+#pragma unroll
+            for (int i = 0; i < NBL; ++i) P_s[i * 33 + lane] = preg[i];        // == pad(32 i + lane)
+            __syncwarp();
             float *dbg = (p.comb_debug != nullptr && has_row)
                              ? p.comb_debug + static_cast<size_t>(it.arow) * sp.n_f0 * 3 : nullptr;
             comb_score<TM, TN, BS>(preg, P_s, scr, sp, mean_p, lane, score, f0, dbg);
