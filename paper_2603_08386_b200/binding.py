@@ -13,7 +13,7 @@ from typing import Any
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libddhf.so")
+LIB_PATH = os.environ.get("DDHF_LIB", os.path.join(_HERE, "libddhf.so"))
 
 DDHF_OK, DDHF_E_INVAL, DDHF_E_CAPACITY, DDHF_E_CUDA, DDHF_E_NOMEM = 0, -1, -2, -3, -4
 DDHF_FLAG_SCORE_ALL, DDHF_FLAG_TIMING = 1, 2

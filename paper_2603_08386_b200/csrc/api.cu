@@ -217,8 +217,8 @@ extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n
     ip.class_cur = ip.class_cnt + kNumClasses;
     ip.counters = out->counters;
     ip.sf = out->sf; ip.score = out->score; ip.f0_idx = out->f0_idx; ip.mask = out->mask;
-    ip.work_cursor = reinterpret_cast<int32_t *>(ws + h->off_cursor);
-    ip.n_long = ip.work_cursor + 1;
+    ip.work_cursor = reinterpret_cast<unsigned long long *>(ws + h->off_cursor);
+    ip.n_long = reinterpret_cast<int32_t *>(ws + h->off_cursor + 16);
     ip.long_rows = reinterpret_cast<int32_t *>(ws + h->off_long);
 
     NdftParams np{};

@@ -45,7 +45,7 @@ struct NdftParams {
     const WorkItem *work;        // DEVICE [n_active] ordered by descending size class
     const uint32_t *csr_ev;
     const int32_t *counters;     // n_active is read from here (device side)
-    int32_t *work_cursor;        // dynamic work queue head
+    unsigned long long *work_cursor;   // dynamic work queue: items taken from the head (hi 32) / tail (lo 32)
     int32_t max_active;
     uint64_t g_f0, g_d, g_h;     // 2^64 * f * 1e-6 for: centre base, df, 16*df
     float *power;                // optional compact spectra
@@ -77,7 +77,7 @@ struct IngestParams {
     float *sf, *score;           // per-pixel maps initialised for inactive pixels
     int32_t *f0_idx;
     uint8_t *mask;
-    int32_t *work_cursor;
+    unsigned long long *work_cursor;
     int32_t *long_rows;          // [np] pixels whose row is longer than the short-row limit
     int32_t *n_long;
 };

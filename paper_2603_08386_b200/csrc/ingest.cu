@@ -69,7 +69,7 @@ __global__ void k_init(IngestParams p)
             p.class_cnt[threadIdx.x] = 0;
             p.class_cur[threadIdx.x] = 0;
         }
-        if (threadIdx.x == 0) { *p.work_cursor = 0; *p.n_long = 0; }
+        if (threadIdx.x == 0) { *p.work_cursor = 0ull; *p.n_long = 0; }
     }
 }
 

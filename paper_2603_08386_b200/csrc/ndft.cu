@@ -34,7 +34,16 @@ namespace ddhf {
 
 namespace {
 
-constexpr int kWarps = 4;          // warps per CTA
+#ifndef DDHF_NDFT_WARPS
+#define DDHF_NDFT_WARPS 12         // warps per CTA: 12 x 32 threads x 168 registers fill the 64 K register file
+#endif
+#ifndef DDHF_NDFT_HEAD_WARPS
+#define DDHF_NDFT_HEAD_WARPS 2     // of every 3 warps, how many start from the long-row end of the work list
+#endif
+#ifndef DDHF_NDFT_BLOCKS
+#define DDHF_NDFT_BLOCKS 1         // CTAs per SM
+#endif
+constexpr int kWarps = DDHF_NDFT_WARPS;
 constexpr int kEC = 16;            // events per table chunk
 constexpr unsigned kFull = 0xffffffffu;
 constexpr uint32_t kInvalidKey = 0x7fffffffu;
@@ -75,6 +84,19 @@ __device__ __forceinline__ void sincos_u32(uint32_t ph, float &s, float &c)
 }
 
 __device__ __forceinline__ int pad(int j) { return j + (j >> 5); }
+
+// The work list is ordered by descending row length.  Warps take items from both ends: "head"
+// warps the long rows (FMA-pipe bound), "tail" warps the short ones (dominated by the
+// per-pixel epilogue, latency bound), so that every SM sub-partition always holds a mix of
+// the two and neither the FMA pipe nor the issue slots sit idle for a whole phase of the
+// kernel.  One 64-bit counter holds both cursors; an item is valid while head + tail < n.
+__device__ __forceinline__ int fetch_item(unsigned long long *cursor, bool head, int n_items)
+{
+    const unsigned long long old = atomicAdd(cursor, head ? (1ull << 32) : 1ull);
+    const unsigned h = static_cast<unsigned>(old >> 32), t = static_cast<unsigned>(old);
+    if (h + t >= static_cast<unsigned>(n_items)) return n_items;
+    return head ? static_cast<int>(h) : n_items - 1 - static_cast<int>(t);
+}
 
 __device__ __forceinline__ WorkItem make_item()
 {
@@ -392,7 +414,7 @@ __device__ __forceinline__ void comb_score(float (&preg)[TM * 2 * TN], const flo
 // The fused kernel.
 // ----------------------------------------------------------------------------------------
 template <int TM, int TN, int BS>
-__global__ void __launch_bounds__(kWarps * 32, 3) k_ndft_score(NdftParams p)
+__global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(NdftParams p)
 {
     using L = Layout<TM, TN, BS>;
     constexpr int NBL = L::NBL;
@@ -412,8 +434,9 @@ __global__ void __launch_bounds__(kWarps * 32, 3) k_ndft_score(NdftParams p)
 
     // dynamic work queue with one item of look-ahead: the next index is fetched while the
     // current pixel is being processed, so the atomic's latency is off the critical path
+    const bool head = (wid % 3) < DDHF_NDFT_HEAD_WARPS;
     int idx = 0;
-    if (lane == 0) idx = atomicAdd(p.work_cursor, 1);
+    if (lane == 0) idx = fetch_item(p.work_cursor, head, n_items);
     idx = __shfl_sync(kFull, idx, 0);
     WorkItem it_next = make_item();
     uint32_t v_first = 0u;
@@ -425,7 +448,7 @@ __global__ void __launch_bounds__(kWarps * 32, 3) k_ndft_score(NdftParams p)
     while (idx < n_items) {
         const WorkItem it = it_next;
         int next_idx = 0;
-        if (lane == 0) next_idx = atomicAdd(p.work_cursor, 1);
+        if (lane == 0) next_idx = fetch_item(p.work_cursor, head, n_items);
 
         float2 acc1[TM][TN], acc2[TM][TN];     // (S1, S4) and (S3, S2)
 #pragma unroll
@@ -464,18 +487,33 @@ __global__ void __launch_bounds__(kWarps * 32, 3) k_ndft_score(NdftParams p)
             }
             __syncwarp();
             // ---- accumulate: 4 real products per (centre, offset pair, event) --------------
-#pragma unroll 1
-            for (int k = 0; k < nc; ++k) {
-                const uint4 ph = phs[k];
-                float2 ar[TM], ai[TM];
+            // software pipelined: the centre phasors of event k+1 (shared-memory read, integer
+            // phase, two SFU ops per centre) are produced under the 64 FFMA2 of event k
+            float ar[TM], ai[TM];
+            {
+                const uint4 ph = phs[0];
 #pragma unroll
                 for (int g = 0; g < TM; ++g) {
                     const uint32_t pc = ph.x + static_cast<uint32_t>(lane) * ph.y +
                                         static_cast<uint32_t>(g * 4 * TN) * ph.z;
                     float s, c;
                     sincos_u32(pc, s, c);
-                    ar[g] = make_float2(c, c);
-                    ai[g] = make_float2(-s, -s);
+                    ar[g] = c;
+                    ai[g] = -s;
+                }
+            }
+#pragma unroll 1
+            for (int k = 0; k < nc; ++k) {
+                const uint4 ph = phs[min(k + 1, nc - 1)];
+                float arn[TM], ain[TM];
+#pragma unroll
+                for (int g = 0; g < TM; ++g) {
+                    const uint32_t pc = ph.x + static_cast<uint32_t>(lane) * ph.y +
+                                        static_cast<uint32_t>(g * 4 * TN) * ph.z;
+                    float s, c;
+                    sincos_u32(pc, s, c);
+                    arn[g] = c;
+                    ain[g] = -s;
                 }
                 const float4 *brow = reinterpret_cast<const float4 *>(btab + k * TN);
 #pragma unroll
@@ -484,12 +522,15 @@ __global__ void __launch_bounds__(kWarps * 32, 3) k_ndft_score(NdftParams p)
                     const float2 b0 = make_float2(bb.x, bb.y), b1 = make_float2(bb.z, bb.w);
 #pragma unroll
                     for (int g = 0; g < TM; ++g) {
-                        acc1[g][2 * m2] = __ffma2_rn(ar[g], b0, acc1[g][2 * m2]);
-                        acc2[g][2 * m2] = __ffma2_rn(ai[g], b0, acc2[g][2 * m2]);
-                        acc1[g][2 * m2 + 1] = __ffma2_rn(ar[g], b1, acc1[g][2 * m2 + 1]);
-                        acc2[g][2 * m2 + 1] = __ffma2_rn(ai[g], b1, acc2[g][2 * m2 + 1]);
+                        const float2 arr = make_float2(ar[g], ar[g]), aii = make_float2(ai[g], ai[g]);
+                        acc1[g][2 * m2] = __ffma2_rn(arr, b0, acc1[g][2 * m2]);
+                        acc2[g][2 * m2] = __ffma2_rn(aii, b0, acc2[g][2 * m2]);
+                        acc1[g][2 * m2 + 1] = __ffma2_rn(arr, b1, acc1[g][2 * m2 + 1]);
+                        acc2[g][2 * m2 + 1] = __ffma2_rn(aii, b1, acc2[g][2 * m2 + 1]);
                     }
                 }
+#pragma unroll
+                for (int g = 0; g < TM; ++g) { ar[g] = arn[g]; ai[g] = ain[g]; }
             }
             __syncwarp();
         }
