@@ -40,6 +40,12 @@ namespace {
 #ifndef DDHF_NDFT_HEAD_WARPS
 #define DDHF_NDFT_HEAD_WARPS 2     // of every 3 warps, how many start from the long-row end of the work list
 #endif
+#ifndef DDHF_PU
+#define DDHF_PU 4                 // table passes issued together
+#endif
+#ifndef DDHF_EXP
+#define DDHF_EXP 0               // timing experiments only (1: no SF loop, 2: no table, 3: one event per chunk)
+#endif
 #ifndef DDHF_NDFT_BLOCKS
 #define DDHF_NDFT_BLOCKS 1         // CTAs per SM
 #endif
@@ -165,20 +171,24 @@ __device__ __forceinline__ void comb_score(float (&preg)[TM * 2 * TN], const flo
     const int r0 = sp.r0, r1 = sp.r1;
     const int slack = (BS - (r1 - r0 + 1)) / 2;
 
+    // The spectrum is read back from the warp's shared-memory copy in rolled loops: this part
+    // runs on a small share of the pixels, and compact code matters more here than registers.
+    uint32_t *K = reinterpret_cast<uint32_t *>(const_cast<float *>(P_s));     // keys: K[33 i + lane]
     // invalid bins (below k_lo, or padding past n_freq) never take part in the order statistics
-#pragma unroll
+#pragma unroll 1
     for (int i = 0; i < NBL; ++i) {
         const int j = i * 32 + lane;
-        if (j < sp.k_lo || j >= sp.n_freq) preg[i] = __uint_as_float(kInvalidKey);
+        if (j < sp.k_lo || j >= sp.n_freq) K[i * 33 + lane] = kInvalidKey;
+        if (i == 0 && sp.k_lo <= 32) i = max(0, (sp.n_freq >> 5) - 1);        // only the ends can be invalid
     }
+    __syncwarp();
 
-    // ---- A: band limits by counting passes over the register-resident spectrum ----------
+    // ---- A: band limits by counting passes over the spectrum -------------------------------
     // find Lkey with  r0 - slack <= #{key < Lkey} <= r0   and Ukey with
     // r1 + 1 <= #{key < Ukey} <= r1 + 1 + slack; on heavy ties the search converges to the
     // exact order statistic and the tied bins are split by their order in the spectrum.
     uint32_t loL = 0u, hiL = 0x7f800001u, loU = 0u, hiU = 0x7f800001u;
     int cntLo_L = 0, cntLo_U = 0;          // #{key < loL}, #{key < loU}
-    int cntHi_U = nb;                      // #{key < hiU}
     bool doneL = false, doneU = false, exactL = false, exactU = false;
     // first pivots: exponential-spectrum guess around the mean power
     uint32_t pivL, pivU;
@@ -191,11 +201,12 @@ __device__ __forceinline__ void comb_score(float (&preg)[TM * 2 * TN], const flo
         pivU = min(max(pivU, 1u), 0x7f800000u);
     }
     int cntL = 0, cntU = 0;
+#pragma unroll 1
     for (int it = 0; it < 80 && !(doneL && doneU); ++it) {
         int cl = 0, cu = 0;
-#pragma unroll
+#pragma unroll 8
         for (int i = 0; i < NBL; ++i) {
-            const uint32_t key = __float_as_uint(preg[i]);
+            const uint32_t key = K[i * 33 + lane];
             cl += (key < pivL);
             cu += (key < pivU);
         }
@@ -217,7 +228,6 @@ __device__ __forceinline__ void comb_score(float (&preg)[TM * 2 * TN], const flo
         if (!doneU) {
             if (cu >= r1 + 1) {
                 hiU = pivU;
-                cntHi_U = cu;
                 if (cu <= r1 + 1 + slack) { doneU = true; cntU = cu; }
             } else {
                 loU = pivU;
@@ -229,7 +239,6 @@ __device__ __forceinline__ void comb_score(float (&preg)[TM * 2 * TN], const flo
             }
         }
     }
-    (void)cntHi_U;
     const uint32_t Lkey = exactL ? loL : pivL;
     const uint32_t Ukey = exactU ? loU : pivU;
     const int tL = exactL ? (r0 - cntL) : 0;           // tied bins at Lkey that count as "below"
@@ -238,15 +247,15 @@ __device__ __forceinline__ void comb_score(float (&preg)[TM * 2 * TN], const flo
     const int cntU_eff = cntU + tU;
     const int nband = cntU_eff - cntL_eff;
 
-    // ---- B: below / in-band flags as ballots (bit l of word i <-> bin 32 i + l) ----------
+    // ---- B + C: below / in-band flags as ballots (bit l of word i <-> bin 32 i + l), running
+    // popcounts, and the in-band powers compacted in bin order -------------------------------
     {
         const uint32_t lt = (1u << lane) - 1u;
-        int runL = 0, runU = 0;
+        int runL = 0, runU = 0, runB = 0, runI = 0;
         const bool ties = (tL | tU) != 0;
-        uint32_t my_bel0 = 0, my_inb0 = 0, my_bel1 = 0, my_inb1 = 0;   // words lane and lane+32
-#pragma unroll
+#pragma unroll 2
         for (int i = 0; i < NBL; ++i) {
-            const uint32_t key = __float_as_uint(preg[i]);
+            const uint32_t key = K[i * 33 + lane];
             bool below = key < Lkey, leu = key < Ukey;
             if (ties) {
                 const uint32_t mL = __ballot_sync(kFull, key == Lkey);
@@ -257,47 +266,23 @@ __device__ __forceinline__ void comb_score(float (&preg)[TM * 2 * TN], const flo
                 below = below || (key == Lkey && trL < tL);
                 leu = leu || (key == Ukey && trU < tU);
             }
+            const bool inb = leu && !below;
             const uint32_t wb = __ballot_sync(kFull, below);
-            const uint32_t wi = __ballot_sync(kFull, leu && !below);
-            if ((i & 31) == lane) {
-                if (i < 32) { my_bel0 = wb; my_inb0 = wi; } else { my_bel1 = wb; my_inb1 = wi; }
+            const uint32_t wi = __ballot_sync(kFull, inb);
+            if (lane == 0) {
+                belw[i] = wb; inbw[i] = wi;
+                belc[i] = runB; inbc[i] = runI;
             }
-        }
-        // exclusive prefix popcounts over the words
-        int cb0 = __popc(my_bel0), ci0 = __popc(my_inb0), cb1 = __popc(my_bel1), ci1 = __popc(my_inb1);
-        int sb0 = cb0, si0 = ci0, sb1 = cb1, si1 = ci1;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int a = __shfl_up_sync(kFull, sb0, o), b = __shfl_up_sync(kFull, si0, o);
-            const int c = __shfl_up_sync(kFull, sb1, o), d = __shfl_up_sync(kFull, si1, o);
-            if (lane >= o) { sb0 += a; si0 += b; sb1 += c; si1 += d; }
-        }
-        const int totb0 = __shfl_sync(kFull, sb0, 31), toti0 = __shfl_sync(kFull, si0, 31);
-        if (lane < NBL) {
-            belw[lane] = my_bel0; inbw[lane] = my_inb0;
-            belc[lane] = sb0 - cb0; inbc[lane] = si0 - ci0;
-        }
-        if (NBL > 32 && lane + 32 < NBL) {
-            belw[lane + 32] = my_bel1; inbw[lane + 32] = my_inb1;
-            belc[lane + 32] = totb0 + sb1 - cb1; inbc[lane + 32] = toti0 + si1 - ci1;
+            if (inb) {
+                const int ib = runI + __popc(wi & lt);
+                if (ib < BS) bandv[ib] = __uint_as_float(key);
+            }
+            runB += __popc(wb);
+            runI += __popc(wi);
         }
         if (lane == 0) {
             belw[NBL] = 0; inbw[NBL] = 0;
             belc[NBL] = cntL_eff; inbc[NBL] = nband;
-        }
-    }
-    __syncwarp();
-
-    // ---- C: compact the in-band powers in bin order ---------------------------------------
-    {
-        const uint32_t lt = (1u << lane) - 1u;
-#pragma unroll
-        for (int i = 0; i < NBL; ++i) {
-            const uint32_t w = inbw[i];
-            if ((w >> lane) & 1u) {
-                const int ib = inbc[i] + __popc(w & lt);
-                if (ib < BS) bandv[ib] = preg[i];
-            }
         }
     }
     __syncwarp();
@@ -472,18 +457,33 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
                 hph = phase_u32(p.g_h, t);
                 phs[lane] = make_uint4(phase_u32(p.g_f0, t), phase_u32(p.g_d, t), hph, 0u);
             }
+#if DDHF_EXP == 2 || DDHF_EXP == 6
+            const int n_pass = 0;
+#else
             const int n_pass = (nc + EPP - 1) / EPP;
+#endif
+            // four passes at a time: their shuffle -> phase -> SFU -> store chains are independent
+            constexpr int PU = (kEC / EPP) < DDHF_PU ? (kEC / EPP) : DDHF_PU;
 #pragma unroll 1
-            for (int ps = 0; ps < n_pass; ++ps) {
-                const int e = ps * EPP + lane / TN, m = lane % TN;
-                const uint32_t ve = __shfl_sync(kFull, v, e);
-                const uint32_t he = __shfl_sync(kFull, hph, e);
-                float s, c;
-                sincos_u32(he * static_cast<uint32_t>(2 * m + 1), s, c);
-                // b = w (cos, -sin) up to the common sign; w = +1 if bit 0 else -1
-                const uint32_t sgn = (ve & 1u) ? 0u : 0x80000000u;
-                btab[e * TN + m] = make_float2(__uint_as_float(__float_as_uint(c) ^ sgn),
-                                               __uint_as_float(__float_as_uint(s) ^ sgn ^ 0x80000000u));
+            for (int ps0 = 0; ps0 < n_pass; ps0 += PU) {
+                float2 bv[PU];
+#pragma unroll
+                for (int u = 0; u < PU; ++u) {
+                    const int e = (ps0 + u) * EPP + lane / TN, m = lane % TN;
+                    const uint32_t ve = __shfl_sync(kFull, v, e & (kEC - 1));
+                    const uint32_t he = __shfl_sync(kFull, hph, e & (kEC - 1));
+                    float s, c;
+                    sincos_u32(he * static_cast<uint32_t>(2 * m + 1), s, c);
+                    // b = w (cos, -sin) up to the common sign; w = +1 if bit 0 else -1
+                    const uint32_t sgn = (ve & 1u) ? 0u : 0x80000000u;
+                    bv[u] = make_float2(__uint_as_float(__float_as_uint(c) ^ sgn),
+                                        __uint_as_float(__float_as_uint(s) ^ sgn ^ 0x80000000u));
+                }
+#pragma unroll
+                for (int u = 0; u < PU; ++u) {
+                    const int e = (ps0 + u) * EPP + lane / TN, m = lane % TN;
+                    if (e < kEC) btab[e * TN + m] = bv[u];
+                }
             }
             __syncwarp();
             // ---- accumulate: 4 real products per (centre, offset pair, event) --------------
@@ -503,7 +503,7 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
                 }
             }
 #pragma unroll 1
-            for (int k = 0; k < nc; ++k) {
+            for (int k = 0; k < ((DDHF_EXP == 3 || DDHF_EXP == 7) ? min(nc, 1) : nc); ++k) {
                 const uint4 ph = phs[min(k + 1, nc - 1)];
                 float arn[TM], ain[TM];
 #pragma unroll
@@ -559,7 +559,9 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
                 if (i * 32 + lane < sp.n_freq) __stcs(dst + i * 32, preg[i]);
         }
         float slog = 0.f, ssum = 0.f;
-        if (full_grid) {
+        if (DDHF_EXP == 1 || DDHF_EXP == 5) {
+            slog = preg[3]; ssum = preg[5] + 1.f;
+        } else if (full_grid) {
             // every bin is in range; only the first k_lo bins (register 0) are left out
             {
                 const float pt = fmaxf(preg[0], sp.sf_eps);
@@ -599,7 +601,7 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
 
         float score = 0.f;
         int f0 = -1;
-        if (sp.score_all || sf_ok) {
+        if ((DDHF_EXP < 4) && (sp.score_all || sf_ok)) {
 #pragma unroll
             for (int i = 0; i < NBL; ++i) P_s[i * 33 + lane] = preg[i];        // == pad(32 i + lane)
             __syncwarp();
