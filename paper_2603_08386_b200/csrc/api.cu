@@ -22,11 +22,13 @@ struct ddhf_handle {
     int n_tiles = 0;
     int comp_cap = 0;
     int launches = 0;
+    int bits1 = 1, bits2 = 1;
+    int chunk_words = 0;
     ScoreParams sp{};
     uint64_t g_f0 = 0, g_d = 0, g_h = 0;
     CandTable *d_cand = nullptr;
     // workspace offsets (bytes)
-    size_t off_cnt = 0, off_pairs = 0, off_work = 0, off_tiles = 0, off_class = 0, off_cursor = 0, off_long = 0,
+    size_t off_cnt = 0, off_pairs = 0, off_work = 0, off_tiles = 0, off_class = 0, off_cursor = 0, off_thist = 0, off_chunk = 0, off_binbase = 0,
            off_parent = 0, off_slot = 0, off_comp = 0, off_comp_label = 0, off_ctiles = 0, ws_bytes = 0;
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     bool timed_once = false;
@@ -144,6 +146,12 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
         delete h;
         return fail(nullptr, DDHF_E_CUDA, msg);
     }
+    if (ingest_configure() != cudaSuccess) {
+        const std::string msg = std::string("ddhf_create: ") + cudaGetErrorString(cudaGetLastError());
+        cudaFree(h->d_cand);
+        delete h;
+        return fail(nullptr, DDHF_E_CUDA, msg);
+    }
     h->sp.n_freq = c.n_freq; h->sp.k_lo = c.k_lo; h->sp.n_f0 = c.n_f0; h->sp.half_bw = d;
     h->sp.r0 = r0; h->sp.r1 = r1;
     h->sp.tau_sf = c.tau_sf; h->sp.tau_comb = c.tau_comb; h->sp.sf_eps = c.sf_eps;
@@ -166,7 +174,25 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
     h->off_tiles = o;      o = align_up(o + sizeof(int32_t) * 4 * 1024);
     h->off_class = o;      o = align_up(o + sizeof(int32_t) * 2 * kNumClasses);
     h->off_cursor = o;     o = align_up(o + 256);
-    h->off_long = o;       o = align_up(o + sizeof(int32_t) * h->np);
+    {
+        // stable radix partition on the pixel index: two digits of ceil(bits/2) / floor(bits/2) bits
+        int bits = 2;
+        while ((1ll << bits) < np) ++bits;
+        h->bits1 = (bits + 1) / 2;
+        h->bits2 = bits - h->bits1;
+        const size_t bins = static_cast<size_t>(1) << h->bits1;
+        const size_t ev_tiles = (static_cast<size_t>(c.max_events) + ingest_tile_events() - 1) / ingest_tile_events();
+        const size_t ev_chunks = (ev_tiles + ingest_chunk_tiles() - 1) / ingest_chunk_tiles();
+        if (2 * ev_chunks * bins >= (1ull << 31)) {
+            cudaFree(h->d_cand);
+            delete h;
+            return fail(nullptr, DDHF_E_INVAL, "ddhf_create: max_events too large for this sensor size");
+        }
+        h->chunk_words = static_cast<int>(2 * ev_chunks * bins);
+        h->off_thist = o;   o = align_up(o + sizeof(int32_t) * ev_tiles * bins);
+        h->off_chunk = o;   o = align_up(o + sizeof(int32_t) * static_cast<size_t>(h->chunk_words));
+        h->off_binbase = o; o = align_up(o + sizeof(int32_t) * 2 * bins);
+    }
     h->off_parent = o;     o = align_up(o + sizeof(int32_t) * h->np);
     h->off_slot = o;       o = align_up(o + sizeof(int32_t) * h->np);
     h->off_comp = o;       o = align_up(o + sizeof(int32_t) * 5 * static_cast<size_t>(h->comp_cap));
@@ -218,8 +244,13 @@ extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n
     ip.counters = out->counters;
     ip.sf = out->sf; ip.score = out->score; ip.f0_idx = out->f0_idx; ip.mask = out->mask;
     ip.work_cursor = reinterpret_cast<unsigned long long *>(ws + h->off_cursor);
-    ip.n_long = reinterpret_cast<int32_t *>(ws + h->off_cursor + 16);
-    ip.long_rows = reinterpret_cast<int32_t *>(ws + h->off_long);
+    ip.bits1 = h->bits1; ip.bits2 = h->bits2;
+    ip.tile_hist = reinterpret_cast<int32_t *>(ws + h->off_thist);
+    ip.chunk1 = reinterpret_cast<int32_t *>(ws + h->off_chunk);
+    ip.chunk2 = ip.chunk1 + h->chunk_words / 2;
+    ip.chunk_words = h->chunk_words;
+    ip.bin_base1 = reinterpret_cast<int32_t *>(ws + h->off_binbase);
+    ip.bin_base2 = ip.bin_base1 + (1 << h->bits1);
 
     NdftParams np{};
     np.work = ip.work; np.csr_ev = out->csr_ev; np.counters = out->counters;

@@ -63,10 +63,15 @@ struct IngestParams {
     int64_t t0, t1;              // window [t0, t1)
     int32_t width, height, np;
     int32_t n_min, max_active;
-    int32_t *cnt;                // [np] histogram, later reused as scatter cursor
+    int32_t *cnt;                // [np] per-pixel histogram
     int32_t *row_ptr;            // [np+1]
     uint32_t *csr_ev;
-    uint64_t *pairs;             // [max_events] (input index << 32 | csr value), unsorted rows
+    uint64_t *pairs;             // [max_events] (pixel << 32 | csr value) after partition pass 1
+    int32_t bits1, bits2;        // digit widths of the two partition passes (low, high)
+    int32_t *tile_hist;          // [ev_tiles][bins] digit histogram of every 8192-event tile
+    int32_t *chunk1, *chunk2;    // [ev_chunks][bins] per pass; chunk2 follows chunk1 in memory
+    int32_t chunk_words;         // words of chunk1 + chunk2 (zeroed every window)
+    int32_t *bin_base1, *bin_base2;   // [bins]
     int32_t *active_idx;
     WorkItem *work;
     int32_t *tile_sum, *tile_act;   // [n_tiles]
@@ -78,8 +83,6 @@ struct IngestParams {
     int32_t *f0_idx;
     uint8_t *mask;
     unsigned long long *work_cursor;
-    int32_t *long_rows;          // [np] pixels whose row is longer than the short-row limit
-    int32_t *n_long;
 };
 
 struct CclParams {
@@ -100,6 +103,9 @@ struct CclParams {
 // kernel-set entry points (host functions that enqueue on `st`); each returns the number
 // of kernels it launched
 int launch_ingest(const IngestParams &p, cudaStream_t st);
+cudaError_t ingest_configure();              // opt in to large dynamic shared memory
+int ingest_tile_events();                    // events per partition tile
+int ingest_chunk_tiles();                    // tiles per scan chunk
 int launch_ndft(const NdftParams &p, int n_freq, int sm_count, cudaStream_t st);
 int launch_ccl(const CclParams &p, cudaStream_t st);
 int ndft_bins_per_lane(int n_freq);          // 8, 16, 32 or 64

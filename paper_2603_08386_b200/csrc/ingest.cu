@@ -1,27 +1,38 @@
 // ingest.cu -- a0-a3: window/sensor filter, per-pixel histogram, exclusive scan + active
-// list + size-classed work list, deterministic (input-order) scatter into CSR.
+// list + size-classed work list, and a STABLE bucketing of the events into CSR form.
 //
 // "For each window, events are moved to the GPU, sorted by pixel index";
 // pixels with fewer than n_min events are discarded (L137).  Readings R19 (half-open
 // window, bad coordinates dropped and counted) and R20 (input order inside a row).
 //
-// HBM-bound: 16 B read per event twice (histogram, scatter) + 8 B written and read once
-// (unsorted pairs, normally L2-resident) + 4 B written (csr_ev).  The scatter takes a slot
-// with an atomic per pixel, which gives an arbitrary order inside a row; k_rowsort then
-// ranks every element of a row by its input index, which restores input order exactly, so
-// csr_ev is bit-reproducible.
+// The bucketing is a two-pass least-significant-digit radix partition on the pixel index
+// (digits of ceil(bits/2) and floor(bits/2) bits, at most 2048 bins), each pass stable, so
+// that events of one pixel keep their input order and csr_ev is bit-reproducible with no
+// atomics deciding any position:
+//
+//   pass 1   k_dhist<1>   one CTA per tile of 8192 events: per-pixel histogram (global
+//                         atomics, order-free), per-tile digit histogram M[tile][bin]
+//            k_binscan<1> bin-major exclusive scan of the tile histograms (per 8-tile chunk)
+//            k_part<1>    re-reads the tile, ranks every event inside its (tile, bin) group in
+//                         input order (warp match + per-warp counters + cross-warp scan) and
+//                         writes (value, pixel) pairs at base + rank
+//   pass 2   the same three kernels on the pairs with the high digit; the output is csr_ev.
+//
+// HBM traffic per event: 16 B read twice (histogram, partition 1), 8 B written and read twice,
+// 4 B written; the tile histograms add 4 B x bins per 8192 events.
 #include "ddhf_internal.cuh"
 
 namespace ddhf {
 
 namespace {
 
-constexpr int kEvThreads = 256;
-constexpr int kEvUnroll = 4;
-constexpr int kRowPix = 128;       // pixels per k_rowsort_short block
-constexpr int kRowCap = 4096;      // pairs staged in shared memory per block
-constexpr int kShortMax = 64;      // rows up to this length are ranked by counting
-constexpr int kLongBlocks = 148 * 6;
+constexpr int kTileThreads = 512;
+constexpr int kTileWarps = kTileThreads / 32;
+constexpr int kTileEv = 16;                          // events per thread
+constexpr int kTile = kTileThreads * kTileEv;        // 8192 events per tile
+constexpr int kWarpSpan = 32 * kTileEv;              // consecutive events owned by one warp
+constexpr int kChunkTiles = 8;                       // tiles per scan chunk
+constexpr unsigned kFullMask = 0xffffffffu;
 
 struct Ev {
     int32_t pix;       // -1 if dropped
@@ -52,7 +63,7 @@ __device__ __forceinline__ int size_class(int n)
     return min(kNumClasses - 1, max(0, bl - 3));
 }
 
-// ---- k_init: per-pixel maps for inactive pixels, zeroed histogram and counters ---------
+// ---- k_init: per-pixel maps for inactive pixels, zeroed histograms and counters ---------
 __global__ void k_init(IngestParams p)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -63,40 +74,334 @@ __global__ void k_init(IngestParams p)
         p.f0_idx[i] = -1;
         p.mask[i] = 0;
     }
+    for (int k = i; k < p.chunk_words; k += gridDim.x * blockDim.x) p.chunk1[k] = 0;   // chunk1, chunk2
     if (blockIdx.x == 0) {
         if (threadIdx.x < DDHF_N_COUNTERS) p.counters[threadIdx.x] = 0;
         if (threadIdx.x < kNumClasses) {
             p.class_cnt[threadIdx.x] = 0;
             p.class_cur[threadIdx.x] = 0;
         }
-        if (threadIdx.x == 0) { *p.work_cursor = 0ull; *p.n_long = 0; }
+        if (threadIdx.x == 0) *p.work_cursor = 0ull;
     }
 }
 
-// ---- k_hist: counts[pix] += 1 (a1), dropped-event counter -----------------------------
-__global__ void __launch_bounds__(kEvThreads) k_hist(IngestParams p)
+// ---- k_dhist: digit histogram of one tile; pass 2 also counts[pix] += n (a1) ---------------
+// The per-pixel histogram is taken in pass 2: its input is sorted by the low digit, so a tile
+// holds very few distinct low digits and the counts of (low digit, high digit) = pixel can be
+// pre-aggregated in shared memory; only the non-zero sums go to global memory as atomics.
+constexpr int kLoSpan = 4;     // distinct low digits per tile that are aggregated in shared memory
+
+template <int PASS>
+__global__ void __launch_bounds__(kTileThreads) k_dhist(IngestParams p)
 {
+    extern __shared__ uint32_t s_hist[];            // [bins] (+ [kLoSpan][bins] in pass 2)
     __shared__ int s_drop;
+    const int bits = (PASS == 1) ? p.bits1 : p.bits2;
+    const int bins = 1 << bits;
+    const int64_t n_src = (PASS == 1) ? p.n : static_cast<int64_t>(p.counters[DDHF_CNT_N_IN]);
+    const int64_t tile_beg = static_cast<int64_t>(blockIdx.x) * kTile;
+    if (tile_beg >= n_src) return;
+    const int words = (PASS == 1) ? bins : (1 + kLoSpan) * bins;
+    for (int b = threadIdx.x; b < words; b += kTileThreads) s_hist[b] = 0;
     if (threadIdx.x == 0) s_drop = 0;
     __syncthreads();
-    const int64_t base = static_cast<int64_t>(blockIdx.x) * (kEvThreads * kEvUnroll) + threadIdx.x;
-    Ev e[kEvUnroll];
+    if (PASS == 1) {
+        int32_t px[kTileEv];
 #pragma unroll
-    for (int u = 0; u < kEvUnroll; ++u) {
-        const int64_t i = base + u * kEvThreads;
-        e[u].pix = -2;
-        if (i < p.n) e[u] = decode_event(p.events, i, p.t0, p.t1, p.width, p.height);
-    }
-    int drop = 0;
+        for (int u = 0; u < kTileEv; ++u) {
+            const int64_t i = tile_beg + u * kTileThreads + threadIdx.x;
+            px[u] = -2;
+            if (i < n_src) px[u] = decode_event(p.events, i, p.t0, p.t1, p.width, p.height).pix;
+        }
+        const uint32_t dmask = static_cast<uint32_t>(bins - 1);
+        int drop = 0;
 #pragma unroll
-    for (int u = 0; u < kEvUnroll; ++u) {
-        if (e[u].pix >= 0) atomicAdd(&p.cnt[e[u].pix], 1);
-        drop += (e[u].pix == -1);
+        for (int u = 0; u < kTileEv; ++u) {
+            if (px[u] >= 0) atomicAdd(&s_hist[static_cast<uint32_t>(px[u]) & dmask], 1u);
+            drop += (px[u] == -1);
+        }
+        drop = __reduce_add_sync(kFullMask, drop);
+        if ((threadIdx.x & 31) == 0 && drop) atomicAdd(&s_drop, drop);
+    } else {
+        uint32_t *s_pix = s_hist + bins;            // [kLoSpan][bins]
+        const uint32_t lmask = (1u << p.bits1) - 1u;
+        const uint32_t lo_first = __ldg(reinterpret_cast<const uint32_t *>(p.pairs + tile_beg) + 1) & lmask;
+        uint32_t px[kTileEv];
+#pragma unroll
+        for (int u = 0; u < kTileEv; ++u) {
+            const int64_t i = tile_beg + u * kTileThreads + threadIdx.x;
+            px[u] = 0xffffffffu;
+            if (i < n_src) px[u] = __ldg(reinterpret_cast<const uint32_t *>(p.pairs + i) + 1);
+        }
+#pragma unroll
+        for (int u = 0; u < kTileEv; ++u) {
+            if (px[u] != 0xffffffffu) {
+                const uint32_t hi = px[u] >> p.bits1, dl = (px[u] & lmask) - lo_first;
+                if (dl < static_cast<uint32_t>(kLoSpan)) {
+                    atomicAdd(&s_pix[dl * bins + hi], 1u);
+                } else {
+                    atomicAdd(&s_hist[hi], 1u);
+                    atomicAdd(&p.cnt[px[u]], 1);
+                }
+            }
+        }
+        __syncthreads();
+        for (int b = threadIdx.x; b < bins; b += kTileThreads) {
+            uint32_t tot = 0;
+#pragma unroll
+            for (int l = 0; l < kLoSpan; ++l) {
+                const uint32_t c = s_pix[l * bins + b];
+                if (c) atomicAdd(&p.cnt[(static_cast<uint32_t>(b) << p.bits1) | (lo_first + l)], static_cast<int>(c));
+                tot += c;
+            }
+            s_hist[b] += tot;                       // same thread reads it below
+        }
     }
-    drop = __reduce_add_sync(0xffffffffu, drop);
-    if ((threadIdx.x & 31) == 0 && drop) atomicAdd(&s_drop, drop);
     __syncthreads();
-    if (threadIdx.x == 0 && s_drop) atomicAdd(&p.counters[DDHF_CNT_N_DROPPED], s_drop);
+    int32_t *row = p.tile_hist + static_cast<size_t>(blockIdx.x) * bins;
+    int32_t *chunk = ((PASS == 1) ? p.chunk1 : p.chunk2) + static_cast<size_t>(blockIdx.x / kChunkTiles) * bins;
+    for (int b = threadIdx.x; b < bins; b += kTileThreads) {
+        const int c = static_cast<int>(s_hist[b]);
+        row[b] = c;
+        if (c) atomicAdd(&chunk[b], c);
+    }
+    if (PASS == 1 && threadIdx.x == 0 && s_drop) atomicAdd(&p.counters[DDHF_CNT_N_DROPPED], s_drop);
+}
+
+// ---- k_binscan: bin-major exclusive scan of the chunk totals (one CTA) -------------------
+// chunk[c][b] becomes the number of events of bin b in chunks before c; bin_base[b] the number
+// of events in bins before b.  Pass 1 also publishes the number of kept events.
+template <int PASS>
+__global__ void __launch_bounds__(1024) k_binscan(IngestParams p)
+{
+    __shared__ int s_w[33];
+    const int bits = (PASS == 1) ? p.bits1 : p.bits2;
+    const int bins = 1 << bits;
+    const int64_t n_src = (PASS == 1) ? p.n : static_cast<int64_t>(p.counters[DDHF_CNT_N_IN]);
+    const int n_tiles = static_cast<int>((n_src + kTile - 1) / kTile);
+    const int n_chunks = (n_tiles + kChunkTiles - 1) / kChunkTiles;
+    int32_t *chunk = (PASS == 1) ? p.chunk1 : p.chunk2;
+    int32_t *bin_base = (PASS == 1) ? p.bin_base1 : p.bin_base2;
+    // thread t owns bins 2t and 2t+1 (bins <= 2048); chunks are read 16 at a time
+    const int b0 = 2 * threadIdx.x;
+    int run0 = 0, run1 = 0;
+    if (b0 < bins) {
+        constexpr int kB = 16;
+        for (int c0 = 0; c0 < n_chunks; c0 += kB) {
+            int2 v[kB];
+#pragma unroll
+            for (int j = 0; j < kB; ++j)
+                v[j] = (c0 + j < n_chunks)
+                           ? *reinterpret_cast<const int2 *>(chunk + static_cast<size_t>(c0 + j) * bins + b0)
+                           : make_int2(0, 0);
+#pragma unroll
+            for (int j = 0; j < kB; ++j) {
+                if (c0 + j < n_chunks)
+                    *reinterpret_cast<int2 *>(chunk + static_cast<size_t>(c0 + j) * bins + b0) = make_int2(run0, run1);
+                run0 += v[j].x;
+                run1 += v[j].y;
+            }
+        }
+    }
+    // block exclusive scan of (run0 + run1)
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int mine = run0 + run1;
+    int inc = mine;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(kFullMask, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) s_w[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        const int w = s_w[lane];
+        int x = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(kFullMask, x, o);
+            if (lane >= o) x += t;
+        }
+        s_w[lane] = x - w;
+        if (lane == 31) s_w[32] = x;
+    }
+    __syncthreads();
+    const int excl = inc - mine + s_w[wid];
+    if (b0 < bins) {
+        bin_base[b0] = excl;
+        bin_base[b0 + 1] = excl + run0;
+    }
+    if (PASS == 1 && threadIdx.x == 0) p.counters[DDHF_CNT_N_IN] = s_w[32];
+}
+
+// ---- k_part: stable partition of one tile by the pass's digit ----------------------------
+// Warp w of the CTA owns the tile's events [512 w, 512 w + 512) and walks them in 16 steps of
+// 32 consecutive events.  Inside a step, lanes with the same digit find each other with
+// match.any; the lowest lane of a group advances the warp's counter of that digit, so an
+// event's rank inside (tile, digit) follows input order exactly.  The tile is then laid out in
+// shared memory in output order (bin-major) and written with consecutive threads on
+// consecutive elements, so that every run of a bin is a coalesced store.
+template <int PASS>
+struct PartSmem {
+    // words: base[bins] | binoff[bins] | wcnt[kTileWarps][bins] (u16) | stage
+    static constexpr int kStageWords = (PASS == 1) ? 2 * kTile : kTile + kTile / 2;
+    static size_t bytes(int bins) { return static_cast<size_t>(bins) * (8 + 2 * kTileWarps) + 4u * kStageWords; }
+};
+
+template <int PASS>
+__global__ void __launch_bounds__(kTileThreads, 2) k_part(IngestParams p)
+{
+    extern __shared__ uint32_t s_raw[];
+    __shared__ int s_ntile;
+    const int bits = (PASS == 1) ? p.bits1 : p.bits2;
+    const int bins = 1 << bits;
+    int32_t *s_base = reinterpret_cast<int32_t *>(s_raw);                              // [bins] global base - tile offset
+    uint32_t *s_binoff = s_raw + bins;                                                 // [bins] tile-local offset of the bin
+    unsigned short *s_wcnt = reinterpret_cast<unsigned short *>(s_raw + 2 * bins);     // [kTileWarps][bins]
+    uint32_t *s_stage = s_raw + 2 * bins + kTileWarps * bins / 2;
+    const int64_t n_src = (PASS == 1) ? p.n : static_cast<int64_t>(p.counters[DDHF_CNT_N_IN]);
+    const int tile = blockIdx.x;
+    const int64_t tile_beg = static_cast<int64_t>(tile) * kTile;
+    if (tile_beg >= n_src) return;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+
+    for (int k = threadIdx.x; k < kTileWarps * bins / 2; k += kTileThreads)
+        reinterpret_cast<uint32_t *>(s_wcnt)[k] = 0u;
+    // global position of the first event of every bin of this tile
+    {
+        const int32_t *chunk = ((PASS == 1) ? p.chunk1 : p.chunk2) + static_cast<size_t>(tile / kChunkTiles) * bins;
+        const int32_t *bin_base = (PASS == 1) ? p.bin_base1 : p.bin_base2;
+        const int32_t *rows = p.tile_hist + static_cast<size_t>(tile / kChunkTiles) * kChunkTiles * bins;
+        const int n_before = tile % kChunkTiles;
+        for (int b = threadIdx.x; b < bins; b += kTileThreads) {
+            int acc = bin_base[b] + chunk[b];
+#pragma unroll
+            for (int t = 0; t < kChunkTiles - 1; ++t)
+                if (t < n_before) acc += rows[static_cast<size_t>(t) * bins + b];
+            s_base[b] = acc;
+        }
+    }
+    uint32_t val[kTileEv], pix[kTileEv];
+    const int64_t warp_beg = tile_beg + wid * kWarpSpan + lane;
+#pragma unroll
+    for (int s = 0; s < kTileEv; ++s) {
+        const int64_t i = warp_beg + s * 32;
+        pix[s] = 0xffffffffu;
+        val[s] = 0u;
+        if (i < n_src) {
+            if (PASS == 1) {
+                const Ev e = decode_event(p.events, i, p.t0, p.t1, p.width, p.height);
+                pix[s] = static_cast<uint32_t>(e.pix);          // -1 -> 0xffffffff
+                val[s] = e.val;
+            } else {
+                const uint2 q = __ldg(reinterpret_cast<const uint2 *>(p.pairs) + i);
+                val[s] = q.x;
+                pix[s] = q.y;
+            }
+        }
+    }
+    __syncthreads();
+
+    // rank inside (warp, digit) in input order
+    unsigned short *my_cnt = s_wcnt + wid * bins;
+    const uint32_t dmask = static_cast<uint32_t>(bins - 1);
+    const uint32_t lt = (1u << lane) - 1u;
+    uint32_t key[kTileEv];                    // digit | rank << 16
+#pragma unroll
+    for (int s = 0; s < kTileEv; ++s) {
+        const bool ok = pix[s] != 0xffffffffu;
+        const uint32_t d = (PASS == 1) ? (pix[s] & dmask) : ((pix[s] >> p.bits1) & dmask);
+        const uint32_t mk = ok ? d : (0x80000000u | static_cast<uint32_t>(lane));
+        const uint32_t peers = __match_any_sync(kFullMask, mk);
+        const uint32_t c = ok ? my_cnt[d] : 0u;                 // every lane of a group reads the same counter
+        __syncwarp();
+        if (ok && (peers & lt) == 0u) my_cnt[d] = static_cast<unsigned short>(c + __popc(peers));
+        __syncwarp();
+        key[s] = ok ? (d | ((c + __popc(peers & lt)) << 16)) : 0xffffffffu;
+    }
+    __syncthreads();
+    // per bin: exclusive scan of the per-warp counters over the warps, then of the bin totals
+    // over the bins (thread t owns `per` consecutive bins)
+    {
+        __shared__ uint32_t s_ws[kTileWarps + 1];
+        const int per = (bins + kTileThreads - 1) / kTileThreads;
+        const int bb = threadIdx.x * per;
+        uint32_t tot[4];                                       // per <= 4 (bins <= 2048)
+        uint32_t sum = 0;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            tot[j] = 0;
+            const int b = bb + j;
+            if (j < per && b < bins) {
+                uint32_t run = 0;
+#pragma unroll
+                for (int w = 0; w < kTileWarps; ++w) {
+                    const uint32_t t = s_wcnt[w * bins + b];
+                    s_wcnt[w * bins + b] = static_cast<unsigned short>(run);
+                    run += t;
+                }
+                tot[j] = run;
+                sum += run;
+            }
+        }
+        uint32_t inc = sum;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(kFullMask, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (lane == 31) s_ws[wid] = inc;
+        __syncthreads();
+        if (wid == 0) {
+            const uint32_t w = (lane < kTileWarps) ? s_ws[lane] : 0u;
+            uint32_t x = w;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t t = __shfl_up_sync(kFullMask, x, o);
+                if (lane >= o) x += t;
+            }
+            if (lane < kTileWarps) s_ws[lane] = x - w;
+        }
+        __syncthreads();
+        uint32_t off = inc - sum + s_ws[wid];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const int b = bb + j;
+            if (j < per && b < bins) {
+                s_binoff[b] = off;
+                s_base[b] -= static_cast<int32_t>(off);
+                off += tot[j];
+            }
+        }
+        if (bb < bins && bb + per >= bins) s_ntile = static_cast<int>(off);
+    }
+    __syncthreads();
+    // lay the tile out in output order
+    unsigned short *s_sbin = reinterpret_cast<unsigned short *>(s_stage + kTile);      // pass 2: bin of every staged element
+#pragma unroll
+    for (int s = 0; s < kTileEv; ++s) {
+        if (key[s] != 0xffffffffu) {
+            const uint32_t d = key[s] & 0xffffu;
+            const uint32_t at = s_binoff[d] + my_cnt[d] + (key[s] >> 16);
+            if (PASS == 1) {
+                reinterpret_cast<uint2 *>(s_stage)[at] = make_uint2(val[s], pix[s]);
+            } else {
+                s_stage[at] = val[s];
+                s_sbin[at] = static_cast<unsigned short>(d);
+            }
+        }
+    }
+    __syncthreads();
+    const int n_tile = s_ntile;                                                          // kept events of this tile
+    for (int i = threadIdx.x; i < n_tile; i += kTileThreads) {
+        if (PASS == 1) {
+            const uint2 q = reinterpret_cast<const uint2 *>(s_stage)[i];
+            const uint32_t d = q.y & dmask;
+            p.pairs[s_base[d] + i] = (static_cast<uint64_t>(q.y) << 32) | q.x;
+        } else {
+            p.csr_ev[s_base[s_sbin[i]] + i] = s_stage[i];
+        }
+    }
 }
 
 // ---- block-wide exclusive scan of two ints (1024 threads) -----------------------------
@@ -202,39 +507,34 @@ __global__ void __launch_bounds__(1024) k_scan_tiles(IngestParams p, int n_tiles
     }
 }
 
-// ---- k_scan_apply: row_ptr, active_idx, work list; re-zero the histogram ---------------
+// ---- k_scan_apply: row_ptr, active_idx, size-classed work list --------------------------
 __global__ void __launch_bounds__(1024) k_scan_apply(IngestParams p)
 {
     __shared__ int s_a[33], s_b[33];
     __shared__ int s_cls[kNumClasses], s_base[kNumClasses];
-    __shared__ int s_nlong, s_longbase;
     if (threadIdx.x < kNumClasses) s_cls[threadIdx.x] = 0;
-    if (threadIdx.x == 0) s_nlong = 0;
     __syncthreads();
     const int base = blockIdx.x * kScanTile + threadIdx.x * 4;
     int v[4];
     load4(p.cnt, base, p.np, v);
     const int nmin = max(p.n_min, 1);
     int sum = 0, act = 0;
-    int lrank[4], llong[4];
+    int lrank[4];
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
         sum += v[j];
         lrank[j] = -1;
-        llong[j] = -1;
         if (v[j] >= nmin) {
             ++act;
             lrank[j] = atomicAdd(&s_cls[size_class(v[j])], 1);
         }
-        if (v[j] > kShortMax) llong[j] = atomicAdd(&s_nlong, 1);
     }
     int ta, tb;
-    block_scan2(sum, act, ta, tb, s_a, s_b);       // contains __syncthreads: s_cls, s_nlong are final
+    block_scan2(sum, act, ta, tb, s_a, s_b);       // contains __syncthreads: s_cls is final
     if (threadIdx.x < kNumClasses) {
         const int n = s_cls[threadIdx.x];
         s_base[threadIdx.x] = p.class_cnt[threadIdx.x] + (n ? atomicAdd(&p.class_cur[threadIdx.x], n) : 0);
     }
-    if (threadIdx.x == 32) s_longbase = s_nlong ? atomicAdd(p.n_long, s_nlong) : 0;
     __syncthreads();
     int off = p.tile_off[blockIdx.x] + sum;
     int aoff = p.tile_aoff[blockIdx.x] + act;
@@ -243,8 +543,6 @@ __global__ void __launch_bounds__(1024) k_scan_apply(IngestParams p)
         const int pix = base + j;
         if (pix < p.np) {
             p.row_ptr[pix] = off;
-            p.cnt[pix] = 0;
-            if (llong[j] >= 0) p.long_rows[s_longbase + llong[j]] = pix;
             if (lrank[j] >= 0) {
                 if (aoff < p.max_active) p.active_idx[aoff] = pix;
                 WorkItem it;
@@ -260,126 +558,41 @@ __global__ void __launch_bounds__(1024) k_scan_apply(IngestParams p)
     }
 }
 
-// ---- k_scatter: pairs[row_ptr[pix] + slot] = (input index, value) ----------------------
-__global__ void __launch_bounds__(kEvThreads) k_scatter(IngestParams p)
-{
-    const int64_t base = static_cast<int64_t>(blockIdx.x) * (kEvThreads * kEvUnroll) + threadIdx.x;
-    Ev e[kEvUnroll];
-#pragma unroll
-    for (int u = 0; u < kEvUnroll; ++u) {
-        const int64_t i = base + u * kEvThreads;
-        e[u].pix = -2;
-        if (i < p.n) e[u] = decode_event(p.events, i, p.t0, p.t1, p.width, p.height);
-    }
-#pragma unroll
-    for (int u = 0; u < kEvUnroll; ++u) {
-        if (e[u].pix >= 0) {
-            const int64_t i = base + u * kEvThreads;
-            const int slot = __ldg(&p.row_ptr[e[u].pix]) + atomicAdd(&p.cnt[e[u].pix], 1);
-            p.pairs[slot] = (static_cast<uint64_t>(i) << 32) | e[u].val;
-        }
-    }
-}
-
-// ---- row sort: restore input order inside every row (a3, R20) ---------------------------
-// Short rows (<= kShortMax events): a block owns kRowPix consecutive pixels, i.e. one
-// contiguous span of slots; every element finds its row by binary search over the block's
-// row starts and its rank inside the row by counting the elements of the row with a smaller
-// input index.  Long rows are listed by k_scan_apply and sorted one per block (bitonic sort
-// in shared memory) by k_rowsort_long.
-__global__ void __launch_bounds__(256) k_rowsort_short(IngestParams p)
-{
-    __shared__ int s_rp[kRowPix + 1];
-    __shared__ uint64_t s_pair[kRowCap];
-    const int p0 = blockIdx.x * kRowPix;
-    const int npx = min(kRowPix, p.np - p0);
-    for (int i = threadIdx.x; i <= npx; i += blockDim.x) s_rp[i] = p.row_ptr[p0 + i];
-    __syncthreads();
-    const int beg = s_rp[0], tot = s_rp[npx] - beg;
-    if (tot == 0) return;
-    const bool staged = tot <= kRowCap;
-    if (staged) {
-        for (int i = threadIdx.x; i < tot; i += blockDim.x) s_pair[i] = p.pairs[beg + i];
-        __syncthreads();
-    }
-    for (int s = threadIdx.x; s < tot; s += blockDim.x) {
-        int lo = 0, hi = npx;                              // row = last r with s_rp[r] - beg <= s
-        while (hi - lo > 1) {
-            const int mid = (lo + hi) >> 1;
-            if (s_rp[mid] - beg <= s) lo = mid; else hi = mid;
-        }
-        const int rb = s_rp[lo] - beg, re = s_rp[lo + 1] - beg;
-        if (re - rb > kShortMax) continue;                 // k_rowsort_long's
-        int rank = 0;
-        uint64_t mine;
-        if (staged) {
-            mine = s_pair[s];
-            for (int j = rb; j < re; ++j) rank += (s_pair[j] < mine);
-        } else {
-            mine = p.pairs[beg + s];
-            for (int j = rb; j < re; ++j) rank += (p.pairs[beg + j] < mine);
-        }
-        p.csr_ev[beg + rb + rank] = static_cast<uint32_t>(mine);
-    }
-}
-
-__global__ void __launch_bounds__(256) k_rowsort_long(IngestParams p)
-{
-    __shared__ uint64_t s_key[kRowCap];
-    const int n_long = *p.n_long;
-    for (int r = blockIdx.x; r < n_long; r += gridDim.x) {
-        const int pix = p.long_rows[r];
-        const int beg = p.row_ptr[pix], n = p.row_ptr[pix + 1] - beg;
-        if (n <= kRowCap) {
-            int np2 = 1;
-            while (np2 < n) np2 <<= 1;
-            for (int i = threadIdx.x; i < np2; i += blockDim.x)
-                s_key[i] = (i < n) ? p.pairs[beg + i] : ~0ull;
-            __syncthreads();
-            for (int k = 2; k <= np2; k <<= 1) {
-                for (int j = k >> 1; j > 0; j >>= 1) {
-                    for (int t = threadIdx.x; t < (np2 >> 1); t += blockDim.x) {
-                        const int lo = ((t & ~(j - 1)) << 1) | (t & (j - 1));    // index with bit j clear
-                        const int hi = lo | j;
-                        const bool asc = (lo & k) == 0;
-                        const uint64_t a = s_key[lo], b = s_key[hi];
-                        if ((a > b) == asc) { s_key[lo] = b; s_key[hi] = a; }
-                    }
-                    __syncthreads();
-                }
-            }
-            for (int i = threadIdx.x; i < n; i += blockDim.x)
-                p.csr_ev[beg + i] = static_cast<uint32_t>(s_key[i]);
-            __syncthreads();
-        } else {
-            // very long row (thousands of events on one pixel): rank by counting from global memory
-            for (int s = threadIdx.x; s < n; s += blockDim.x) {
-                const uint64_t mine = p.pairs[beg + s];
-                int rank = 0;
-                for (int j = 0; j < n; ++j) rank += (p.pairs[beg + j] < mine);
-                p.csr_ev[beg + rank] = static_cast<uint32_t>(mine);
-            }
-        }
-    }
-}
 
 }  // namespace
+
+cudaError_t ingest_configure()
+{
+    // sized for the largest digit (2048 bins)
+    cudaError_t e = cudaFuncSetAttribute(k_part<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         static_cast<int>(PartSmem<1>::bytes(2048)));
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_part<2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                static_cast<int>(PartSmem<2>::bytes(2048)));
+}
+
+int ingest_tile_events() { return kTile; }
+int ingest_chunk_tiles() { return kChunkTiles; }
 
 int launch_ingest(const IngestParams &p, cudaStream_t st)
 {
     const int n_tiles = (p.np + kScanTile - 1) / kScanTile;
-    const int ev_blocks = static_cast<int>((p.n + kEvThreads * kEvUnroll - 1) / (kEvThreads * kEvUnroll));
+    const int ev_tiles = static_cast<int>((p.n + kTile - 1) / kTile);
+    const int bins1 = 1 << p.bits1, bins2 = 1 << p.bits2;
+    const size_t part1_smem = PartSmem<1>::bytes(bins1), part2_smem = PartSmem<2>::bytes(bins2);
     int launches = 0;
     k_init<<<(p.np + 255) / 256, 256, 0, st>>>(p); ++launches;
-    if (ev_blocks > 0) { k_hist<<<ev_blocks, kEvThreads, 0, st>>>(p); ++launches; }
+    if (ev_tiles > 0) {
+        k_dhist<1><<<ev_tiles, kTileThreads, bins1 * 4, st>>>(p); ++launches;
+        k_binscan<1><<<1, 1024, 0, st>>>(p); ++launches;
+        k_part<1><<<ev_tiles, kTileThreads, part1_smem, st>>>(p); ++launches;
+        k_dhist<2><<<ev_tiles, kTileThreads, (1 + kLoSpan) * bins2 * 4, st>>>(p); ++launches;
+        k_binscan<2><<<1, 1024, 0, st>>>(p); ++launches;
+        k_part<2><<<ev_tiles, kTileThreads, part2_smem, st>>>(p); ++launches;
+    }
     k_scan_reduce<<<n_tiles, 1024, 0, st>>>(p); ++launches;
     k_scan_tiles<<<1, 1024, 0, st>>>(p, n_tiles); ++launches;
     k_scan_apply<<<n_tiles, 1024, 0, st>>>(p); ++launches;
-    if (ev_blocks > 0) {
-        k_scatter<<<ev_blocks, kEvThreads, 0, st>>>(p); ++launches;
-        k_rowsort_short<<<(p.np + kRowPix - 1) / kRowPix, 256, 0, st>>>(p); ++launches;
-        k_rowsort_long<<<kLongBlocks, 256, 0, st>>>(p); ++launches;
-    }
     return launches;
 }
 
