@@ -191,7 +191,7 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
         h->chunk_words = static_cast<int>(2 * ev_chunks * bins);
         h->off_thist = o;   o = align_up(o + sizeof(int32_t) * ev_tiles * bins);
         h->off_chunk = o;   o = align_up(o + sizeof(int32_t) * static_cast<size_t>(h->chunk_words));
-        h->off_binbase = o; o = align_up(o + sizeof(int32_t) * 2 * bins);
+        h->off_binbase = o; o = align_up(o + sizeof(int32_t) * 3 * bins);
     }
     h->off_parent = o;     o = align_up(o + sizeof(int32_t) * h->np);
     h->off_slot = o;       o = align_up(o + sizeof(int32_t) * h->np);
@@ -251,6 +251,8 @@ extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n
     ip.chunk_words = h->chunk_words;
     ip.bin_base1 = reinterpret_cast<int32_t *>(ws + h->off_binbase);
     ip.bin_base2 = ip.bin_base1 + (1 << h->bits1);
+    ip.bin_tot = ip.bin_base2 + (1 << h->bits1);
+    ip.scan_done = reinterpret_cast<int32_t *>(ws + h->off_cursor + 16);
 
     NdftParams np{};
     np.work = ip.work; np.csr_ev = out->csr_ev; np.counters = out->counters;

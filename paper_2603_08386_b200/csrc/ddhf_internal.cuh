@@ -72,6 +72,8 @@ struct IngestParams {
     int32_t *chunk1, *chunk2;    // [ev_chunks][bins] per pass; chunk2 follows chunk1 in memory
     int32_t chunk_words;         // words of chunk1 + chunk2 (zeroed every window)
     int32_t *bin_base1, *bin_base2;   // [bins]
+    int32_t *bin_tot;            // [bins] scratch of k_binscan
+    int32_t *scan_done;          // [2] CTAs of k_binscan<1>, <2> that have finished
     int32_t *active_idx;
     WorkItem *work;
     int32_t *tile_sum, *tile_act;   // [n_tiles]

@@ -81,7 +81,7 @@ __global__ void k_init(IngestParams p)
             p.class_cnt[threadIdx.x] = 0;
             p.class_cur[threadIdx.x] = 0;
         }
-        if (threadIdx.x == 0) *p.work_cursor = 0ull;
+        if (threadIdx.x == 0) { *p.work_cursor = 0ull; p.scan_done[0] = 0; p.scan_done[1] = 0; }
     }
 }
 
@@ -168,13 +168,17 @@ __global__ void __launch_bounds__(kTileThreads) k_dhist(IngestParams p)
     if (PASS == 1 && threadIdx.x == 0 && s_drop) atomicAdd(&p.counters[DDHF_CNT_N_DROPPED], s_drop);
 }
 
-// ---- k_binscan: bin-major exclusive scan of the chunk totals (one CTA) -------------------
+// ---- k_binscan: bin-major exclusive scan of the chunk totals ------------------------------
 // chunk[c][b] becomes the number of events of bin b in chunks before c; bin_base[b] the number
-// of events in bins before b.  Pass 1 also publishes the number of kept events.
+// of events in bins before b.  One CTA per 32 bins; warp g of a CTA owns a contiguous range
+// of chunks, lane l the bin.  The last CTA to finish scans the bin totals.
+// Pass 1 also publishes the number of kept events.
 template <int PASS>
 __global__ void __launch_bounds__(1024) k_binscan(IngestParams p)
 {
+    __shared__ int s_grp[32][33];
     __shared__ int s_w[33];
+    __shared__ bool s_last;
     const int bits = (PASS == 1) ? p.bits1 : p.bits2;
     const int bins = 1 << bits;
     const int64_t n_src = (PASS == 1) ? p.n : static_cast<int64_t>(p.counters[DDHF_CNT_N_IN]);
@@ -182,29 +186,43 @@ __global__ void __launch_bounds__(1024) k_binscan(IngestParams p)
     const int n_chunks = (n_tiles + kChunkTiles - 1) / kChunkTiles;
     int32_t *chunk = (PASS == 1) ? p.chunk1 : p.chunk2;
     int32_t *bin_base = (PASS == 1) ? p.bin_base1 : p.bin_base2;
-    // thread t owns bins 2t and 2t+1 (bins <= 2048); chunks are read 16 at a time
-    const int b0 = 2 * threadIdx.x;
-    int run0 = 0, run1 = 0;
-    if (b0 < bins) {
-        constexpr int kB = 16;
-        for (int c0 = 0; c0 < n_chunks; c0 += kB) {
-            int2 v[kB];
-#pragma unroll
-            for (int j = 0; j < kB; ++j)
-                v[j] = (c0 + j < n_chunks)
-                           ? *reinterpret_cast<const int2 *>(chunk + static_cast<size_t>(c0 + j) * bins + b0)
-                           : make_int2(0, 0);
-#pragma unroll
-            for (int j = 0; j < kB; ++j) {
-                if (c0 + j < n_chunks)
-                    *reinterpret_cast<int2 *>(chunk + static_cast<size_t>(c0 + j) * bins + b0) = make_int2(run0, run1);
-                run0 += v[j].x;
-                run1 += v[j].y;
-            }
-        }
+    int32_t *bin_tot = p.bin_tot;
+    const int lane = threadIdx.x & 31, g = threadIdx.x >> 5;
+    const int b = blockIdx.x * 32 + lane;
+    const bool live = b < bins;
+    const int per_g = (n_chunks + 31) / 32;
+    const int c_beg = min(g * per_g, n_chunks), c_end = min(c_beg + per_g, n_chunks);
+    int sum = 0;
+    if (live)
+        for (int c = c_beg; c < c_end; ++c) sum += chunk[static_cast<size_t>(c) * bins + b];
+    s_grp[g][lane] = sum;
+    __syncthreads();
+    int pre = 0, tot = 0;
+    for (int q = 0; q < 32; ++q) {
+        const int a = s_grp[q][lane];
+        if (q < g) pre += a;
+        tot += a;
     }
-    // block exclusive scan of (run0 + run1)
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    if (live)
+        for (int c = c_beg; c < c_end; ++c) {
+            int32_t *q = chunk + static_cast<size_t>(c) * bins + b;
+            const int v = *q;
+            *q = pre;
+            pre += v;
+        }
+    if (g == 0 && live) bin_tot[b] = tot;
+    // last CTA: exclusive scan of the bin totals
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(p.scan_done + (PASS - 1), 1) == static_cast<int>(gridDim.x) - 1);
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    // thread t owns bins 2t and 2t+1 (bins <= 2048)
+    const int b0 = 2 * threadIdx.x;
+    const int run0 = (b0 < bins) ? *reinterpret_cast<volatile int32_t *>(bin_tot + b0) : 0;
+    const int run1 = (b0 + 1 < bins) ? *reinterpret_cast<volatile int32_t *>(bin_tot + b0 + 1) : 0;
+    const int wid = g;
     const int mine = run0 + run1;
     int inc = mine;
 #pragma unroll
@@ -227,17 +245,15 @@ __global__ void __launch_bounds__(1024) k_binscan(IngestParams p)
     }
     __syncthreads();
     const int excl = inc - mine + s_w[wid];
-    if (b0 < bins) {
-        bin_base[b0] = excl;
-        bin_base[b0 + 1] = excl + run0;
-    }
+    if (b0 < bins) bin_base[b0] = excl;
+    if (b0 + 1 < bins) bin_base[b0 + 1] = excl + run0;
     if (PASS == 1 && threadIdx.x == 0) p.counters[DDHF_CNT_N_IN] = s_w[32];
 }
 
 // ---- k_part: stable partition of one tile by the pass's digit ----------------------------
 // Warp w of the CTA owns the tile's events [512 w, 512 w + 512) and walks them in 16 steps of
 // 32 consecutive events.  Inside a step, lanes with the same digit find each other with
-// match.any; the lowest lane of a group advances the warp's counter of that digit, so an
+// a ballot per digit bit; the lowest lane of a group advances the warp's counter of that digit, so an
 // event's rank inside (tile, digit) follows input order exactly.  The tile is then laid out in
 // shared memory in output order (bin-major) and written with consecutive threads on
 // consecutive elements, so that every run of a bin is a coalesced store.
@@ -311,8 +327,13 @@ __global__ void __launch_bounds__(kTileThreads, 2) k_part(IngestParams p)
     for (int s = 0; s < kTileEv; ++s) {
         const bool ok = pix[s] != 0xffffffffu;
         const uint32_t d = (PASS == 1) ? (pix[s] & dmask) : ((pix[s] >> p.bits1) & dmask);
-        const uint32_t mk = ok ? d : (0x80000000u | static_cast<uint32_t>(lane));
-        const uint32_t peers = __match_any_sync(kFullMask, mk);
+        // lanes with the same digit: one ballot per digit bit (MATCH.ANY is far slower on sm_100)
+        uint32_t peers = __ballot_sync(kFullMask, ok);
+        for (int k = 0; k < bits; ++k) {
+            const bool bit = (d >> k) & 1u;
+            const uint32_t bal = __ballot_sync(kFullMask, bit);
+            peers &= bit ? bal : ~bal;
+        }
         const uint32_t c = ok ? my_cnt[d] : 0u;                 // every lane of a group reads the same counter
         __syncwarp();
         if (ok && (peers & lt) == 0u) my_cnt[d] = static_cast<unsigned short>(c + __popc(peers));
@@ -584,10 +605,10 @@ int launch_ingest(const IngestParams &p, cudaStream_t st)
     k_init<<<(p.np + 255) / 256, 256, 0, st>>>(p); ++launches;
     if (ev_tiles > 0) {
         k_dhist<1><<<ev_tiles, kTileThreads, bins1 * 4, st>>>(p); ++launches;
-        k_binscan<1><<<1, 1024, 0, st>>>(p); ++launches;
+        k_binscan<1><<<(bins1 + 31) / 32, 1024, 0, st>>>(p); ++launches;
         k_part<1><<<ev_tiles, kTileThreads, part1_smem, st>>>(p); ++launches;
         k_dhist<2><<<ev_tiles, kTileThreads, (1 + kLoSpan) * bins2 * 4, st>>>(p); ++launches;
-        k_binscan<2><<<1, 1024, 0, st>>>(p); ++launches;
+        k_binscan<2><<<(bins2 + 31) / 32, 1024, 0, st>>>(p); ++launches;
         k_part<2><<<ev_tiles, kTileThreads, part2_smem, st>>>(p); ++launches;
     }
     k_scan_reduce<<<n_tiles, 1024, 0, st>>>(p); ++launches;
