@@ -327,18 +327,30 @@ __global__ void __launch_bounds__(kTileThreads, 2) k_part(IngestParams p)
     for (int s = 0; s < kTileEv; ++s) {
         const bool ok = pix[s] != 0xffffffffu;
         const uint32_t d = (PASS == 1) ? (pix[s] & dmask) : ((pix[s] >> p.bits1) & dmask);
-        // lanes with the same digit: one ballot per digit bit (MATCH.ANY is far slower on sm_100)
-        uint32_t peers = __ballot_sync(kFullMask, ok);
-        for (int k = 0; k < bits; ++k) {
-            const bool bit = (d >> k) & 1u;
-            const uint32_t bal = __ballot_sync(kFullMask, bit);
-            peers &= bit ? bal : ~bal;
+        // Optimistic step: every lane bumps its digit's counter and tags it with its lane id
+        // (counts are <= 512, the tag sits above bit 11).  If every lane reads its own tag back,
+        // no two lanes shared a digit and the ranks are simply the old counts.
+        const uint32_t c = ok ? (my_cnt[d] & 0x7ffu) : 0u;
+        __syncwarp();
+        if (ok) my_cnt[d] = static_cast<unsigned short>((c + 1u) | (static_cast<uint32_t>(lane) << 11));
+        __syncwarp();
+        const bool lost = ok && (static_cast<uint32_t>(my_cnt[d]) >> 11) != static_cast<uint32_t>(lane);
+        uint32_t rank = c;
+        if (__any_sync(kFullMask, lost)) {
+            // lanes with the same digit, by one ballot per digit bit (MATCH.ANY is far slower on
+            // sm_100); the lowest lane of a group writes the group's count
+            uint32_t peers = __ballot_sync(kFullMask, ok);
+#pragma unroll
+            for (int k = 0; k < 11; ++k) {
+                const bool bit = (d >> k) & 1u;
+                const uint32_t bal = __ballot_sync(kFullMask, bit);
+                peers &= bit ? bal : ~bal;
+            }
+            if (ok && (peers & lt) == 0u) my_cnt[d] = static_cast<unsigned short>(c + __popc(peers));
+            rank = c + __popc(peers & lt);
+            __syncwarp();
         }
-        const uint32_t c = ok ? my_cnt[d] : 0u;                 // every lane of a group reads the same counter
-        __syncwarp();
-        if (ok && (peers & lt) == 0u) my_cnt[d] = static_cast<unsigned short>(c + __popc(peers));
-        __syncwarp();
-        key[s] = ok ? (d | ((c + __popc(peers & lt)) << 16)) : 0xffffffffu;
+        key[s] = ok ? (d | (rank << 16)) : 0xffffffffu;
     }
     __syncthreads();
     // per bin: exclusive scan of the per-warp counters over the warps, then of the bin totals
@@ -357,7 +369,7 @@ __global__ void __launch_bounds__(kTileThreads, 2) k_part(IngestParams p)
                 uint32_t run = 0;
 #pragma unroll
                 for (int w = 0; w < kTileWarps; ++w) {
-                    const uint32_t t = s_wcnt[w * bins + b];
+                    const uint32_t t = s_wcnt[w * bins + b] & 0x7ffu;
                     s_wcnt[w * bins + b] = static_cast<unsigned short>(run);
                     run += t;
                 }
