@@ -94,6 +94,9 @@ typedef struct {
     int64_t max_events;             /* capacity: events per window                        */
     int32_t max_active;             /* capacity: rows of the compact power output         */
     int32_t max_boxes;              /* capacity: boxes                                    */
+    int32_t max_scored;             /* capacity (rows of n_freq floats) of the deferred comb-
+                                       scoring queue in the workspace; 0 = min(NP, 32768).
+                                       Pixels beyond it are scored in place: same results   */
     uint32_t flags;                 /* DDHF_FLAG_*                                        */
 } ddhf_config;
 

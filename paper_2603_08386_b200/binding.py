@@ -40,6 +40,7 @@ class DdhfConfig(C.Structure):
         ("tau_sf", C.c_float), ("tau_comb", C.c_float), ("sf_eps", C.c_float),
         ("k_lo", C.c_int32),
         ("max_events", C.c_int64), ("max_active", C.c_int32), ("max_boxes", C.c_int32),
+        ("max_scored", C.c_int32),
         ("flags", C.c_uint32),
     ]
 
@@ -102,7 +103,7 @@ class DdhfError(RuntimeError):
 
 
 def make_config(params: dict[str, Any], *, max_events: int, max_active: int | None = None,
-                max_boxes: int = 4096, flags: int = 0) -> DdhfConfig:
+                max_boxes: int = 4096, max_scored: int = 0, flags: int = 0) -> DdhfConfig:
     c = DdhfConfig()
     for name in ("width", "height", "f_min_hz", "df_hz", "n_freq", "f0_min_hz", "f0_step_hz",
                  "n_f0", "n_harm", "half_bw_bins", "h_min", "n_min", "a_min", "tau_sf", "tau_comb",
@@ -111,6 +112,7 @@ def make_config(params: dict[str, Any], *, max_events: int, max_active: int | No
     c.max_events = int(max_events)
     c.max_active = int(max_active if max_active is not None else params["width"] * params["height"])
     c.max_boxes = int(max_boxes)
+    c.max_scored = int(max_scored)
     c.flags = int(flags)
     return c
 
@@ -180,7 +182,7 @@ class Detector:
     """Owns the handle, the workspace and the output tensors for one configuration."""
 
     def __init__(self, params: dict[str, Any], *, max_events: int, max_active: int | None = None,
-                 max_boxes: int = 4096, score_all: bool = False, timing: bool = False,
+                 max_boxes: int = 4096, max_scored: int = 0, score_all: bool = False, timing: bool = False,
                  want_power: bool = False, want_labels: bool = True, want_debug: bool = False,
                  device: str = "cuda:0"):
         import torch
@@ -192,7 +194,7 @@ class Detector:
         flags = (DDHF_FLAG_SCORE_ALL if score_all else 0) | (DDHF_FLAG_TIMING if timing else 0)
         self.params = dict(params)
         self.cfg = make_config(params, max_events=max_events, max_active=max_active,
-                               max_boxes=max_boxes, flags=flags)
+                               max_boxes=max_boxes, max_scored=max_scored, flags=flags)
         self.h = ddhf_create(self.cfg)
         c = self.cfg
         self.np_ = c.width * c.height

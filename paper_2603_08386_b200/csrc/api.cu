@@ -24,11 +24,12 @@ struct ddhf_handle {
     int launches = 0;
     int bits1 = 1, bits2 = 1;
     int chunk_words = 0;
+    int spill_cap = 0;
     ScoreParams sp{};
     uint64_t g_f0 = 0, g_d = 0, g_h = 0;
     CandTable *d_cand = nullptr;
     // workspace offsets (bytes)
-    size_t off_cnt = 0, off_pairs = 0, off_work = 0, off_tiles = 0, off_class = 0, off_cursor = 0, off_thist = 0, off_chunk = 0, off_binbase = 0,
+    size_t off_cnt = 0, off_pairs = 0, off_work = 0, off_tiles = 0, off_class = 0, off_cursor = 0, off_thist = 0, off_chunk = 0, off_binbase = 0, off_spill = 0, off_spillrec = 0,
            off_parent = 0, off_slot = 0, off_comp = 0, off_comp_label = 0, off_ctiles = 0, ws_bytes = 0;
     cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
     bool timed_once = false;
@@ -193,6 +194,12 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
         h->off_chunk = o;   o = align_up(o + sizeof(int32_t) * static_cast<size_t>(h->chunk_words));
         h->off_binbase = o; o = align_up(o + sizeof(int32_t) * 3 * bins);
     }
+    // deferred-scoring queue: spectra of the pixels that pass the SF filter (32 Ki rows at most;
+    // pixels beyond the capacity are scored in place by the NDFT kernel)
+    h->spill_cap = h->np < 32768 ? h->np : 32768;
+    if (c.max_scored > 0) h->spill_cap = c.max_scored < h->np ? c.max_scored : h->np;
+    h->off_spill = o;      o = align_up(o + sizeof(float) * static_cast<size_t>(h->spill_cap) * ndft_padded_bins(c.n_freq));
+    h->off_spillrec = o;   o = align_up(o + sizeof(SpillRec) * static_cast<size_t>(h->spill_cap));
     h->off_parent = o;     o = align_up(o + sizeof(int32_t) * h->np);
     h->off_slot = o;       o = align_up(o + sizeof(int32_t) * h->np);
     h->off_comp = o;       o = align_up(o + sizeof(int32_t) * 5 * static_cast<size_t>(h->comp_cap));
@@ -252,7 +259,7 @@ extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n
     ip.bin_base1 = reinterpret_cast<int32_t *>(ws + h->off_binbase);
     ip.bin_base2 = ip.bin_base1 + (1 << h->bits1);
     ip.bin_tot = ip.bin_base2 + (1 << h->bits1);
-    ip.scan_done = reinterpret_cast<int32_t *>(ws + h->off_cursor + 16);
+    ip.scan_done = reinterpret_cast<int32_t *>(ws + h->off_cursor + 16);     // [2], followed by the spill counter
 
     NdftParams np{};
     np.work = ip.work; np.csr_ev = out->csr_ev; np.counters = out->counters;
@@ -261,6 +268,10 @@ extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n
     np.power = out->power; np.sf = out->sf; np.score = out->score; np.f0_idx = out->f0_idx;
     np.mask = out->mask; np.comb_debug = out->comb_debug;
     np.n_scored = out->counters + DDHF_CNT_N_SCORED;
+    np.spill = reinterpret_cast<float *>(ws + h->off_spill);
+    np.spill_rec = reinterpret_cast<SpillRec *>(ws + h->off_spillrec);
+    np.spill_count = reinterpret_cast<int32_t *>(ws + h->off_cursor + 24);
+    np.spill_cap = h->spill_cap;
     np.sp = h->sp;
 
     CclParams cp{};

@@ -41,6 +41,14 @@ struct ScoreParams {
     const CandTable *cand;       // DEVICE [n_f0]
 };
 
+// One row of the deferred-scoring queue (a pixel that passed the SF filter).
+struct __align__(16) SpillRec {
+    int32_t pix;
+    int32_t arow;
+    float mean_p;        // mean of the floored spectrum over [k_lo, n_freq): seed of the band search
+    int32_t _pad;
+};
+
 struct NdftParams {
     const WorkItem *work;        // DEVICE [n_active] ordered by descending size class
     const uint32_t *csr_ev;
@@ -54,6 +62,11 @@ struct NdftParams {
     uint8_t *mask;
     float *comb_debug;
     int32_t *n_scored;
+    // deferred comb scoring: spectra of the pixels to score are queued and scored by k_comb_deferred
+    float *spill;                // [spill_cap][padded n_freq]
+    SpillRec *spill_rec;         // [spill_cap]
+    int32_t *spill_count;        // rows requested (may exceed spill_cap: the excess is scored in place)
+    int32_t spill_cap;
     ScoreParams sp;
 };
 
@@ -113,6 +126,7 @@ int launch_ccl(const CclParams &p, cudaStream_t st);
 int ndft_bins_per_lane(int n_freq);          // 8, 16, 32 or 64
 int ndft_tn(int n_freq);                     // offset pairs per centre for that kernel
 size_t ndft_smem_bytes(int n_freq);
+int ndft_padded_bins(int n_freq);            // row length of the deferred-scoring queue
 int ndft_band_size(int n_freq, int r0, int r1);   // sort capacity needed, 0 if unsupported
 cudaError_t ndft_configure();                // opt in to large dynamic shared memory
 

@@ -147,11 +147,11 @@ __device__ __forceinline__ void bitonic_sort_regs(float (&x)[E], int lane)
 }
 
 // ----------------------------------------------------------------------------------------
-// a6: comb score of one pixel.  preg: the lane's NBL powers (bins lane + 32 i); P_s: the same
-// spectrum in shared memory (padded); returns (score, f0 index) on every lane.
+// a6: comb score of one pixel.  P_s: the spectrum in the warp's shared memory, bin j at
+// P_s[j + (j >> 5)]; returns (score, f0 index) on every lane.
 // ----------------------------------------------------------------------------------------
 template <int TM, int TN, int BS>
-__device__ __forceinline__ void comb_score(float (&preg)[TM * 2 * TN], const float *P_s, uint32_t *scr,
+__device__ __forceinline__ void comb_score(const float *P_s, uint32_t *scr,
                                            const ScoreParams &sp, float mean_p, int lane,
                                            float &score_out, int &f0_out, float *dbg)
 {
@@ -601,23 +601,88 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
 
         float score = 0.f;
         int f0 = -1;
+        bool deferred = false;
         if ((DDHF_EXP < 4) && (sp.score_all || sf_ok)) {
+            // queue the spectrum for k_comb_deferred; if the queue is full, score it here
+            int slot = 0;
+            if (lane == 0) slot = atomicAdd(p.spill_count, 1);
+            slot = __shfl_sync(kFull, slot, 0);
+            if (slot < p.spill_cap) {
+                deferred = true;
+                float *dst = p.spill + static_cast<size_t>(slot) * L::NB + lane;
 #pragma unroll
-            for (int i = 0; i < NBL; ++i) P_s[i * 33 + lane] = preg[i];        // == pad(32 i + lane)
-            __syncwarp();
-            float *dbg = (p.comb_debug != nullptr && has_row)
-                             ? p.comb_debug + static_cast<size_t>(it.arow) * sp.n_f0 * 3 : nullptr;
-            comb_score<TM, TN, BS>(preg, P_s, scr, sp, mean_p, lane, score, f0, dbg);
-            if (lane == 0) atomicAdd(p.n_scored, 1);
+                for (int i = 0; i < NBL; ++i) dst[i * 32] = preg[i];
+                if (lane == 0) {
+                    SpillRec r;
+                    r.pix = it.pix; r.arow = has_row ? it.arow : -1; r.mean_p = mean_p; r._pad = 0;
+                    p.spill_rec[slot] = r;
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < NBL; ++i) P_s[i * 33 + lane] = preg[i];        // == pad(32 i + lane)
+                __syncwarp();
+                float *dbg = (p.comb_debug != nullptr && has_row)
+                                 ? p.comb_debug + static_cast<size_t>(it.arow) * sp.n_f0 * 3 : nullptr;
+                comb_score<TM, TN, BS>(P_s, scr, sp, mean_p, lane, score, f0, dbg);
+                if (lane == 0) atomicAdd(p.n_scored, 1);
+            }
         }
         if (lane == 0) {
             p.sf[it.pix] = sfv;
-            p.score[it.pix] = score;
-            p.f0_idx[it.pix] = f0;
-            p.mask[it.pix] = (sf_ok && f0 >= 0 && score >= sp.tau_comb) ? 1 : 0;   // eq. 11
+            if (!deferred) {
+                p.score[it.pix] = score;
+                p.f0_idx[it.pix] = f0;
+                p.mask[it.pix] = (sf_ok && f0 >= 0 && score >= sp.tau_comb) ? 1 : 0;   // eq. 11
+            }
         }
         __syncwarp();
     }
+}
+
+
+// ----------------------------------------------------------------------------------------
+// Deferred comb scoring: one warp per queued pixel, at an occupancy the 168-register NDFT
+// kernel cannot offer (the code is latency-bound: dependent shared-memory and shuffle chains).
+// Same comb_score() as the in-place path, on the same float spectrum, so results are identical
+// whichever path scores a pixel.
+// ----------------------------------------------------------------------------------------
+constexpr int kScoreWarps = 4;
+
+template <int TM, int TN, int BS>
+__global__ void __launch_bounds__(kScoreWarps * 32) k_comb_deferred(NdftParams p)
+{
+    using L = Layout<TM, TN, BS>;
+    constexpr int NBL = L::NBL;
+    constexpr int WORDS = ((L::P_WORDS + L::SCORE_WORDS + 3) / 4) * 4;
+    extern __shared__ __align__(16) uint32_t smem_raw[];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    uint32_t *wsm = smem_raw + wid * WORDS;
+    float *P_s = reinterpret_cast<float *>(wsm);
+    uint32_t *scr = wsm + L::P_WORDS;
+    const ScoreParams &sp = p.sp;
+    const int n_rows = min(*p.spill_count, p.spill_cap);
+    const int n_warps = gridDim.x * kScoreWarps;
+    for (int row = blockIdx.x * kScoreWarps + wid; row < n_rows; row += n_warps) {
+        const SpillRec r = p.spill_rec[row];
+        const float *src = p.spill + static_cast<size_t>(row) * L::NB + lane;
+#pragma unroll 8
+        for (int i = 0; i < NBL; ++i) P_s[i * 33 + lane] = __ldcs(src + i * 32);
+        __syncwarp();
+        float score;
+        int f0;
+        float *dbg = (p.comb_debug != nullptr && r.arow >= 0)
+                         ? p.comb_debug + static_cast<size_t>(r.arow) * sp.n_f0 * 3 : nullptr;
+        comb_score<TM, TN, BS>(P_s, scr, sp, r.mean_p, lane, score, f0, dbg);
+        if (lane == 0) {
+            // the pixel is in the queue because SF <= tau_sf or score_all; the mask needs both
+            const bool sf_ok = p.sf[r.pix] <= sp.tau_sf;
+            p.score[r.pix] = score;
+            p.f0_idx[r.pix] = f0;
+            p.mask[r.pix] = (sf_ok && f0 >= 0 && score >= sp.tau_comb) ? 1 : 0;       // eq. 11
+        }
+        __syncwarp();
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(p.n_scored, n_rows);
 }
 
 template <int TM, int TN, int BS>
@@ -625,17 +690,24 @@ int launch_one(const NdftParams &p, int sm_count, cudaStream_t st)
 {
     using L = Layout<TM, TN, BS>;
     static bool configured = false;
-    static int blocks_per_sm = 1;
+    static int blocks_per_sm = 1, score_blocks_per_sm = 1;
+    constexpr size_t score_smem = static_cast<size_t>(((L::P_WORDS + L::SCORE_WORDS + 3) / 4) * 4) * 4 * kScoreWarps;
     if (!configured) {
         cudaFuncSetAttribute(k_ndft_score<TM, TN, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              static_cast<int>(L::SMEM_BYTES));
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, k_ndft_score<TM, TN, BS>,
                                                       kWarps * 32, L::SMEM_BYTES);
         if (blocks_per_sm < 1) blocks_per_sm = 1;
+        cudaFuncSetAttribute(k_comb_deferred<TM, TN, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             static_cast<int>(score_smem));
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&score_blocks_per_sm, k_comb_deferred<TM, TN, BS>,
+                                                      kScoreWarps * 32, score_smem);
+        if (score_blocks_per_sm < 1) score_blocks_per_sm = 1;
         configured = true;
     }
     k_ndft_score<TM, TN, BS><<<sm_count * blocks_per_sm, kWarps * 32, L::SMEM_BYTES, st>>>(p);
-    return 1;
+    k_comb_deferred<TM, TN, BS><<<sm_count * score_blocks_per_sm, kScoreWarps * 32, score_smem, st>>>(p);
+    return 2;
 }
 
 }  // namespace
@@ -647,6 +719,8 @@ int ndft_bins_per_lane(int n_freq)
     if (n_freq <= 1024) return 32;
     return 64;
 }
+
+int ndft_padded_bins(int n_freq) { return ndft_bins_per_lane(n_freq) * 32; }
 
 int ndft_tn(int n_freq)
 {

@@ -157,6 +157,22 @@ def test_deterministic_and_stateless():
         assert same, k
 
 
+@pytest.mark.parametrize("score_all", [False, True])
+def test_scoring_queue_overflow_scores_in_place(score_all):
+    """A deferred-scoring queue of 3 rows: every further pixel is scored inside the NDFT kernel.
+    Both paths run the same code on the same float spectrum, so all outputs are bit-identical
+    to those of a queue that holds every pixel."""
+    w = wl.make(2)
+    prm = dict(w.params, n_min=3)
+    a = gu.run_gpu(prm, w.events, 0, w.window_us, score_all=score_all, want_debug=True)
+    b = gu.run_gpu(prm, w.events, 0, w.window_us, score_all=score_all, want_debug=True, max_scored=3)
+    assert a["n_scored"] == b["n_scored"] and a["n_scored"] > 3
+    for k in ("sf", "score", "f0_idx", "mask", "labels", "boxes", "comb_debug"):
+        same = (np.array_equal(a[k], b[k], equal_nan=True) if a[k].dtype.kind == "f"
+                else np.array_equal(a[k], b[k]))
+        assert same, k
+
+
 def test_host_buffer_entry_point_matches_device_path():
     """ddhf_window_host (H2D + kernels + D2H inside the call) == ddhf_window on device buffers."""
     import torch
