@@ -146,12 +146,37 @@ __device__ __forceinline__ void bitonic_sort_regs(float (&x)[E], int lane)
     }
 }
 
+// Next trial key of the band-limit search.  [lo, hi] brackets the wanted key, cLo / cHi are
+// #{key < lo}, #{key < hi}.  Without a finite upper bound: exponential-tail model through
+// (lo, cLo); otherwise linear interpolation of the rank in value space, with a plain bisection
+// of the key interval every third step so that the search always converges.
+__device__ __forceinline__ uint32_t next_pivot(uint32_t lo, uint32_t hi, int cLo, int cHi, float target,
+                                               int it, float nbf)
+{
+    uint32_t piv;
+    if (hi > 0x7f7fffffu) {
+        float g = 4.f;
+        if (cLo > 0)
+            g = __logf(fmaxf(1.f - target / nbf, 1e-6f)) / __logf(fmaxf(1.f - static_cast<float>(cLo) / nbf, 1e-6f));
+        g = fminf(fmaxf(g, 1.0625f), 16.f);
+        piv = __float_as_uint(fmaxf(__uint_as_float(lo), 1e-30f) * g);
+    } else if ((it % 3) == 2 || cHi <= cLo) {
+        piv = lo + ((hi - lo) >> 1);
+    } else {
+        const float vlo = __uint_as_float(lo), vhi = __uint_as_float(hi);
+        const float fr = (target - static_cast<float>(cLo)) / static_cast<float>(cHi - cLo);
+        piv = __float_as_uint(vlo + (vhi - vlo) * fminf(fmaxf(fr, 0.02f), 0.98f));
+    }
+    return min(max(piv, lo + 1u), hi - 1u);
+}
+
 // ----------------------------------------------------------------------------------------
-// a6: comb score of one pixel.  P_s: the spectrum in the warp's shared memory, bin j at
-// P_s[j + (j >> 5)]; returns (score, f0 index) on every lane.
+// a6: comb score of one pixel.  preg: the lane's NBL powers (bins lane + 32 i); P_s: the same
+// spectrum in the warp's shared memory, bin j at P_s[j + (j >> 5)] (overwritten);
+// returns (score, f0 index) on every lane.
 // ----------------------------------------------------------------------------------------
 template <int TM, int TN, int BS>
-__device__ __forceinline__ void comb_score(const float *P_s, uint32_t *scr,
+__device__ __forceinline__ void comb_score(const float (&preg)[TM * 2 * TN], float *P_s, uint32_t *scr,
                                            const ScoreParams &sp, float mean_p, int lane,
                                            float &score_out, int &f0_out, float *dbg)
 {
@@ -173,7 +198,7 @@ __device__ __forceinline__ void comb_score(const float *P_s, uint32_t *scr,
 
     // The spectrum is read back from the warp's shared-memory copy in rolled loops: this part
     // runs on a small share of the pixels, and compact code matters more here than registers.
-    uint32_t *K = reinterpret_cast<uint32_t *>(const_cast<float *>(P_s));     // keys: K[33 i + lane]
+    uint32_t *K = reinterpret_cast<uint32_t *>(P_s);     // keys: K[33 i + lane]
     // invalid bins (below k_lo, or padding past n_freq) never take part in the order statistics
 #pragma unroll 1
     for (int i = 0; i < NBL; ++i) {
@@ -189,6 +214,9 @@ __device__ __forceinline__ void comb_score(const float *P_s, uint32_t *scr,
     // exact order statistic and the tied bins are split by their order in the spectrum.
     uint32_t loL = 0u, hiL = 0x7f800001u, loU = 0u, hiU = 0x7f800001u;
     int cntLo_L = 0, cntLo_U = 0;          // #{key < loL}, #{key < loU}
+    int cntHi_L = nb, cntHi_U = nb;        // #{key < hiL}, #{key < hiU}
+    const float nbf = static_cast<float>(nb);
+    const float tgtL = r0 - 0.5f * slack, tgtU = r1 + 1 + 0.5f * slack;
     bool doneL = false, doneU = false, exactL = false, exactU = false;
     // first pivots: exponential-spectrum guess around the mean power
     uint32_t pivL, pivU;
@@ -202,7 +230,7 @@ __device__ __forceinline__ void comb_score(const float *P_s, uint32_t *scr,
     }
     int cntL = 0, cntU = 0;
 #pragma unroll 1
-    for (int it = 0; it < 80 && !(doneL && doneU); ++it) {
+    for (int it = 0; it < 120 && !(doneL && doneU); ++it) {
         int cl = 0, cu = 0;
 #pragma unroll 8
         for (int i = 0; i < NBL; ++i) {
@@ -215,6 +243,7 @@ __device__ __forceinline__ void comb_score(const float *P_s, uint32_t *scr,
         if (!doneL) {
             if (cl > r0) {
                 hiL = pivL;
+                cntHi_L = cl;
             } else {
                 loL = pivL;
                 cntLo_L = cl;
@@ -222,12 +251,13 @@ __device__ __forceinline__ void comb_score(const float *P_s, uint32_t *scr,
             }
             if (!doneL) {
                 if (hiL - loL <= 1u) { doneL = true; exactL = true; cntL = cntLo_L; }
-                else pivL = loL + ((hiL - loL) >> 1);
+                else pivL = next_pivot(loL, hiL, cntLo_L, cntHi_L, tgtL, it, nbf);
             }
         }
         if (!doneU) {
             if (cu >= r1 + 1) {
                 hiU = pivU;
+                cntHi_U = cu;
                 if (cu <= r1 + 1 + slack) { doneU = true; cntU = cu; }
             } else {
                 loU = pivU;
@@ -235,7 +265,7 @@ __device__ __forceinline__ void comb_score(const float *P_s, uint32_t *scr,
             }
             if (!doneU) {
                 if (hiU - loU <= 1u) { doneU = true; exactU = true; cntU = cntLo_U; }
-                else pivU = loU + ((hiU - loU) >> 1);
+                else pivU = next_pivot(loU, hiU, cntLo_U, cntHi_U, tgtU, it, nbf);
             }
         }
     }
@@ -317,10 +347,37 @@ __device__ __forceinline__ void comb_score(const float *P_s, uint32_t *scr,
     }
     __syncwarp();
 
+    // ---- W: forward block maxima M[k] = max P[k .. k + blk - 1], blk = 2^s <= min(2d+1, 32), by
+    // s doubling steps on the register copy (bin k + sh lives sh lanes further, in register i or
+    // i + 1); written over the spectrum, which only the window maxima of eq. 8 still need ------
+    const int d = sp.half_bw;
+    const int wlen = 2 * d + 1;
+    const int s_lvl = min(31 - __clz(wlen), 5);
+    const int blk = 1 << s_lvl;
+    {
+        float mreg[NBL];
+#pragma unroll
+        for (int i = 0; i < NBL; ++i) mreg[i] = preg[i];
+#pragma unroll 1
+        for (int t = 0; t < s_lvl; ++t) {
+            const int sh = 1 << t;
+            const int src = (lane + sh) & 31;
+            const bool wrap = lane + sh >= 32;
+#pragma unroll
+            for (int i = 0; i < NBL; ++i) {
+                const float a = __shfl_sync(kFull, mreg[i], src);
+                const float b = (i + 1 < NBL) ? __shfl_sync(kFull, mreg[i + 1], src) : 0.f;
+                mreg[i] = fmaxf(mreg[i], wrap ? b : a);
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < NBL; ++i) P_s[i * 33 + lane] = mreg[i];
+    }
+    __syncwarp();
+
     // ---- F: one candidate per lane ------------------------------------------------------------
     float best = 0.f;
     int best_c = 0x7fffffff;
-    const int d = sp.half_bw;
     for (int c0 = 0; c0 < sp.n_f0; c0 += 32) {
         const int c = c0 + lane;
         float snr = 0.f, num = 0.f, med = 0.f;
@@ -334,7 +391,8 @@ __device__ __forceinline__ void comb_score(const float *P_s, uint32_t *scr,
                 for (int m = 0; m < mv; ++m) {
                     const int kc = ct->kc[m];
                     float mx = 0.f;
-                    for (int k = kc - d; k <= kc + d; ++k) mx = fmaxf(mx, P_s[pad(k)]);
+                    for (int off = 0; off < wlen; off += blk)
+                        mx = fmaxf(mx, P_s[pad(min(kc - d + off, kc + d - blk + 1))]);
                     num += mx;
                 }
                 num = num / static_cast<float>(mv);
@@ -623,7 +681,7 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
                 __syncwarp();
                 float *dbg = (p.comb_debug != nullptr && has_row)
                                  ? p.comb_debug + static_cast<size_t>(it.arow) * sp.n_f0 * 3 : nullptr;
-                comb_score<TM, TN, BS>(P_s, scr, sp, mean_p, lane, score, f0, dbg);
+                comb_score<TM, TN, BS>(preg, P_s, scr, sp, mean_p, lane, score, f0, dbg);
                 if (lane == 0) atomicAdd(p.n_scored, 1);
             }
         }
@@ -649,7 +707,7 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
 constexpr int kScoreWarps = 4;
 
 template <int TM, int TN, int BS>
-__global__ void __launch_bounds__(kScoreWarps * 32) k_comb_deferred(NdftParams p)
+__global__ void __launch_bounds__(kScoreWarps * 32, 4) k_comb_deferred(NdftParams p)
 {
     using L = Layout<TM, TN, BS>;
     constexpr int NBL = L::NBL;
@@ -665,14 +723,17 @@ __global__ void __launch_bounds__(kScoreWarps * 32) k_comb_deferred(NdftParams p
     for (int row = blockIdx.x * kScoreWarps + wid; row < n_rows; row += n_warps) {
         const SpillRec r = p.spill_rec[row];
         const float *src = p.spill + static_cast<size_t>(row) * L::NB + lane;
-#pragma unroll 8
-        for (int i = 0; i < NBL; ++i) P_s[i * 33 + lane] = __ldcs(src + i * 32);
+        float preg[NBL];
+#pragma unroll
+        for (int i = 0; i < NBL; ++i) preg[i] = __ldcs(src + i * 32);
+#pragma unroll
+        for (int i = 0; i < NBL; ++i) P_s[i * 33 + lane] = preg[i];
         __syncwarp();
         float score;
         int f0;
         float *dbg = (p.comb_debug != nullptr && r.arow >= 0)
                          ? p.comb_debug + static_cast<size_t>(r.arow) * sp.n_f0 * 3 : nullptr;
-        comb_score<TM, TN, BS>(P_s, scr, sp, r.mean_p, lane, score, f0, dbg);
+        comb_score<TM, TN, BS>(preg, P_s, scr, sp, r.mean_p, lane, score, f0, dbg);
         if (lane == 0) {
             // the pixel is in the queue because SF <= tau_sf or score_all; the mask needs both
             const bool sf_ok = p.sf[r.pix] <= sp.tau_sf;
