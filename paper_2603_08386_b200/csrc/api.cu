@@ -161,9 +161,10 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
 
     // ---- fixed-point frequency constants of the factorised NDFT ------------------------------
     const int tn = ndft_tn(c.n_freq);
-    h->g_h = freq_const(16.0 * c.df_hz);
-    h->g_d = freq_const(c.df_hz);
-    h->g_f0 = freq_const(c.f_min_hz + (32.0 * tn - 16.0) * c.df_hz);
+    // negated (mod 2^64): the kernel evaluates (sin, cos) of -2 pi f t directly
+    h->g_h = 0ull - freq_const(16.0 * c.df_hz);
+    h->g_d = 0ull - freq_const(c.df_hz);
+    h->g_f0 = 0ull - freq_const(c.f_min_hz + (32.0 * tn - 16.0) * c.df_hz);
 
     // ---- workspace layout -----------------------------------------------------------------------
     h->n_tiles = (h->np + kScanTile - 1) / kScanTile;

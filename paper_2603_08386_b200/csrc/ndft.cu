@@ -50,7 +50,7 @@ namespace {
 #define DDHF_NDFT_BLOCKS 1         // CTAs per SM
 #endif
 constexpr int kWarps = DDHF_NDFT_WARPS;
-constexpr int kEC = 16;            // events per table chunk
+constexpr int kEC = 32;            // events per table chunk
 constexpr unsigned kFull = 0xffffffffu;
 constexpr uint32_t kInvalidKey = 0x7fffffffu;
 
@@ -68,7 +68,8 @@ struct Layout {
     static constexpr int MASK_WORDS = BS;                   // maskw[BS/32][32]
     static constexpr int SCORE_WORDS = BAL_WORDS + BAND_WORDS + SORT_WORDS + POS_WORDS + MASK_WORDS;
     static constexpr int SCRATCH_WORDS = (SCORE_WORDS > TAB_WORDS ? SCORE_WORDS : TAB_WORDS);
-    static constexpr int WARP_WORDS = ((P_WORDS + SCRATCH_WORDS + 3) / 4) * 4;
+    static constexpr int EV_WORDS = 2 * kEC;                // staged CSR events, double buffered
+    static constexpr int WARP_WORDS = ((P_WORDS + SCRATCH_WORDS + EV_WORDS + 3) / 4) * 4;
     static constexpr size_t SMEM_BYTES = static_cast<size_t>(WARP_WORDS) * 4 * kWarps;
 };
 
@@ -83,8 +84,8 @@ __device__ __forceinline__ uint32_t phase_u32(uint64_t g, uint32_t t)
 // phasors are always multiplied, so it cancels.  Argument of the SFU is in [-pi, pi).
 __device__ __forceinline__ void sincos_u32(uint32_t ph, float &s, float &c)
 {
-    const float x = __uint_as_float((ph >> 9) | 0x3f800000u) - 1.5f;
-    const float r = x * 6.283185307179586f;
+    // 1 + turns in [1, 2) from the top 23 phase bits; 2 pi (that - 3/2) in one FMA
+    const float r = fmaf(__uint_as_float((ph >> 9) | 0x3f800000u), 6.283185307179586f, -9.42477796076938f);
     s = __sinf(r);
     c = __cosf(r);
 }
@@ -96,12 +97,30 @@ __device__ __forceinline__ int pad(int j) { return j + (j >> 5); }
 // per-pixel epilogue, latency bound), so that every SM sub-partition always holds a mix of
 // the two and neither the FMA pipe nor the issue slots sit idle for a whole phase of the
 // kernel.  One 64-bit counter holds both cursors; an item is valid while head + tail < n.
-__device__ __forceinline__ int fetch_item(unsigned long long *cursor, bool head, int n_items)
+// Tail warps claim kTailBatch items per atomic (short rows cost about a thousand cycles each, so a
+// global atomic per pixel is a visible stall); item i of a claim made at (h, t) is valid while
+// h + t + i < n.  Returns the first index of the claim and its valid count.
+constexpr int kTailBatch = 4;
+
+__device__ __forceinline__ int fetch_items(unsigned long long *cursor, bool head, int n_items, int &cnt)
 {
-    const unsigned long long old = atomicAdd(cursor, head ? (1ull << 32) : 1ull);
+    const unsigned b = head ? 1u : static_cast<unsigned>(kTailBatch);
+    const unsigned long long old = atomicAdd(cursor, head ? (1ull << 32) : static_cast<unsigned long long>(b));
     const unsigned h = static_cast<unsigned>(old >> 32), t = static_cast<unsigned>(old);
-    if (h + t >= static_cast<unsigned>(n_items)) return n_items;
+    const unsigned used = h + t, n = static_cast<unsigned>(n_items);
+    cnt = (used >= n) ? 0 : static_cast<int>(min(b, n - used));
     return head ? static_cast<int>(h) : n_items - 1 - static_cast<int>(t);
+}
+
+__device__ __forceinline__ void stage_event(uint32_t *dst_smem, const uint32_t *src)
+{
+    const unsigned d = static_cast<unsigned>(__cvta_generic_to_shared(dst_smem));
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(d), "l"(src) : "memory");
+}
+
+__device__ __forceinline__ void stage_wait()
+{
+    asm volatile("cp.async.wait_all;" ::: "memory");
 }
 
 __device__ __forceinline__ WorkItem make_item()
@@ -457,7 +476,11 @@ __device__ __forceinline__ void comb_score(const float (&preg)[TM * 2 * TN], flo
 // The fused kernel.
 // ----------------------------------------------------------------------------------------
 template <int TM, int TN, int BS>
+#ifdef DDHF_NDFT_MAXNREG
+__global__ void __maxnreg__(DDHF_NDFT_MAXNREG) k_ndft_score(NdftParams p)
+#else
 __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(NdftParams p)
+#endif
 {
     using L = Layout<TM, TN, BS>;
     constexpr int NBL = L::NBL;
@@ -475,23 +498,30 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
     const bool full_grid = (sp.n_freq == L::NB) && (sp.k_lo <= 32);
     const bool store_power = p.power != nullptr;
 
-    // dynamic work queue with one item of look-ahead: the next index is fetched while the
-    // current pixel is being processed, so the atomic's latency is off the critical path
+    // dynamic work queue with one item of look-ahead: the next work item is loaded while the
+    // current pixel is being processed, and its first events are staged in shared memory by
+    // cp.async (no register holds data in flight, so nothing waits on a spill)
+    uint32_t *ev_s = scr + L::SCRATCH_WORDS;                        // [2][kEC]
+    int evb = 0;                                                    // staging buffer in use
     const bool head = (wid % 3) < DDHF_NDFT_HEAD_WARPS;
+    int claim_left = 0;                                             // items of the current claim not yet started
     int idx = 0;
-    if (lane == 0) idx = fetch_item(p.work_cursor, head, n_items);
+    if (lane == 0) idx = fetch_items(p.work_cursor, head, n_items, claim_left);
     idx = __shfl_sync(kFull, idx, 0);
+    claim_left = __shfl_sync(kFull, claim_left, 0);
+    if (claim_left == 0) idx = n_items;
+    --claim_left;
     WorkItem it_next = make_item();
-    uint32_t v_first = 0u;
     if (idx < n_items) {
         it_next = p.work[idx];
-        if (lane < kEC && lane < it_next.n) v_first = __ldg(p.csr_ev + it_next.row_begin + lane);
+        if (lane < it_next.n) stage_event(ev_s + lane, p.csr_ev + it_next.row_begin + lane);
     }
 
     while (idx < n_items) {
         const WorkItem it = it_next;
-        int next_idx = 0;
-        if (lane == 0) next_idx = fetch_item(p.work_cursor, head, n_items);
+        // next item: the following one of the claim (tail warps walk down the list), or a new claim
+        int next_idx = idx - 1, next_cnt = claim_left;
+        if (claim_left <= 0 && lane == 0) next_idx = fetch_items(p.work_cursor, head, n_items, next_cnt);
 
         float2 acc1[TM][TN], acc2[TM][TN];     // (S1, S4) and (S3, S2)
 #pragma unroll
@@ -502,99 +532,101 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
                 acc2[g][m] = make_float2(0.f, 0.f);
             }
 
-        uint32_t v_next = v_first;
         for (int base = 0; base < it.n; base += kEC) {
             const int nc = min(kEC, it.n - base);
             // ---- per-event phase words and the offset-phasor table of this chunk ----------
-            const uint32_t v = v_next;
-            if (base + kEC + lane < it.n && lane < kEC)           // prefetch the next chunk
-                v_next = __ldg(p.csr_ev + it.row_begin + base + kEC + lane);
-            uint32_t hph = 0;
+            stage_wait();
+            const uint32_t v = ev_s[evb * kEC + lane];
+            evb ^= 1;
+            if (base + kEC + lane < it.n)                         // stage the next chunk
+                stage_event(ev_s + evb * kEC + lane, p.csr_ev + it.row_begin + base + kEC + lane);
             if (lane < nc) {
                 const uint32_t t = v >> 1;
-                hph = phase_u32(p.g_h, t);
-                phs[lane] = make_uint4(phase_u32(p.g_f0, t), phase_u32(p.g_d, t), hph, 0u);
+                // .w: sign mask of the weight, w = +1 if bit 0 of the CSR value else -1
+                phs[lane] = make_uint4(phase_u32(p.g_f0, t), phase_u32(p.g_d, t), phase_u32(p.g_h, t),
+                                       (v & 1u) ? 0u : 0x80000000u);
             }
+            __syncwarp();
 #if DDHF_EXP == 2 || DDHF_EXP == 6
             const int n_pass = 0;
 #else
             const int n_pass = (nc + EPP - 1) / EPP;
 #endif
-            // four passes at a time: their shuffle -> phase -> SFU -> store chains are independent
+            // PU passes at a time: their phase -> SFU -> store chains are independent
             constexpr int PU = (kEC / EPP) < DDHF_PU ? (kEC / EPP) : DDHF_PU;
+            {
+                const int e_l = lane / TN, m_l = lane % TN;
+                const uint32_t mult = static_cast<uint32_t>(2 * m_l + 1);
 #pragma unroll 1
-            for (int ps0 = 0; ps0 < n_pass; ps0 += PU) {
-                float2 bv[PU];
+                for (int ps0 = 0; ps0 < n_pass; ps0 += PU) {
 #pragma unroll
-                for (int u = 0; u < PU; ++u) {
-                    const int e = (ps0 + u) * EPP + lane / TN, m = lane % TN;
-                    const uint32_t ve = __shfl_sync(kFull, v, e & (kEC - 1));
-                    const uint32_t he = __shfl_sync(kFull, hph, e & (kEC - 1));
-                    float s, c;
-                    sincos_u32(he * static_cast<uint32_t>(2 * m + 1), s, c);
-                    // b = w (cos, -sin) up to the common sign; w = +1 if bit 0 else -1
-                    const uint32_t sgn = (ve & 1u) ? 0u : 0x80000000u;
-                    bv[u] = make_float2(__uint_as_float(__float_as_uint(c) ^ sgn),
-                                        __uint_as_float(__float_as_uint(s) ^ sgn ^ 0x80000000u));
-                }
-#pragma unroll
-                for (int u = 0; u < PU; ++u) {
-                    const int e = (ps0 + u) * EPP + lane / TN, m = lane % TN;
-                    if (e < kEC) btab[e * TN + m] = bv[u];
+                    for (int u = 0; u < PU; ++u) {
+                        const int e = (ps0 + u) * EPP + e_l;
+                        if (e < kEC) {
+                            const uint2 hw = *reinterpret_cast<const uint2 *>(&phs[e].z);
+                            float sn, cs;
+                            sincos_u32(hw.x * mult, sn, cs);
+                            // b = w e^{-i phi} up to the common sign of every phasor of the kernel
+                            btab[e * TN + m_l] = make_float2(__uint_as_float(__float_as_uint(cs) ^ hw.y),
+                                                             __uint_as_float(__float_as_uint(sn) ^ hw.y));
+                        }
+                    }
                 }
             }
             __syncwarp();
             // ---- accumulate: 4 real products per (centre, offset pair, event) --------------
-            // software pipelined: the centre phasors of event k+1 (shared-memory read, integer
-            // phase, two SFU ops per centre) are produced under the 64 FFMA2 of event k
-            float ar[TM], ai[TM];
-            {
-                const uint4 ph = phs[0];
-#pragma unroll
-                for (int g = 0; g < TM; ++g) {
-                    const uint32_t pc = ph.x + static_cast<uint32_t>(lane) * ph.y +
-                                        static_cast<uint32_t>(g * 4 * TN) * ph.z;
-                    float s, c;
-                    sincos_u32(pc, s, c);
-                    ar[g] = c;
-                    ai[g] = -s;
-                }
+            // software pipelined by hand, two events per trip: the centre phasors of the next
+            // event (shared-memory read, integer phase, two SFU ops per centre) are produced under
+            // the FFMA2 block of the current one, in alternating register sets (no copies)
+            float a0r[TM], a0i[TM], a1r[TM], a1i[TM];
+            const uint32_t lane_u = static_cast<uint32_t>(lane);
+#define DDHF_CENTRES(AR, AI, K)                                                                  \
+            {                                                                                    \
+                const uint4 ph = phs[K];                                                         \
+                const uint32_t pc0 = ph.x + lane_u * ph.y;                                       \
+                _Pragma("unroll") for (int g = 0; g < TM; ++g)                                   \
+                    sincos_u32(pc0 + static_cast<uint32_t>(g * 4 * TN) * ph.z, AI[g], AR[g]);    \
             }
+#define DDHF_FMA_BLOCK(AR, AI, K)                                                                \
+            {                                                                                    \
+                const float4 *brow = reinterpret_cast<const float4 *>(btab + (K) * TN);          \
+                _Pragma("unroll") for (int m2 = 0; m2 < TN / 2; ++m2) {                          \
+                    const float4 bb = brow[m2];                                                  \
+                    const float2 b0 = make_float2(bb.x, bb.y), b1 = make_float2(bb.z, bb.w);     \
+                    _Pragma("unroll") for (int g = 0; g < TM; ++g) {                             \
+                        const float2 arr = make_float2(AR[g], AR[g]), aii = make_float2(AI[g], AI[g]); \
+                        acc1[g][2 * m2] = __ffma2_rn(arr, b0, acc1[g][2 * m2]);                  \
+                        acc2[g][2 * m2] = __ffma2_rn(aii, b0, acc2[g][2 * m2]);                  \
+                        acc1[g][2 * m2 + 1] = __ffma2_rn(arr, b1, acc1[g][2 * m2 + 1]);          \
+                        acc2[g][2 * m2 + 1] = __ffma2_rn(aii, b1, acc2[g][2 * m2 + 1]);          \
+                    }                                                                            \
+                }                                                                                \
+            }
+            const int nce = (DDHF_EXP == 3 || DDHF_EXP == 7) ? min(nc, 1) : nc;
+            DDHF_CENTRES(a0r, a0i, 0)
+            int k = 0;
 #pragma unroll 1
-            for (int k = 0; k < ((DDHF_EXP == 3 || DDHF_EXP == 7) ? min(nc, 1) : nc); ++k) {
-                const uint4 ph = phs[min(k + 1, nc - 1)];
-                float arn[TM], ain[TM];
-#pragma unroll
-                for (int g = 0; g < TM; ++g) {
-                    const uint32_t pc = ph.x + static_cast<uint32_t>(lane) * ph.y +
-                                        static_cast<uint32_t>(g * 4 * TN) * ph.z;
-                    float s, c;
-                    sincos_u32(pc, s, c);
-                    arn[g] = c;
-                    ain[g] = -s;
-                }
-                const float4 *brow = reinterpret_cast<const float4 *>(btab + k * TN);
-#pragma unroll
-                for (int m2 = 0; m2 < TN / 2; ++m2) {
-                    const float4 bb = brow[m2];
-                    const float2 b0 = make_float2(bb.x, bb.y), b1 = make_float2(bb.z, bb.w);
-#pragma unroll
-                    for (int g = 0; g < TM; ++g) {
-                        const float2 arr = make_float2(ar[g], ar[g]), aii = make_float2(ai[g], ai[g]);
-                        acc1[g][2 * m2] = __ffma2_rn(arr, b0, acc1[g][2 * m2]);
-                        acc2[g][2 * m2] = __ffma2_rn(aii, b0, acc2[g][2 * m2]);
-                        acc1[g][2 * m2 + 1] = __ffma2_rn(arr, b1, acc1[g][2 * m2 + 1]);
-                        acc2[g][2 * m2 + 1] = __ffma2_rn(aii, b1, acc2[g][2 * m2 + 1]);
-                    }
-                }
-#pragma unroll
-                for (int g = 0; g < TM; ++g) { ar[g] = arn[g]; ai[g] = ain[g]; }
+            for (; k + 1 < nce; k += 2) {
+                DDHF_CENTRES(a1r, a1i, k + 1)
+                DDHF_FMA_BLOCK(a0r, a0i, k)
+                DDHF_CENTRES(a0r, a0i, min(k + 2, nce - 1))
+                DDHF_FMA_BLOCK(a1r, a1i, k + 1)
             }
+            if (k < nce) DDHF_FMA_BLOCK(a0r, a0i, k)
+#undef DDHF_CENTRES
+#undef DDHF_FMA_BLOCK
             __syncwarp();
         }
 
         // the next pixel's work item and first events are fetched under the epilogue
-        idx = __shfl_sync(kFull, next_idx, 0);
+        if (claim_left <= 0) {
+            idx = __shfl_sync(kFull, next_idx, 0);
+            claim_left = __shfl_sync(kFull, next_cnt, 0);
+            if (claim_left == 0) idx = n_items;
+        } else {
+            idx = next_idx;
+        }
+        --claim_left;
         if (idx < n_items) it_next = p.work[idx];
 
         // ---- epilogue: powers, optional spectrum store, spectral flatness -------------------
@@ -649,9 +681,8 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
             slog += __shfl_xor_sync(kFull, slog, o);
             ssum += __shfl_xor_sync(kFull, ssum, o);
         }
-        v_first = 0u;
-        if (idx < n_items && lane < kEC && lane < it_next.n)
-            v_first = __ldg(p.csr_ev + it_next.row_begin + lane);
+        if (idx < n_items && lane < it_next.n)
+            stage_event(ev_s + evb * kEC + lane, p.csr_ev + it_next.row_begin + lane);
         const float inv_nb = 1.f / static_cast<float>(sp.n_freq - sp.k_lo);
         const float mean_p = ssum * inv_nb;
         const float sfv = exp2f(slog * inv_nb) / mean_p;         // eq. 7
