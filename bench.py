@@ -36,47 +36,59 @@ sys.path.insert(0, ROOT)
 
 NOMINAL_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # 74.45: SMs x FP32 lanes x 2 flop x max SM clock
 FLOP_PER_TERM = 4.0                                        # one complex phasor accumulate = 2 FMA
+NDFT_DRAM_BYTES_NCU = 46.4e6                               # profiles/r1a_baseline.md (config 4, no spectra output)
 
 
 class ClockSampler(threading.Thread):
-    """Samples nvidia-smi clocks / throttle reasons while the timed region runs."""
+    """Samples SM clock, power and throttle reasons through NVML while the timed region runs
+    (every 2 ms; `nvidia-smi` takes ~100 ms per query, longer than a whole timed pass)."""
 
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
-         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-         "clocks_event_reasons.sw_power_cap")
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown"}
 
     def __init__(self, index: int):
         super().__init__(daemon=True)
         self.index = index
-        self.samples: list[list[str]] = []
+        self.mhz: list[float] = []
+        self.power: list[float] = []
+        self.reasons: set[str] = set()
+        self.max_mhz = None
         self.stop_flag = threading.Event()
+        self.nvml = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(vis.split(",")[index]) if vis and vis.split(",")[index].isdigit() else index
+            self.handle = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.handle, pynvml.NVML_CLOCK_SM))
+            self.nvml = pynvml
+        except Exception:
+            self.nvml = None
+
+    def sample(self):
+        n = self.nvml
+        self.mhz.append(float(n.nvmlDeviceGetClockInfo(self.handle, n.NVML_CLOCK_SM)))
+        self.power.append(n.nvmlDeviceGetPowerUsage(self.handle) / 1000.0)
+        bits = int(n.nvmlDeviceGetCurrentClocksEventReasons(self.handle))
+        for bit, name in self.REASONS.items():
+            if bits & bit:
+                self.reasons.add(name)
 
     def run(self):
+        if self.nvml is None:
+            return
         while not self.stop_flag.is_set():
             try:
-                out = subprocess.run(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                                      "--format=csv,noheader,nounits"], capture_output=True, text=True,
-                                     timeout=5).stdout.strip()
-                if out:
-                    self.samples.append([s.strip() for s in out.split(",")])
+                self.sample()
             except Exception:
                 pass
-            self.stop_flag.wait(0.1)
+            self.stop_flag.wait(0.002)
 
     def summary(self) -> dict:
-        mhz = [float(s[0]) for s in self.samples if s and s[0].replace(".", "").isdigit()]
-        mx = [float(s[1]) for s in self.samples if len(s) > 1 and s[1].replace(".", "").isdigit()]
-        pw = [float(s[2]) for s in self.samples if len(s) > 2 and s[2].replace(".", "").isdigit()]
-        reasons = set()
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        for s in self.samples:
-            for name, v in zip(names, s[3:7]):
-                if v.lower().startswith("active"):
-                    reasons.add(name)
-        return {"sm_mhz": float(np.median(mhz)) if mhz else None,
-                "sm_max_mhz": float(max(mx)) if mx else None,
-                "power_w_max": float(max(pw)) if pw else None,
-                "samples": len(self.samples), "reasons": sorted(reasons)}
+        return {"sm_mhz": float(np.median(self.mhz)) if self.mhz else None, "sm_max_mhz": self.max_mhz,
+                "power_w_max": float(max(self.power)) if self.power else None,
+                "samples": len(self.mhz), "reasons": sorted(self.reasons),
+                "source": "nvml" if self.nvml is not None else "unavailable"}
 
 
 def load_workload(name: str):
@@ -129,6 +141,20 @@ def time_oracle(w, steps: int, warmup: int):
         terms = terms_of(out, prm["n_freq"], prm["n_min"])
     return dict(value=terms / np.mean(times) / 1e9, unit="Gterms/s", cores=ddhf_oracle.num_threads(),
                 kind="oracle", sample=what, ms_per_step=float(np.mean(times) * 1e3), terms_per_step=terms)
+
+
+def aggregate_over_ranks(time_ms: float, units: float, world: int, device="cpu"):
+    """Whole-job numbers of a replicas-only run: the slowest rank's time and the units of all ranks.
+    The only data exchanged between ranks in this repository."""
+    if world <= 1:
+        return float(time_ms), float(units)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([time_ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    u = torch.tensor([units], device=device, dtype=torch.float64)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
 
 
 def main():
@@ -223,20 +249,12 @@ def main():
         det.window(d_ev, n, t0, w.window_us, offset_events=lo)
         ms = det.stage_ms()
         stage.append(ms)
-        per_step_ms.append(ms[3])
+        per_step_ms.append(ms[4])
     sampler.stop_flag.set()
     sampler.join()
     stage = np.array(stage)
     terms_total = sum(terms_by_win[k][0] for k in wins[warmup:])
-    if world > 1:
-        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-        tt = torch.tensor([terms_total], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.SUM)
-        terms_all = float(tt.item())
-    else:
-        terms_all = float(terms_total)
+    total_ms, terms_all = aggregate_over_ranks(total_ms, terms_total, world, dev)
     value = terms_all / (total_ms * 1e-3) / 1e9
 
     # ---- end to end through the host-buffer entry point -------------------------------------------
@@ -260,11 +278,7 @@ def main():
     barrier()
     e2e_s = time.perf_counter() - t_start
     e2e_terms = sum(terms_by_win[k][0] for k in wins[warmup:warmup + e2e_steps])
-    if world > 1:
-        t = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
-        e2e_terms *= world
+    e2e_s, e2e_terms = aggregate_over_ranks(e2e_s, e2e_terms, world, dev)
     d2h = NP + 32 + 24 * int(h_cnt[3])
     e2e = {"value": e2e_terms / e2e_s / 1e9, "unit": "Gterms/s", "ms_per_step": e2e_s / e2e_steps * 1e3,
            "h2d_bytes_per_step": h2d // e2e_steps, "d2h_bytes_per_step": d2h, "steps": e2e_steps}
@@ -280,7 +294,10 @@ def main():
     achieved = terms_per_step * FLOP_PER_TERM / (ndft_ms * 1e-3) / 1e12
     probe = binding.ddhf_fma_peak_probe(20.0)
     roofline = {"bound": "alu", "kernel": "k_ndft_score", "achieved": achieved, "peak": NOMINAL_FP32_TFLOPS,
-                "unit": "TFLOP/s", "frac": achieved / NOMINAL_FP32_TFLOPS, "traffic": None,
+                "unit": "TFLOP/s", "frac": achieved / NOMINAL_FP32_TFLOPS,
+                "traffic": NDFT_DRAM_BYTES_NCU if args.workload == "cfg4" and not args.spectra else None,
+                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture "
+                                  "(profiles/), config 4, per launch",
                 "peak_kind": "nominal FP32 FMA: 148 SM x 128 lanes x 2 flop x 1.965 GHz (DESIGN.md section 5)",
                 "flop_per_term": FLOP_PER_TERM, "kernel_ms": ndft_ms,
                 "gterms_per_s_kernel": terms_per_step / (ndft_ms * 1e-3) / 1e9,
@@ -302,7 +319,8 @@ def main():
                    "l2": "inputs larger than L2 (events %.0f MB + pairs + csr per step)" % (16 * res0["n_in"] / 1e6),
                    "replicas": world},
         "latency_ms": {"p50": float(np.percentile(per_step_ms, 50)), "p99": float(np.percentile(per_step_ms, 99)),
-                       "ingest": float(stage[:, 0].mean()), "ndft_score": ndft_ms, "ccl": float(stage[:, 2].mean())},
+                       "ingest": float(stage[:, 0].mean()), "ndft": ndft_ms, "comb_score": float(stage[:, 2].mean()),
+                       "ccl": float(stage[:, 3].mean())},
         "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": launches_per_window * steps,
         "roofline": roofline,
         "paper_context": "DDHF 2.39 ms/frame, YOLOv11-n 12.40 ms/frame on an NVIDIA L40-8Q, 33.3 ms windows (PAPER.md L154-156)",

@@ -160,8 +160,9 @@ int ddhf_window_host(ddhf_handle *h, const ddhf_event *h_events, int64_t n, int6
                      int64_t window_us, const ddhf_host_outputs *out, void *cuda_stream);
 
 /* With DDHF_FLAG_TIMING: waits for the last ddhf_window() on this handle and returns the
- * device time of its stages in ms: [0] ingest a0-a3, [1] NDFT + scoring a4-a7,
- * [2] CCL + boxes a8, [3] total.  ms: HOST float[4]. */
+ * device time of its stages in ms: [0] ingest a0-a3, [1] the NDFT kernel (a4, a5 and the
+ * queueing of the spectra to score), [2] deferred comb scoring a6-a7, [3] CCL + boxes a8,
+ * [4] total.  ms: HOST float[5]. */
 int ddhf_stage_ms(ddhf_handle *h, float *ms);
 
 /* Number of kernels ddhf_window() launches per call (constant for a handle). */

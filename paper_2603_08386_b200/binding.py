@@ -148,7 +148,7 @@ def ddhf_window_host(h, h_events_ptr: int, n: int, t0_us: int, window_us: int,
 
 
 def ddhf_stage_ms(h) -> list[float]:
-    ms = (C.c_float * 4)()
+    ms = (C.c_float * 5)()
     rc = lib().ddhf_stage_ms(h, ms)
     if rc != DDHF_OK:
         raise DdhfError(rc, (lib().ddhf_last_error(h) or b"").decode())

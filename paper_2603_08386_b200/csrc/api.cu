@@ -31,7 +31,7 @@ struct ddhf_handle {
     // workspace offsets (bytes)
     size_t off_cnt = 0, off_pairs = 0, off_work = 0, off_tiles = 0, off_class = 0, off_cursor = 0, off_thist = 0, off_chunk = 0, off_binbase = 0, off_spill = 0, off_spillrec = 0,
            off_parent = 0, off_slot = 0, off_comp = 0, off_comp_label = 0, off_ctiles = 0, ws_bytes = 0;
-    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     bool timed_once = false;
     // buffers of the host-buffer variant
     ddhf_event *hb_events = nullptr;
@@ -209,7 +209,7 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
     h->ws_bytes = o;
 
     if (c.flags & DDHF_FLAG_TIMING)
-        for (int i = 0; i < 4; ++i) cudaEventCreate(&h->ev[i]);
+        for (int i = 0; i < 5; ++i) cudaEventCreate(&h->ev[i]);
     *out = h;
     return DDHF_OK;
 }
@@ -291,10 +291,10 @@ extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n
     if (timing) cudaEventRecord(h->ev[0], st);
     launches += launch_ingest(ip, st);
     if (timing) cudaEventRecord(h->ev[1], st);
-    launches += launch_ndft(np, c.n_freq, h->sm_count, st);
-    if (timing) cudaEventRecord(h->ev[2], st);
+    launches += launch_ndft(np, c.n_freq, h->sm_count, st, timing ? h->ev[2] : nullptr);
+    if (timing) cudaEventRecord(h->ev[3], st);
     launches += launch_ccl(cp, st);
-    if (timing) { cudaEventRecord(h->ev[3], st); h->timed_once = true; }
+    if (timing) { cudaEventRecord(h->ev[4], st); h->timed_once = true; }
     h->launches = launches;
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(h, DDHF_E_CUDA, std::string("ddhf_window: ") + cudaGetErrorString(e));
@@ -306,12 +306,10 @@ extern "C" int ddhf_stage_ms(ddhf_handle *h, float *ms)
     if (!h || !ms) return DDHF_E_INVAL;
     if (!(h->cfg.flags & DDHF_FLAG_TIMING) || !h->timed_once)
         return fail(h, DDHF_E_INVAL, "ddhf_stage_ms: handle was not created with DDHF_FLAG_TIMING or no window ran");
-    if (cudaEventSynchronize(h->ev[3]) != cudaSuccess)
+    if (cudaEventSynchronize(h->ev[4]) != cudaSuccess)
         return fail(h, DDHF_E_CUDA, std::string("ddhf_stage_ms: ") + cudaGetErrorString(cudaGetLastError()));
-    cudaEventElapsedTime(&ms[0], h->ev[0], h->ev[1]);
-    cudaEventElapsedTime(&ms[1], h->ev[1], h->ev[2]);
-    cudaEventElapsedTime(&ms[2], h->ev[2], h->ev[3]);
-    cudaEventElapsedTime(&ms[3], h->ev[0], h->ev[3]);
+    for (int i = 0; i < 4; ++i) cudaEventElapsedTime(&ms[i], h->ev[i], h->ev[i + 1]);
+    cudaEventElapsedTime(&ms[4], h->ev[0], h->ev[4]);
     return DDHF_OK;
 }
 
@@ -389,7 +387,7 @@ extern "C" int ddhf_destroy(ddhf_handle *h)
 {
     if (!h) return DDHF_OK;
     if (h->d_cand) cudaFree(h->d_cand);
-    for (int i = 0; i < 4; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
+    for (int i = 0; i < 5; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
     if (h->hb_events) cudaFree(h->hb_events);
     if (h->hb_ws) cudaFree(h->hb_ws);
     void *bufs[] = {h->hb_out.row_ptr, h->hb_out.csr_ev, h->hb_out.active_idx, h->hb_out.power,

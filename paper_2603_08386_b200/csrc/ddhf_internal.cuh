@@ -121,7 +121,8 @@ int launch_ingest(const IngestParams &p, cudaStream_t st);
 cudaError_t ingest_configure();              // opt in to large dynamic shared memory
 int ingest_tile_events();                    // events per partition tile
 int ingest_chunk_tiles();                    // tiles per scan chunk
-int launch_ndft(const NdftParams &p, int n_freq, int sm_count, cudaStream_t st);
+int launch_ndft(const NdftParams &p, int n_freq, int sm_count, cudaStream_t st, cudaEvent_t between);
+                                             // `between` (optional) is recorded after the NDFT kernel, before the scoring kernel
 int launch_ccl(const CclParams &p, cudaStream_t st);
 int ndft_bins_per_lane(int n_freq);          // 8, 16, 32 or 64
 int ndft_tn(int n_freq);                     // offset pairs per centre for that kernel

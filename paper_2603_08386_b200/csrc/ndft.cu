@@ -778,7 +778,7 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 4) k_comb_deferred(NdftParam
 }
 
 template <int TM, int TN, int BS>
-int launch_one(const NdftParams &p, int sm_count, cudaStream_t st)
+int launch_one(const NdftParams &p, int sm_count, cudaStream_t st, cudaEvent_t between)
 {
     using L = Layout<TM, TN, BS>;
     static bool configured = false;
@@ -798,6 +798,7 @@ int launch_one(const NdftParams &p, int sm_count, cudaStream_t st)
         configured = true;
     }
     k_ndft_score<TM, TN, BS><<<sm_count * blocks_per_sm, kWarps * 32, L::SMEM_BYTES, st>>>(p);
+    if (between) cudaEventRecord(between, st);
     k_comb_deferred<TM, TN, BS><<<sm_count * score_blocks_per_sm, kScoreWarps * 32, score_smem, st>>>(p);
     return 2;
 }
@@ -830,16 +831,16 @@ int ndft_band_size(int n_freq, int r0, int r1)
     return 0;
 }
 
-int launch_ndft(const NdftParams &p, int n_freq, int sm_count, cudaStream_t st)
+int launch_ndft(const NdftParams &p, int n_freq, int sm_count, cudaStream_t st, cudaEvent_t between)
 {
     const int nbl = ndft_bins_per_lane(n_freq);
     const int bs = ndft_band_size(n_freq, p.sp.r0, p.sp.r1);
-    if (nbl == 8) return launch_one<1, 4, 256>(p, sm_count, st);
-    if (nbl == 16) return bs == 256 ? launch_one<1, 8, 256>(p, sm_count, st) : launch_one<1, 8, 512>(p, sm_count, st);
-    if (nbl == 32) return bs == 256 ? launch_one<1, 16, 256>(p, sm_count, st) : launch_one<1, 16, 512>(p, sm_count, st);
-    if (bs == 256) return launch_one<2, 16, 256>(p, sm_count, st);
-    if (bs == 512) return launch_one<2, 16, 512>(p, sm_count, st);
-    return launch_one<2, 16, 1024>(p, sm_count, st);
+    if (nbl == 8) return launch_one<1, 4, 256>(p, sm_count, st, between);
+    if (nbl == 16) return bs == 256 ? launch_one<1, 8, 256>(p, sm_count, st, between) : launch_one<1, 8, 512>(p, sm_count, st, between);
+    if (nbl == 32) return bs == 256 ? launch_one<1, 16, 256>(p, sm_count, st, between) : launch_one<1, 16, 512>(p, sm_count, st, between);
+    if (bs == 256) return launch_one<2, 16, 256>(p, sm_count, st, between);
+    if (bs == 512) return launch_one<2, 16, 512>(p, sm_count, st, between);
+    return launch_one<2, 16, 1024>(p, sm_count, st, between);
 }
 
 }  // namespace ddhf

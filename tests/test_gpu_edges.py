@@ -195,7 +195,7 @@ def test_host_buffer_entry_point_matches_device_path():
     for _ in range(2):                       # second call reuses the handle's buffers
         binding.ddhf_window_host(h, ev.data_ptr(), len(w.events), 0, w.window_us, out, 0)
     ms = binding.ddhf_stage_ms(h)
-    assert all(m >= 0 for m in ms) and abs(ms[3] - sum(ms[:3])) < 0.05 * ms[3] + 0.01
+    assert len(ms) == 5 and all(m >= 0 for m in ms) and abs(ms[4] - sum(ms[:4])) < 0.05 * ms[4] + 0.01
     assert binding.ddhf_launches_per_window(h) >= 10
     binding.ddhf_destroy(h)
     n_in, n_act, n_box = (int(host["counters"][i]) for i in (0, 2, 3))
