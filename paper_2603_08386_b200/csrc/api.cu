@@ -20,7 +20,6 @@ struct ddhf_handle {
     int np = 0;
     int sm_count = 0;
     int n_tiles = 0;
-    int comp_cap = 0;
     int launches = 0;
     int bits1 = 1, bits2 = 1;
     int chunk_words = 0;
@@ -30,7 +29,7 @@ struct ddhf_handle {
     CandTable *d_cand = nullptr;
     // workspace offsets (bytes)
     size_t off_cnt = 0, off_pairs = 0, off_work = 0, off_tiles = 0, off_class = 0, off_cursor = 0, off_thist = 0, off_chunk = 0, off_binbase = 0, off_spill = 0, off_spillrec = 0,
-           off_parent = 0, off_slot = 0, off_comp = 0, off_comp_label = 0, off_ctiles = 0, ws_bytes = 0;
+           off_parent = 0, off_rec = 0, off_ctiles = 0, ws_bytes = 0;
     cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     bool timed_once = false;
     // buffers of the host-buffer variant
@@ -168,7 +167,6 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
 
     // ---- workspace layout -----------------------------------------------------------------------
     h->n_tiles = (h->np + kScanTile - 1) / kScanTile;
-    h->comp_cap = ((c.width + 1) / 2) * ((c.height + 1) / 2);     // most 8-connected components possible
     size_t o = 0;
     h->off_cnt = o;        o = align_up(o + sizeof(int32_t) * h->np);
     h->off_pairs = o;      o = align_up(o + sizeof(uint64_t) * static_cast<size_t>(c.max_events));
@@ -202,10 +200,8 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
     h->off_spill = o;      o = align_up(o + sizeof(float) * static_cast<size_t>(h->spill_cap) * ndft_padded_bins(c.n_freq));
     h->off_spillrec = o;   o = align_up(o + sizeof(SpillRec) * static_cast<size_t>(h->spill_cap));
     h->off_parent = o;     o = align_up(o + sizeof(int32_t) * h->np);
-    h->off_slot = o;       o = align_up(o + sizeof(int32_t) * h->np);
-    h->off_comp = o;       o = align_up(o + sizeof(int32_t) * 5 * static_cast<size_t>(h->comp_cap));
-    h->off_comp_label = o; o = align_up(o + sizeof(int32_t) * static_cast<size_t>(h->comp_cap));
-    h->off_ctiles = o;     o = align_up(o + sizeof(int32_t) * 2 * 1024);
+    h->off_rec = o;        o = align_up(o + sizeof(int32_t) * 5 * static_cast<size_t>(h->np));
+    h->off_ctiles = o;     o = align_up(o + sizeof(int32_t) * 1024);
     h->ws_bytes = o;
 
     if (c.flags & DDHF_FLAG_TIMING)
@@ -236,6 +232,7 @@ extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n
     const ddhf_config &c = h->cfg;
     const bool timing = (c.flags & DDHF_FLAG_TIMING) != 0;
 
+    int32_t *cp_parent = out->labels ? out->labels : reinterpret_cast<int32_t *>(ws + h->off_parent);
     IngestParams ip{};
     ip.events = d_events; ip.n = n; ip.t0 = t0_us; ip.t1 = t0_us + window_us;
     ip.width = c.width; ip.height = c.height; ip.np = h->np;
@@ -262,6 +259,8 @@ extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n
     ip.bin_tot = ip.bin_base2 + (1 << h->bits1);
     ip.scan_done = reinterpret_cast<int32_t *>(ws + h->off_cursor + 16);     // [2], followed by the spill counter
 
+    ip.ccl_parent = cp_parent;
+
     NdftParams np{};
     np.work = ip.work; np.csr_ev = out->csr_ev; np.counters = out->counters;
     np.work_cursor = ip.work_cursor; np.max_active = c.max_active;
@@ -278,13 +277,9 @@ extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n
     CclParams cp{};
     cp.mask = out->mask; cp.width = c.width; cp.height = c.height; cp.np = h->np;
     cp.a_min = c.a_min; cp.max_boxes = c.max_boxes;
-    cp.parent = out->labels ? out->labels : reinterpret_cast<int32_t *>(ws + h->off_parent);
-    cp.slot = reinterpret_cast<int32_t *>(ws + h->off_slot);
-    int32_t *ct = reinterpret_cast<int32_t *>(ws + h->off_ctiles);
-    cp.tile_sum = ct; cp.tile_off = ct + 1024;
-    cp.comp = reinterpret_cast<int32_t *>(ws + h->off_comp);
-    cp.comp_cap = h->comp_cap;
-    cp.comp_label = reinterpret_cast<int32_t *>(ws + h->off_comp_label);
+    cp.parent = cp_parent;
+    cp.rec = reinterpret_cast<int32_t *>(ws + h->off_rec);
+    cp.tile_sum = reinterpret_cast<int32_t *>(ws + h->off_ctiles);
     cp.boxes = out->boxes; cp.counters = out->counters;
 
     int launches = 0;

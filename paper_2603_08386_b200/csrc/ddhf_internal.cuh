@@ -98,19 +98,16 @@ struct IngestParams {
     int32_t *f0_idx;
     uint8_t *mask;
     unsigned long long *work_cursor;
+    int32_t *ccl_parent;         // [np] union-find array of the CCL stage, reset here
 };
 
 struct CclParams {
     const uint8_t *mask;
     int32_t width, height, np;
     int32_t a_min, max_boxes;
-    int32_t *parent;             // [np] = labels output or workspace
-    int32_t *slot;               // [np] root pixel -> component slot
-    int32_t *tile_sum, *tile_off;
-    int32_t *comp;               // [np/4+1][5] x0,y0,x1,y1,n per component slot (capped)
-    int32_t comp_cap;
-    int32_t *comp_label;         // [comp_cap]
-    int32_t *keep_off;           // [comp_cap] scan of the A_min filter
+    int32_t *parent;             // [np] = labels output or workspace; arrives filled with INT_MAX
+    int32_t *rec;                // [np][5] x0,y0,x1,y1,n of the component rooted at the pixel (mask pixels only)
+    int32_t *tile_sum;           // [<= 1024] boxes that pass A_min per tile of 4096 pixels
     ddhf_box *boxes;
     int32_t *counters;
 };

@@ -73,6 +73,7 @@ __global__ void k_init(IngestParams p)
         p.score[i] = 0.f;
         p.f0_idx[i] = -1;
         p.mask[i] = 0;
+        p.ccl_parent[i] = 0x7fffffff;           // no parent yet
     }
     for (int k = i; k < p.chunk_words; k += gridDim.x * blockDim.x) p.chunk1[k] = 0;   // chunk1, chunk2
     if (blockIdx.x == 0) {
