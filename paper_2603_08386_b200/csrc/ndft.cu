@@ -475,7 +475,8 @@ __device__ __forceinline__ void comb_score(const float (&preg)[TM * 2 * TN], flo
 // ----------------------------------------------------------------------------------------
 // The fused kernel.
 // ----------------------------------------------------------------------------------------
-template <int TM, int TN, int BS>
+// FULL: n_freq fills the padded grid (n_freq == 32 NBL) and k_lo <= 32, so no per-bin range checks
+template <int TM, int TN, int BS, bool FULL>
 #ifdef DDHF_NDFT_MAXNREG
 __global__ void __maxnreg__(DDHF_NDFT_MAXNREG) k_ndft_score(NdftParams p)
 #else
@@ -495,7 +496,7 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
     const int n_items = p.counters[DDHF_CNT_N_ACTIVE];
     const ScoreParams &sp = p.sp;
     constexpr int EPP = 32 / TN;       // events per table pass
-    const bool full_grid = (sp.n_freq == L::NB) && (sp.k_lo <= 32);
+    constexpr bool full_grid = FULL;
     const bool store_power = p.power != nullptr;
 
     // dynamic work queue with one item of look-ahead: the next work item is loaded while the
@@ -646,25 +647,38 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
             float *dst = p.power + static_cast<size_t>(it.arow) * sp.n_freq + lane;
 #pragma unroll
             for (int i = 0; i < NBL; ++i)
-                if (i * 32 + lane < sp.n_freq) __stcs(dst + i * 32, preg[i]);
+                if (full_grid || i * 32 + lane < sp.n_freq) __stcs(dst + i * 32, preg[i]);
         }
         float slog = 0.f, ssum = 0.f;
         if (DDHF_EXP == 1 || DDHF_EXP == 5) {
             slog = preg[3]; ssum = preg[5] + 1.f;
         } else if (full_grid) {
-            // every bin is in range; only the first k_lo bins (register 0) are left out
-            {
-                const float pt = fmaxf(preg[0], sp.sf_eps);
-                const bool in = lane >= sp.k_lo;
-                slog = in ? __log2f(pt) : 0.f;
-                ssum = in ? pt : 0.f;
-            }
+            // every bin is in range; only the first k_lo bins (register 0) are left out.  Bins are
+            // taken in pairs, log2(a b) = log2 a + log2 b (one SFU op per two bins; a b stays a
+            // normal number: sf_eps^2 >= 1e-36 is checked, P <= n^2 < 2^62), four partial sums
+            const bool in0 = lane >= sp.k_lo;
+            float sl[4] = {0.f, 0.f, 0.f, 0.f}, ss[4] = {0.f, 0.f, 0.f, 0.f};
+            if (sp.sf_eps >= 1e-18f) {
 #pragma unroll
-            for (int i = 1; i < NBL; ++i) {
-                const float pt = fmaxf(preg[i], sp.sf_eps);
-                slog += __log2f(pt);
-                ssum += pt;
+                for (int i = 0; i < NBL; i += 2) {
+                    float a = fmaxf(preg[i], sp.sf_eps);
+                    const float b = fmaxf(preg[i + 1], sp.sf_eps);
+                    float sa = a;
+                    if (i == 0) { sa = in0 ? a : 0.f; a = in0 ? a : 1.f; }
+                    sl[(i >> 1) & 3] += __log2f(a * b);
+                    ss[(i >> 1) & 3] += sa + b;
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < NBL; ++i) {
+                    const float pt = fmaxf(preg[i], sp.sf_eps);
+                    const bool in = (i > 0) || in0;
+                    sl[i & 3] += in ? __log2f(pt) : 0.f;
+                    ss[i & 3] += in ? pt : 0.f;
+                }
             }
+            slog = (sl[0] + sl[1]) + (sl[2] + sl[3]);
+            ssum = (ss[0] + ss[1]) + (ss[2] + ss[3]);
         } else {
 #pragma unroll
             for (int i = 0; i < NBL; ++i) {
@@ -777,7 +791,7 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 4) k_comb_deferred(NdftParam
     if (blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(p.n_scored, n_rows);
 }
 
-template <int TM, int TN, int BS>
+template <int TM, int TN, int BS, bool FULL>
 int launch_one(const NdftParams &p, int sm_count, cudaStream_t st, cudaEvent_t between)
 {
     using L = Layout<TM, TN, BS>;
@@ -785,9 +799,9 @@ int launch_one(const NdftParams &p, int sm_count, cudaStream_t st, cudaEvent_t b
     static int blocks_per_sm = 1, score_blocks_per_sm = 1;
     constexpr size_t score_smem = static_cast<size_t>(((L::P_WORDS + L::SCORE_WORDS + 3) / 4) * 4) * 4 * kScoreWarps;
     if (!configured) {
-        cudaFuncSetAttribute(k_ndft_score<TM, TN, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaFuncSetAttribute(k_ndft_score<TM, TN, BS, FULL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              static_cast<int>(L::SMEM_BYTES));
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, k_ndft_score<TM, TN, BS>,
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, k_ndft_score<TM, TN, BS, FULL>,
                                                       kWarps * 32, L::SMEM_BYTES);
         if (blocks_per_sm < 1) blocks_per_sm = 1;
         cudaFuncSetAttribute(k_comb_deferred<TM, TN, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -797,7 +811,7 @@ int launch_one(const NdftParams &p, int sm_count, cudaStream_t st, cudaEvent_t b
         if (score_blocks_per_sm < 1) score_blocks_per_sm = 1;
         configured = true;
     }
-    k_ndft_score<TM, TN, BS><<<sm_count * blocks_per_sm, kWarps * 32, L::SMEM_BYTES, st>>>(p);
+    k_ndft_score<TM, TN, BS, FULL><<<sm_count * blocks_per_sm, kWarps * 32, L::SMEM_BYTES, st>>>(p);
     if (between) cudaEventRecord(between, st);
     k_comb_deferred<TM, TN, BS><<<sm_count * score_blocks_per_sm, kScoreWarps * 32, score_smem, st>>>(p);
     return 2;
@@ -831,16 +845,28 @@ int ndft_band_size(int n_freq, int r0, int r1)
     return 0;
 }
 
+namespace {
+
+template <int TM, int TN, int BS>
+int launch_full(const NdftParams &p, bool full, int sm_count, cudaStream_t st, cudaEvent_t between)
+{
+    return full ? launch_one<TM, TN, BS, true>(p, sm_count, st, between)
+                : launch_one<TM, TN, BS, false>(p, sm_count, st, between);
+}
+
+}  // namespace
+
 int launch_ndft(const NdftParams &p, int n_freq, int sm_count, cudaStream_t st, cudaEvent_t between)
 {
+    const bool full = (n_freq == ndft_bins_per_lane(n_freq) * 32) && (p.sp.k_lo <= 32);
     const int nbl = ndft_bins_per_lane(n_freq);
     const int bs = ndft_band_size(n_freq, p.sp.r0, p.sp.r1);
-    if (nbl == 8) return launch_one<1, 4, 256>(p, sm_count, st, between);
-    if (nbl == 16) return bs == 256 ? launch_one<1, 8, 256>(p, sm_count, st, between) : launch_one<1, 8, 512>(p, sm_count, st, between);
-    if (nbl == 32) return bs == 256 ? launch_one<1, 16, 256>(p, sm_count, st, between) : launch_one<1, 16, 512>(p, sm_count, st, between);
-    if (bs == 256) return launch_one<2, 16, 256>(p, sm_count, st, between);
-    if (bs == 512) return launch_one<2, 16, 512>(p, sm_count, st, between);
-    return launch_one<2, 16, 1024>(p, sm_count, st, between);
+    if (nbl == 8) return launch_full<1, 4, 256>(p, full, sm_count, st, between);
+    if (nbl == 16) return bs == 256 ? launch_full<1, 8, 256>(p, full, sm_count, st, between) : launch_full<1, 8, 512>(p, full, sm_count, st, between);
+    if (nbl == 32) return bs == 256 ? launch_full<1, 16, 256>(p, full, sm_count, st, between) : launch_full<1, 16, 512>(p, full, sm_count, st, between);
+    if (bs == 256) return launch_full<2, 16, 256>(p, full, sm_count, st, between);
+    if (bs == 512) return launch_full<2, 16, 512>(p, full, sm_count, st, between);
+    return launch_full<2, 16, 1024>(p, full, sm_count, st, between);
 }
 
 }  // namespace ddhf
