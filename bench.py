@@ -36,7 +36,7 @@ sys.path.insert(0, ROOT)
 
 NOMINAL_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # 74.45: SMs x FP32 lanes x 2 flop x max SM clock
 FLOP_PER_TERM = 4.0                                        # one complex phasor accumulate = 2 FMA
-NDFT_DRAM_BYTES_NCU = 46.4e6                               # profiles/r1a_baseline.md (config 4, no spectra output)
+NDFT_DRAM_BYTES_NCU = 83.7e6                               # profiles/r1b_summary.md (config 4, no spectra output)
 
 
 class ClockSampler(threading.Thread):
