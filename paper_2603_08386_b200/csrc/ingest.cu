@@ -258,6 +258,25 @@ __global__ void __launch_bounds__(1024) k_binscan(IngestParams p)
 // event's rank inside (tile, digit) follows input order exactly.  The tile is then laid out in
 // shared memory in output order (bin-major) and written with consecutive threads on
 // consecutive elements, so that every run of a bin is a coalesced store.
+// Slow path of the ranking step (two lanes of the warp share a digit): lanes with the same digit
+// find each other by one ballot per digit bit (MATCH.ANY is far slower on sm_100); the lowest lane
+// of a group writes the group's count.  Kept out of line so that the common conflict-free step
+// does not pay for it.
+__device__ __noinline__ uint32_t rank_by_ballots(bool ok, uint32_t d, uint32_t c, int lane, unsigned short *my_cnt)
+{
+    const uint32_t lt = (1u << lane) - 1u;
+    uint32_t peers = __ballot_sync(kFullMask, ok);
+#pragma unroll
+    for (int k = 0; k < 11; ++k) {
+        const bool bit = (d >> k) & 1u;
+        const uint32_t bal = __ballot_sync(kFullMask, bit);
+        peers &= bit ? bal : ~bal;
+    }
+    if (ok && (peers & lt) == 0u) my_cnt[d] = static_cast<unsigned short>(c + __popc(peers));
+    __syncwarp();
+    return c + __popc(peers & lt);
+}
+
 template <int PASS>
 struct PartSmem {
     // words: base[bins] | binoff[bins] | wcnt[kTileWarps][bins] (u16) | stage
@@ -337,20 +356,7 @@ __global__ void __launch_bounds__(kTileThreads, 2) k_part(IngestParams p)
         __syncwarp();
         const bool lost = ok && (static_cast<uint32_t>(my_cnt[d]) >> 11) != static_cast<uint32_t>(lane);
         uint32_t rank = c;
-        if (__any_sync(kFullMask, lost)) {
-            // lanes with the same digit, by one ballot per digit bit (MATCH.ANY is far slower on
-            // sm_100); the lowest lane of a group writes the group's count
-            uint32_t peers = __ballot_sync(kFullMask, ok);
-#pragma unroll
-            for (int k = 0; k < 11; ++k) {
-                const bool bit = (d >> k) & 1u;
-                const uint32_t bal = __ballot_sync(kFullMask, bit);
-                peers &= bit ? bal : ~bal;
-            }
-            if (ok && (peers & lt) == 0u) my_cnt[d] = static_cast<unsigned short>(c + __popc(peers));
-            rank = c + __popc(peers & lt);
-            __syncwarp();
-        }
+        if (__any_sync(kFullMask, lost)) rank = rank_by_ballots(ok, d, c, lane, my_cnt);
         key[s] = ok ? (d | (rank << 16)) : 0xffffffffu;
     }
     __syncthreads();
