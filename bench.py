@@ -257,31 +257,53 @@ def main():
     total_ms, terms_all = aggregate_over_ranks(total_ms, terms_total, world, dev)
     value = terms_all / (total_ms * 1e-3) / 1e9
 
-    # ---- end to end through the host-buffer entry point -------------------------------------------
+    # ---- end to end through the host-buffer entry points -------------------------------------------
+    # e2e: ddhf_host_submit / ddhf_host_wait (two windows in flight: the 16 B/event host->device copy
+    # of window i+1 overlaps the kernels of window i); every step copies its events from pinned host
+    # memory and reads mask, boxes and counters back.  e2e_serial: ddhf_window_host, one window at a
+    # time (copy, kernels, copy back, synchronise).
     NP = prm["width"] * prm["height"]
     h_ev = torch.from_numpy(np.ascontiguousarray(w.events).view(np.uint8).copy()).pin_memory()
-    h_mask = torch.zeros(NP, dtype=torch.uint8).pin_memory()
-    h_boxes = torch.zeros(det.cfg.max_boxes * 6, dtype=torch.int32).pin_memory()
-    h_cnt = torch.zeros(8, dtype=torch.int32).pin_memory()
-    hout = binding.DdhfHostOutputs()
-    hout.mask, hout.boxes, hout.counters = h_mask.data_ptr(), h_boxes.data_ptr(), h_cnt.data_ptr()
+    houts, hbufs = [], []
+    for _ in range(2):
+        t = (torch.zeros(NP, dtype=torch.uint8).pin_memory(),
+             torch.zeros(det.cfg.max_boxes * 6, dtype=torch.int32).pin_memory(),
+             torch.zeros(8, dtype=torch.int32).pin_memory())
+        o = binding.DdhfHostOutputs()
+        o.mask, o.boxes, o.counters = t[0].data_ptr(), t[1].data_ptr(), t[2].data_ptr()
+        hbufs.append(t)
+        houts.append(o)
     st = torch.cuda.current_stream(dev).cuda_stream
     e2e_steps = min(steps, 10)
-    for lo, n, t0 in wins[:2]:
-        binding.ddhf_window_host(det.h, h_ev.data_ptr() + 16 * lo, n, t0, w.window_us, hout, st)
-    barrier()
-    t_start = time.perf_counter()
-    h2d = 0
-    for lo, n, t0 in wins[warmup:warmup + e2e_steps]:
-        binding.ddhf_window_host(det.h, h_ev.data_ptr() + 16 * lo, n, t0, w.window_us, hout, st)
-        h2d += 16 * n
-    barrier()
-    e2e_s = time.perf_counter() - t_start
-    e2e_terms = sum(terms_by_win[k][0] for k in wins[warmup:warmup + e2e_steps])
-    e2e_s, e2e_terms = aggregate_over_ranks(e2e_s, e2e_terms, world, dev)
-    d2h = NP + 32 + 24 * int(h_cnt[3])
-    e2e = {"value": e2e_terms / e2e_s / 1e9, "unit": "Gterms/s", "ms_per_step": e2e_s / e2e_steps * 1e3,
-           "h2d_bytes_per_step": h2d // e2e_steps, "d2h_bytes_per_step": d2h, "steps": e2e_steps}
+    e2e_wins = wins[warmup:warmup + e2e_steps]
+
+    def run_pipelined(ws):
+        for i, (lo, n, t0) in enumerate(ws):
+            binding.ddhf_host_submit(det.h, h_ev.data_ptr() + 16 * lo, n, t0, w.window_us, houts[i & 1], st)
+            if i >= 1:
+                binding.ddhf_host_wait(det.h)
+        binding.ddhf_host_wait(det.h)
+
+    def run_serial(ws):
+        for lo, n, t0 in ws:
+            binding.ddhf_window_host(det.h, h_ev.data_ptr() + 16 * lo, n, t0, w.window_us, houts[0], st)
+
+    e2e_terms = sum(terms_by_win[k][0] for k in e2e_wins)
+    h2d = sum(16 * n for _, n, _ in e2e_wins)
+    d2h = NP + 32 + 24 * det.cfg.max_boxes
+    results = {}
+    for name, fn in (("pipelined", run_pipelined), ("serial", run_serial)):
+        fn(wins[:2])
+        barrier()
+        t_start = time.perf_counter()
+        fn(e2e_wins)
+        barrier()
+        sec, terms_e = aggregate_over_ranks((time.perf_counter() - t_start) * 1e3, e2e_terms, world, dev)
+        sec *= 1e-3
+        results[name] = {"value": terms_e / sec / 1e9, "unit": "Gterms/s", "ms_per_step": sec / e2e_steps * 1e3,
+                         "h2d_bytes_per_step": h2d // e2e_steps, "d2h_bytes_per_step": d2h, "steps": e2e_steps}
+    e2e = dict(results["pipelined"], api="ddhf_host_submit/ddhf_host_wait, 2 windows in flight")
+    e2e_serial = dict(results["serial"], api="ddhf_window_host")
 
     if rank != 0:
         if world > 1:
@@ -321,7 +343,7 @@ def main():
         "latency_ms": {"p50": float(np.percentile(per_step_ms, 50)), "p99": float(np.percentile(per_step_ms, 99)),
                        "ingest": float(stage[:, 0].mean()), "ndft": ndft_ms, "comb_score": float(stage[:, 2].mean()),
                        "ccl": float(stage[:, 3].mean())},
-        "clocks": sampler.summary(), "e2e": e2e, "gpu_launches": launches_per_window * steps,
+        "clocks": sampler.summary(), "e2e": e2e, "e2e_serial": e2e_serial, "gpu_launches": launches_per_window * steps,
         "roofline": roofline,
         "paper_context": "DDHF 2.39 ms/frame, YOLOv11-n 12.40 ms/frame on an NVIDIA L40-8Q, 33.3 ms windows (PAPER.md L154-156)",
     }

@@ -159,6 +159,21 @@ int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n, int64_t t
 int ddhf_window_host(ddhf_handle *h, const ddhf_event *h_events, int64_t n, int64_t t0_us,
                      int64_t window_us, const ddhf_host_outputs *out, void *cuda_stream);
 
+/* Pipelined end-to-end variant (two windows in flight): ddhf_host_submit() enqueues the
+ * host->device copy of the events on an internal copy stream, the window on `cuda_stream`
+ * (after the copy) and the device->host copies of the requested outputs, and returns without
+ * waiting, so that the copy of window i+1 overlaps the kernels of window i (SURVEY 8(f)-3:
+ * double-buffered H2D).  ddhf_host_wait() blocks until the OLDEST submitted window is complete;
+ * its outputs are then valid.  h_events and every buffer named in `out` are HOST memory (pinned,
+ * or the copies are not asynchronous) and must stay valid and untouched until that wait returns.
+ * Only the fixed-size outputs are supported here: row_ptr, sf, score, f0_idx, mask, labels, boxes
+ * (all max_boxes records are copied) and counters; csr_ev, active_idx and power must be NULL.
+ * Errors: DDHF_E_INVAL (NULL arguments, unsupported output requested, more than two windows in
+ * flight on submit, none in flight on wait), DDHF_E_CAPACITY, DDHF_E_CUDA. */
+int ddhf_host_submit(ddhf_handle *h, const ddhf_event *h_events, int64_t n, int64_t t0_us,
+                     int64_t window_us, const ddhf_host_outputs *out, void *cuda_stream);
+int ddhf_host_wait(ddhf_handle *h);
+
 /* With DDHF_FLAG_TIMING: waits for the last ddhf_window() on this handle and returns the
  * device time of its stages in ms: [0] ingest a0-a3, [1] the NDFT kernel (a4, a5 and the
  * queueing of the spectra to score), [2] deferred comb scoring a6-a7, [3] CCL + boxes a8,

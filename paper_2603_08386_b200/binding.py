@@ -23,6 +23,7 @@ N_COUNTERS = 8
 
 #: every symbol include/ddhf.h declares
 EXPORTS = ["ddhf_create", "ddhf_workspace_bytes", "ddhf_window", "ddhf_window_host",
+           "ddhf_host_submit", "ddhf_host_wait",
            "ddhf_stage_ms", "ddhf_launches_per_window", "ddhf_fma_peak_probe", "ddhf_destroy",
            "ddhf_last_error", "ddhf_version"]
 
@@ -80,6 +81,11 @@ def lib() -> C.CDLL:
         L.ddhf_window_host.restype = C.c_int
         L.ddhf_window_host.argtypes = [vp, vp, C.c_int64, C.c_int64, C.c_int64,
                                        C.POINTER(DdhfHostOutputs), vp]
+        L.ddhf_host_submit.restype = C.c_int
+        L.ddhf_host_submit.argtypes = [vp, vp, C.c_int64, C.c_int64, C.c_int64,
+                                       C.POINTER(DdhfHostOutputs), vp]
+        L.ddhf_host_wait.restype = C.c_int
+        L.ddhf_host_wait.argtypes = [vp]
         L.ddhf_stage_ms.restype = C.c_int
         L.ddhf_stage_ms.argtypes = [vp, C.POINTER(C.c_float)]
         L.ddhf_launches_per_window.restype = C.c_int
@@ -143,6 +149,19 @@ def ddhf_window(h, d_events_ptr: int, n: int, t0_us: int, window_us: int, d_work
 def ddhf_window_host(h, h_events_ptr: int, n: int, t0_us: int, window_us: int,
                      out: DdhfHostOutputs, stream_ptr: int = 0) -> None:
     rc = lib().ddhf_window_host(h, h_events_ptr, n, t0_us, window_us, C.byref(out), stream_ptr)
+    if rc != DDHF_OK:
+        raise DdhfError(rc, (lib().ddhf_last_error(h) or b"").decode())
+
+
+def ddhf_host_submit(h, h_events_ptr: int, n: int, t0_us: int, window_us: int,
+                     out: DdhfHostOutputs, stream_ptr: int = 0) -> None:
+    rc = lib().ddhf_host_submit(h, h_events_ptr, n, t0_us, window_us, C.byref(out), stream_ptr)
+    if rc != DDHF_OK:
+        raise DdhfError(rc, (lib().ddhf_last_error(h) or b"").decode())
+
+
+def ddhf_host_wait(h) -> None:
+    rc = lib().ddhf_host_wait(h)
     if rc != DDHF_OK:
         raise DdhfError(rc, (lib().ddhf_last_error(h) or b"").decode())
 

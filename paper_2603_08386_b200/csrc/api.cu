@@ -37,6 +37,16 @@ struct ddhf_handle {
     void *hb_ws = nullptr;
     ddhf_outputs hb_out{};
     bool hb_ready = false;
+    // double-buffered pipeline of ddhf_host_submit / ddhf_host_wait
+    struct PipeSlot {
+        ddhf_event *events = nullptr;
+        void *ws = nullptr;
+        ddhf_outputs out{};
+        cudaEvent_t copied = nullptr, done = nullptr;
+    } pipe[2];
+    cudaStream_t copy_stream = nullptr;
+    bool pipe_ready = false;
+    long long pipe_head = 0, pipe_tail = 0;      // windows submitted / waited for
     std::string err;
 };
 
@@ -372,6 +382,79 @@ extern "C" int ddhf_window_host(ddhf_handle *h, const ddhf_event *h_events, int6
     return DDHF_OK;
 }
 
+#define PIPE_CHECK(call)                                                                       \
+    do {                                                                                       \
+        const cudaError_t e_ = (call);                                                         \
+        if (e_ != cudaSuccess)                                                                 \
+            return fail(h, DDHF_E_CUDA, std::string("ddhf_host_submit: ") + cudaGetErrorString(e_)); \
+    } while (0)
+
+extern "C" int ddhf_host_submit(ddhf_handle *h, const ddhf_event *h_events, int64_t n, int64_t t0_us,
+                                int64_t window_us, const ddhf_host_outputs *out, void *cuda_stream)
+{
+    if (!h) return DDHF_E_INVAL;
+    if (!out || (n > 0 && !h_events)) return fail(h, DDHF_E_INVAL, "ddhf_host_submit: NULL argument");
+    if (out->csr_ev || out->active_idx || out->power)
+        return fail(h, DDHF_E_INVAL, "ddhf_host_submit: csr_ev, active_idx and power are not available in the pipelined call");
+    if (n > h->cfg.max_events) return fail(h, DDHF_E_CAPACITY, "ddhf_host_submit: n > max_events");
+    if (h->pipe_head - h->pipe_tail >= 2)
+        return fail(h, DDHF_E_INVAL, "ddhf_host_submit: two windows already in flight, call ddhf_host_wait");
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const ddhf_config &c = h->cfg;
+    const size_t np = h->np;
+    if (!h->pipe_ready) {
+        PIPE_CHECK(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+        for (auto &s : h->pipe) {
+            PIPE_CHECK(cudaMalloc(&s.events, sizeof(ddhf_event) * static_cast<size_t>(c.max_events)));
+            PIPE_CHECK(cudaMalloc(&s.ws, h->ws_bytes));
+            PIPE_CHECK(cudaMalloc(&s.out.row_ptr, sizeof(int32_t) * (np + 1)));
+            PIPE_CHECK(cudaMalloc(&s.out.csr_ev, sizeof(uint32_t) * static_cast<size_t>(c.max_events)));
+            PIPE_CHECK(cudaMalloc(&s.out.active_idx, sizeof(int32_t) * static_cast<size_t>(c.max_active)));
+            PIPE_CHECK(cudaMalloc(&s.out.sf, sizeof(float) * np));
+            PIPE_CHECK(cudaMalloc(&s.out.score, sizeof(float) * np));
+            PIPE_CHECK(cudaMalloc(&s.out.f0_idx, sizeof(int32_t) * np));
+            PIPE_CHECK(cudaMalloc(&s.out.mask, np));
+            PIPE_CHECK(cudaMalloc(&s.out.labels, sizeof(int32_t) * np));
+            PIPE_CHECK(cudaMalloc(&s.out.boxes, sizeof(ddhf_box) * static_cast<size_t>(c.max_boxes)));
+            PIPE_CHECK(cudaMalloc(&s.out.counters, sizeof(int32_t) * DDHF_N_COUNTERS));
+            PIPE_CHECK(cudaEventCreateWithFlags(&s.copied, cudaEventDisableTiming));
+            PIPE_CHECK(cudaEventCreateWithFlags(&s.done, cudaEventDisableTiming));
+        }
+        h->pipe_ready = true;
+    }
+    ddhf_handle::PipeSlot &s = h->pipe[h->pipe_head & 1];
+    // the slot's previous window (two submits ago) has been waited for, so its buffers are free
+    if (n > 0) PIPE_CHECK(cudaMemcpyAsync(s.events, h_events, sizeof(ddhf_event) * static_cast<size_t>(n),
+                                          cudaMemcpyHostToDevice, h->copy_stream));
+    PIPE_CHECK(cudaEventRecord(s.copied, h->copy_stream));
+    PIPE_CHECK(cudaStreamWaitEvent(st, s.copied, 0));
+    const int rc = ddhf_window(h, s.events, n, t0_us, window_us, s.ws, &s.out, st);
+    if (rc != DDHF_OK) return rc;
+    const ddhf_outputs &d = s.out;
+    if (out->counters) PIPE_CHECK(cudaMemcpyAsync(out->counters, d.counters, sizeof(int32_t) * DDHF_N_COUNTERS, cudaMemcpyDeviceToHost, st));
+    if (out->mask) PIPE_CHECK(cudaMemcpyAsync(out->mask, d.mask, np, cudaMemcpyDeviceToHost, st));
+    if (out->boxes) PIPE_CHECK(cudaMemcpyAsync(out->boxes, d.boxes, sizeof(ddhf_box) * static_cast<size_t>(c.max_boxes), cudaMemcpyDeviceToHost, st));
+    if (out->sf) PIPE_CHECK(cudaMemcpyAsync(out->sf, d.sf, sizeof(float) * np, cudaMemcpyDeviceToHost, st));
+    if (out->score) PIPE_CHECK(cudaMemcpyAsync(out->score, d.score, sizeof(float) * np, cudaMemcpyDeviceToHost, st));
+    if (out->f0_idx) PIPE_CHECK(cudaMemcpyAsync(out->f0_idx, d.f0_idx, sizeof(int32_t) * np, cudaMemcpyDeviceToHost, st));
+    if (out->labels) PIPE_CHECK(cudaMemcpyAsync(out->labels, d.labels, sizeof(int32_t) * np, cudaMemcpyDeviceToHost, st));
+    if (out->row_ptr) PIPE_CHECK(cudaMemcpyAsync(out->row_ptr, d.row_ptr, sizeof(int32_t) * (np + 1), cudaMemcpyDeviceToHost, st));
+    PIPE_CHECK(cudaEventRecord(s.done, st));
+    ++h->pipe_head;
+    return DDHF_OK;
+}
+
+extern "C" int ddhf_host_wait(ddhf_handle *h)
+{
+    if (!h) return DDHF_E_INVAL;
+    if (h->pipe_head == h->pipe_tail) return fail(h, DDHF_E_INVAL, "ddhf_host_wait: no window in flight");
+    ddhf_handle::PipeSlot &s = h->pipe[h->pipe_tail & 1];
+    const cudaError_t e = cudaEventSynchronize(s.done);
+    ++h->pipe_tail;
+    if (e != cudaSuccess) return fail(h, DDHF_E_CUDA, std::string("ddhf_host_wait: ") + cudaGetErrorString(e));
+    return DDHF_OK;
+}
+
 extern "C" int ddhf_fma_peak_probe(float ms_target, float *tflops_out, void *cuda_stream)
 {
     if (!tflops_out) return DDHF_E_INVAL;
@@ -389,6 +472,14 @@ extern "C" int ddhf_destroy(ddhf_handle *h)
                     h->hb_out.sf, h->hb_out.score, h->hb_out.f0_idx, h->hb_out.mask,
                     h->hb_out.labels, h->hb_out.boxes, h->hb_out.counters};
     for (void *b : bufs) if (b) cudaFree(b);
+    for (auto &s : h->pipe) {
+        void *pb[] = {s.events, s.ws, s.out.row_ptr, s.out.csr_ev, s.out.active_idx, s.out.sf, s.out.score,
+                      s.out.f0_idx, s.out.mask, s.out.labels, s.out.boxes, s.out.counters};
+        for (void *b : pb) if (b) cudaFree(b);
+        if (s.copied) cudaEventDestroy(s.copied);
+        if (s.done) cudaEventDestroy(s.done);
+    }
+    if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
     delete h;
     return DDHF_OK;
 }

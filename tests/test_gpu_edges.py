@@ -210,6 +210,62 @@ def test_host_buffer_entry_point_matches_device_path():
     assert np.array_equal(host["boxes"][:n_box], ref["boxes"])
 
 
+def test_pipelined_host_submit_wait_matches_device_path():
+    """ddhf_host_submit / ddhf_host_wait: two windows in flight on two buffer sets, different
+    windows back to back; every window's outputs equal the device-buffer path; error codes."""
+    import torch
+    from paper_2603_08386_b200 import binding
+    w = wl.make(5, n_windows=4)
+    wins = [w.window_slice(k) for k in range(4)]
+    refs = [gu.run_gpu(w.params, w.events[lo:lo + n], t0, w.window_us, max_events=len(w.events))
+            for lo, n, t0 in wins]
+    cfg = binding.make_config(w.params, max_events=len(w.events))
+    h = binding.ddhf_create(cfg)
+    NP = w.width * w.height
+    ev = torch.from_numpy(np.ascontiguousarray(w.events).view(np.uint8).copy()).pin_memory()
+    st = torch.cuda.current_stream().cuda_stream
+    bufs, outs = [], []
+    for _ in range(2):
+        t = dict(mask=torch.zeros(NP, dtype=torch.uint8).pin_memory(),
+                 score=torch.zeros(NP, dtype=torch.float32).pin_memory(),
+                 labels=torch.zeros(NP, dtype=torch.int32).pin_memory(),
+                 boxes=torch.zeros(cfg.max_boxes * 6, dtype=torch.int32).pin_memory(),
+                 counters=torch.zeros(8, dtype=torch.int32).pin_memory())
+        o = binding.DdhfHostOutputs()
+        for k, v in t.items():
+            setattr(o, k, v.data_ptr())
+        bufs.append(t)
+        outs.append(o)
+    with pytest.raises(binding.DdhfError):
+        binding.ddhf_host_wait(h)                                   # nothing in flight
+
+    def check(k):
+        t, ref = bufs[k & 1], refs[k]
+        cnt = t["counters"].numpy()
+        assert int(cnt[0]) == ref["n_in"] and int(cnt[2]) == ref["n_active"] and int(cnt[3]) == ref["n_boxes"]
+        assert np.array_equal(t["mask"].numpy().reshape(ref["mask"].shape), ref["mask"])
+        assert np.array_equal(t["score"].numpy().reshape(ref["mask"].shape), ref["score"])
+        assert np.array_equal(t["labels"].numpy().reshape(ref["mask"].shape), ref["labels"])
+        nb = ref["n_boxes"]
+        assert np.array_equal(t["boxes"].numpy()[: nb * 6].view(binding.BOX_DTYPE).reshape(-1), ref["boxes"])
+
+    for k, (lo, n, t0) in enumerate(wins):
+        binding.ddhf_host_submit(h, ev.data_ptr() + 16 * lo, n, t0, w.window_us, outs[k & 1], st)
+        if k == 1:
+            with pytest.raises(binding.DdhfError):                  # a third window in flight
+                binding.ddhf_host_submit(h, ev.data_ptr(), wins[0][1], 0, w.window_us, outs[0], st)
+        if k >= 1:
+            binding.ddhf_host_wait(h)
+            check(k - 1)
+    binding.ddhf_host_wait(h)
+    check(len(wins) - 1)
+    bad = binding.DdhfHostOutputs()
+    bad.csr_ev = bufs[0]["mask"].data_ptr()
+    with pytest.raises(binding.DdhfError):
+        binding.ddhf_host_submit(h, ev.data_ptr(), wins[0][1], 0, w.window_us, bad, st)
+    binding.ddhf_destroy(h)
+
+
 def test_fma_probe_reports_plausible_peak():
     from paper_2603_08386_b200 import binding
     scalar, packed = binding.ddhf_fma_peak_probe(5.0)
