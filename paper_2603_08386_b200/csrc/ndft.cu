@@ -533,7 +533,9 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
                 acc2[g][m] = make_float2(0.f, 0.f);
             }
 
-        for (int base = 0; base < it.n; base += kEC) {
+        // an active pixel has at least one event: do-while, so the accumulators are set up once
+        int base = 0;
+        do {
             const int nc = min(kEC, it.n - base);
             // ---- per-event phase words and the offset-phasor table of this chunk ----------
             stage_wait();
@@ -617,7 +619,8 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
 #undef DDHF_CENTRES
 #undef DDHF_FMA_BLOCK
             __syncwarp();
-        }
+            base += kEC;
+        } while (base < it.n);
 
         // the next pixel's work item and first events are fetched under the epilogue
         if (claim_left <= 0) {
