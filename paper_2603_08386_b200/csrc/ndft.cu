@@ -100,7 +100,10 @@ __device__ __forceinline__ int pad(int j) { return j + (j >> 5); }
 // Tail warps claim kTailBatch items per atomic (short rows cost about a thousand cycles each, so a
 // global atomic per pixel is a visible stall); item i of a claim made at (h, t) is valid while
 // h + t + i < n.  Returns the first index of the claim and its valid count.
-constexpr int kTailBatch = 4;
+#ifndef DDHF_TAIL_BATCH
+#define DDHF_TAIL_BATCH 4
+#endif
+constexpr int kTailBatch = DDHF_TAIL_BATCH;
 
 __device__ __forceinline__ int fetch_items(unsigned long long *cursor, bool head, int n_items, int &cnt)
 {
