@@ -160,6 +160,17 @@ def test_config3_full_size_sampled(oracle):
 
 
 @pytest.mark.slow
+def test_config3_score_all_overflows_the_scoring_queue(oracle):
+    """DDHF_FLAG_SCORE_ALL on config 3: ~100 k pixels to score against a queue of 32 Ki rows, so
+    most pixels take the in-place path inside the NDFT kernel; sampled against the oracle."""
+    w = wl.make(3)
+    gpu, wp, wsf, ws = _sampled_compare(oracle, w, w.params, w.events, 0, 300, score_all=True, seed=2)
+    assert gpu["n_scored"] == gpu["n_active"] > 32768
+    print(f"cfg3 score_all: active {gpu['n_active']}, scored {gpu['n_scored']}, "
+          f"power {wp:.2e}, sf {wsf:.2e}, score {ws:.2e}")
+
+
+@pytest.mark.slow
 def test_config4_full_size_sampled(oracle):
     """BASELINE.json's 1280x720 / 10 M event window in the launch configuration bench.py times."""
     w = wl.make(4)
