@@ -223,6 +223,56 @@ int32_t orc_ccl_boxes(const uint8_t *mask, int32_t width, int32_t height, int32_
 }
 
 /* ---------------------------------------------------------------------------------- */
+/* Box merge, eq. 12 (L166-176): merged if dist(c1, c2) < alpha * max(w1, h1, w2, h2).   */
+/* Transitive closure by repeated relabelling (plain and slow), R27-R29.                 */
+/* ---------------------------------------------------------------------------------- */
+int32_t orc_merge_boxes(const orc_box *boxes, int32_t n, double alpha, orc_box *out)
+{
+    if (n <= 0) return 0;
+    int32_t *grp = (int32_t *)malloc(sizeof(int32_t) * (size_t)n);
+    for (int32_t i = 0; i < n; ++i) grp[i] = i;
+    int changed = 1;
+    while (changed) {                                   /* propagate the smallest index */
+        changed = 0;
+        for (int32_t i = 0; i < n; ++i)
+            for (int32_t j = 0; j < n; ++j) {
+                if (i == j || grp[i] == grp[j]) continue;
+                const double cxi = 0.5 * (boxes[i].x0 + boxes[i].x1), cyi = 0.5 * (boxes[i].y0 + boxes[i].y1);
+                const double cxj = 0.5 * (boxes[j].x0 + boxes[j].x1), cyj = 0.5 * (boxes[j].y0 + boxes[j].y1);
+                const double dist = sqrt((cxi - cxj) * (cxi - cxj) + (cyi - cyj) * (cyi - cyj));
+                double m = boxes[i].x1 - boxes[i].x0 + 1;
+                if (boxes[i].y1 - boxes[i].y0 + 1 > m) m = boxes[i].y1 - boxes[i].y0 + 1;
+                if (boxes[j].x1 - boxes[j].x0 + 1 > m) m = boxes[j].x1 - boxes[j].x0 + 1;
+                if (boxes[j].y1 - boxes[j].y0 + 1 > m) m = boxes[j].y1 - boxes[j].y0 + 1;
+                if (dist < alpha * m) {                 /* eq. 12 */
+                    const int32_t g = grp[i] < grp[j] ? grp[i] : grp[j];
+                    grp[i] = g;
+                    grp[j] = g;
+                    changed = 1;
+                }
+            }
+    }
+    int32_t n_out = 0;
+    for (int32_t g = 0; g < n; ++g) {                   /* groups in ascending smallest member */
+        int first = 1;
+        orc_box b = boxes[g];
+        for (int32_t i = 0; i < n; ++i) {
+            if (grp[i] != g) continue;
+            if (first) { b = boxes[i]; first = 0; continue; }
+            if (boxes[i].x0 < b.x0) b.x0 = boxes[i].x0;
+            if (boxes[i].y0 < b.y0) b.y0 = boxes[i].y0;
+            if (boxes[i].x1 > b.x1) b.x1 = boxes[i].x1;
+            if (boxes[i].y1 > b.y1) b.y1 = boxes[i].y1;
+            b.n_pix += boxes[i].n_pix;
+            if (boxes[i].label < b.label) b.label = boxes[i].label;
+        }
+        if (!first) out[n_out++] = b;
+    }
+    free(grp);
+    return n_out;
+}
+
+/* ---------------------------------------------------------------------------------- */
 /* Whole window, L137-139 + L164: bucket -> per active pixel NDFT power -> SF -> comb   */
 /* -> mask -> CCL/boxes.                                                               */
 /* ---------------------------------------------------------------------------------- */

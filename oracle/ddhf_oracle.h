@@ -22,6 +22,8 @@
  *                   M_valid-prefix, h_min, overlapping-window and even-count cases
  *   bucket          numpy stable argsort / bincount / cumsum
  *   ccl_boxes       scipy.ndimage.label with the 3x3 structure + find_objects
+ *   merge_boxes     hand-placed boxes (far / near / chain), scipy.sparse.csgraph.connected_components
+ *                   on an adjacency built independently in numpy
  * No function here is "parity unpinned".
  */
 #ifndef DDHF_ORACLE_H
@@ -90,6 +92,14 @@ double orc_comb_score(const double *power, const orc_config *cfg, int32_t *f0_id
  * number of boxes written (at most max_boxes; *n_total = number that passed the filter). */
 int32_t orc_ccl_boxes(const uint8_t *mask, int32_t width, int32_t height, int32_t a_min,
                       int32_t *labels, orc_box *boxes, int32_t max_boxes, int32_t *n_total);
+
+/* Box merge, eq. 12 (L166): two boxes are merged if dist(c1, c2) < alpha max(w1, h1, w2, h2).
+ * Readings R27-R29: c = centre of the bounding box, w = x1 - x0 + 1, h = y1 - y0 + 1; the rule is
+ * evaluated on the boxes that enter the step and merging is transitive (connected components
+ * of the "close" relation); a merged box is the bounding box of its members, n_pix their sum,
+ * label their smallest label; output ascending by label.  out has room for n boxes.  Returns
+ * the number of merged boxes. */
+int32_t orc_merge_boxes(const orc_box *boxes, int32_t n, double alpha, orc_box *out);
 
 /* Whole window: a0-a8.  All output pointers are host memory owned by the caller; power
  * (n_active x n_freq doubles, row r <-> active_idx[r]) and labels may be NULL.

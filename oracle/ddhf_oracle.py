@@ -52,6 +52,8 @@ def lib():
         L.orc_spectral_flatness.argtypes = [vp, C.c_int32, C.c_int32, C.c_double]
         L.orc_comb_score.restype = C.c_double
         L.orc_comb_score.argtypes = [vp, C.POINTER(OrcConfig), C.POINTER(C.c_int32), vp, vp, vp]
+        L.orc_merge_boxes.restype = C.c_int32
+        L.orc_merge_boxes.argtypes = [vp, C.c_int32, C.c_double, vp]
         L.orc_ccl_boxes.restype = C.c_int32
         L.orc_ccl_boxes.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, vp, vp, C.c_int32,
                                     C.POINTER(C.c_int32)]
@@ -122,6 +124,14 @@ def ccl_boxes(mask: np.ndarray, a_min: int, max_boxes: int = 1 << 20):
     tot = C.c_int32(0)
     nb = lib().orc_ccl_boxes(_p(m), w, h, a_min, _p(labels), _p(boxes), max_boxes, C.byref(tot))
     return labels, boxes[:nb].copy(), int(tot.value)
+
+
+def merge_boxes(boxes: np.ndarray, alpha: float) -> np.ndarray:
+    """Eq. 12 box merge (transitive); boxes: ORC_BOX array sorted by label."""
+    b = np.ascontiguousarray(boxes, dtype=ORC_BOX)
+    out = np.zeros(max(len(b), 1), dtype=ORC_BOX)
+    n = lib().orc_merge_boxes(_p(b), len(b), float(alpha), _p(out))
+    return out[:n]
 
 
 def window(params: dict, events: np.ndarray, t0_us: int, window_us: int, *,

@@ -146,3 +146,60 @@ def test_config1_ground_truth(oracle):
     assert len(out["boxes"]) == 1
     b = out["boxes"][0]
     assert 38 <= b["x0"] <= 42 and 45 <= b["x1"] <= 49 and 22 <= b["y0"] <= 26 and 29 <= b["y1"] <= 33
+
+
+# ---- box merge (eq. 12) --------------------------------------------------------------------
+def _boxes(rows):
+    import ddhf_oracle
+    b = np.zeros(len(rows), dtype=ddhf_oracle.ORC_BOX)
+    for i, (x0, y0, x1, y1) in enumerate(rows):
+        b[i] = (x0, y0, x1, y1, (x1 - x0 + 1) * (y1 - y0 + 1), y0 * 10000 + x0)
+    return b
+
+
+def test_merge_far_near_and_chain(oracle):
+    # two 10x10 boxes 100 px apart: dist 100 >= alpha*10 for alpha 5 -> separate; alpha 11 -> merged
+    b = _boxes([(0, 0, 9, 9), (100, 0, 109, 9)])
+    assert len(oracle.merge_boxes(b, 5.0)) == 2
+    m = oracle.merge_boxes(b, 11.0)
+    assert len(m) == 1 and (m[0]["x0"], m[0]["y0"], m[0]["x1"], m[0]["y1"]) == (0, 0, 109, 9)
+    assert m[0]["n_pix"] == 200 and m[0]["label"] == b[0]["label"]
+    # exactly on the threshold is NOT merged (strict <): dist 100, alpha*max = 10*10
+    assert len(oracle.merge_boxes(b, 10.0)) == 2
+    # chain A~B, B~C but A !~ C: transitive -> one box (R28)
+    c = _boxes([(0, 0, 9, 9), (60, 0, 69, 9), (120, 0, 129, 9)])
+    assert len(oracle.merge_boxes(c, 6.5)) == 1 and len(oracle.merge_boxes(c, 5.9)) == 3
+    # the larger box sets the scale: a 40-wide box reaches a small one that could not reach it alone
+    d = _boxes([(0, 0, 39, 3), (100, 0, 101, 1)])
+    assert len(oracle.merge_boxes(d, 2.5)) == 1            # centre distance 81 < 2.5 * 40
+    assert len(oracle.merge_boxes(_boxes([(0, 0, 1, 1), (100, 0, 101, 1)]), 2.5)) == 2
+    assert len(oracle.merge_boxes(_boxes([]), 3.0)) == 0
+
+
+def test_merge_matches_connected_components_of_the_close_relation(oracle):
+    """Independent construction: adjacency by eq. 12 in numpy, components by scipy.sparse.csgraph."""
+    from scipy.sparse import csr_matrix
+    from scipy.sparse.csgraph import connected_components
+    rng = np.random.default_rng(12)
+    for alpha in (0.8, 2.0, 4.0):
+        rows = []
+        for _ in range(60):
+            x0, y0 = int(rng.integers(0, 600)), int(rng.integers(0, 400))
+            rows.append((x0, y0, x0 + int(rng.integers(1, 30)), y0 + int(rng.integers(1, 30))))
+        rows.sort(key=lambda r: r[1] * 10000 + r[0])
+        b = _boxes(rows)
+        cx, cy = (b["x0"] + b["x1"]) / 2.0, (b["y0"] + b["y1"]) / 2.0
+        dim = np.maximum(b["x1"] - b["x0"] + 1, b["y1"] - b["y0"] + 1).astype(float)
+        dist = np.hypot(cx[:, None] - cx[None, :], cy[:, None] - cy[None, :])
+        adj = dist < alpha * np.maximum(dim[:, None], dim[None, :])
+        n_comp, lab = connected_components(csr_matrix(adj), directed=False)
+        m = oracle.merge_boxes(b, alpha)
+        assert len(m) == n_comp
+        for k in range(n_comp):
+            members = b[lab == k]
+            hit = m[m["label"] == members["label"].min()]
+            assert len(hit) == 1
+            assert hit[0]["x0"] == members["x0"].min() and hit[0]["x1"] == members["x1"].max()
+            assert hit[0]["y0"] == members["y0"].min() and hit[0]["y1"] == members["y1"].max()
+            assert hit[0]["n_pix"] == members["n_pix"].sum()
+        assert np.all(np.diff(m["label"]) > 0)
