@@ -268,7 +268,7 @@ def main():
     for _ in range(2):
         t = (torch.zeros(NP, dtype=torch.uint8).pin_memory(),
              torch.zeros(det.cfg.max_boxes * 6, dtype=torch.int32).pin_memory(),
-             torch.zeros(8, dtype=torch.int32).pin_memory())
+             torch.zeros(16, dtype=torch.int32).pin_memory())
         o = binding.DdhfHostOutputs()
         o.mask, o.boxes, o.counters = t[0].data_ptr(), t[1].data_ptr(), t[2].data_ptr()
         hbufs.append(t)
@@ -290,7 +290,7 @@ def main():
 
     e2e_terms = sum(terms_by_win[k][0] for k in e2e_wins)
     h2d = sum(16 * n for _, n, _ in e2e_wins)
-    d2h = NP + 32 + 24 * det.cfg.max_boxes
+    d2h = NP + 64 + 24 * det.cfg.max_boxes
     results = {}
     for name, fn in (("pipelined", run_pipelined), ("serial", run_serial)):
         fn(wins[:2])

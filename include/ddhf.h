@@ -17,6 +17,8 @@
  *          argmax                                                 (eq. 8-11)
  *   a7     mask = active and SF <= tau_sf and max SNR_M >= tau_comb      (L107, L131, L139)
  *   a8     8-connected components of the mask, bounding boxes, A_min filter      (L164)
+ *   a9     boxes whose centres are closer than alpha x their largest side are merged
+ *          into the final detections                                  (eq. 12)
  *
  * Conventions
  *   - Every function returns 0 (DDHF_OK) or a negative DDHF_E_* code; nothing throws
@@ -59,7 +61,8 @@ extern "C" {
 #define DDHF_CNT_OVERFLOW      5  /* bit 0: n_active > max_active, bit 1: boxes > max_boxes */
 #define DDHF_CNT_N_SCORED      6  /* active pixels on which the comb score was evaluated   */
 #define DDHF_CNT_N_COMPONENTS  7  /* connected components before the A_min filter          */
-#define DDHF_N_COUNTERS        8
+#define DDHF_CNT_N_MERGED      8  /* detections written to merged_boxes (eq. 12)           */
+#define DDHF_N_COUNTERS        16 /* 9..15 reserved, written as 0                          */
 
 /* Event tuple (x, y, p, t) of a temporal-contrast sensor (L55).  16 bytes. */
 typedef struct {
@@ -88,6 +91,8 @@ typedef struct {
     int32_t h_min;                  /* min matched harmonics, L115 / Table 2         */
     int32_t n_min;                  /* min events per active pixel, L137 / Table 2   */
     int32_t a_min;                  /* min bounding-box area in px, L164 / Table 2   */
+    float   merge_alpha;            /* alpha of eq. 12 (L166, Table 2: 19.05); <= 0
+                                       leaves merged_boxes untouched                       */
     float   tau_sf, tau_comb;       /* thresholds, L107 / L131                            */
     float   sf_eps;                 /* floor under log P and under the median (R6, R11)   */
     int32_t k_lo;                   /* first bin used by SF and the comb (R6)             */
@@ -114,6 +119,9 @@ typedef struct {
     int32_t  *labels;      /* optional [NP]  component label (min linear index), -1 off-mask */
     ddhf_box *boxes;       /* [max_boxes]  boxes that passed A_min, ascending label         */
     int32_t  *counters;    /* [DDHF_N_COUNTERS]                                             */
+    ddhf_box *merged_boxes;/* optional [max_boxes]  final detections: boxes merged by eq. 12 (L166;
+                              R27-R29: box centres, transitive, evaluated on the boxes that passed
+                              A_min and fit in boxes[]), ascending label                        */
     float    *comb_debug;  /* optional [max_active * n_f0 * 3]  per candidate (SNR_M, N, median)
                               of eq. 10 / 8 / 9 for rows whose comb was evaluated; tests only */
 } ddhf_outputs;
@@ -131,6 +139,7 @@ typedef struct {
     int32_t  *labels;
     ddhf_box *boxes;
     int32_t  *counters;
+    ddhf_box *merged_boxes;
 } ddhf_host_outputs;
 
 typedef struct ddhf_handle ddhf_handle;

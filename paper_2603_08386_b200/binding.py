@@ -18,8 +18,8 @@ LIB_PATH = os.environ.get("DDHF_LIB", os.path.join(_HERE, "libddhf.so"))
 DDHF_OK, DDHF_E_INVAL, DDHF_E_CAPACITY, DDHF_E_CUDA, DDHF_E_NOMEM = 0, -1, -2, -3, -4
 DDHF_FLAG_SCORE_ALL, DDHF_FLAG_TIMING = 1, 2
 (CNT_N_IN, CNT_N_DROPPED, CNT_N_ACTIVE, CNT_N_BOXES, CNT_N_BOXES_TOTAL, CNT_OVERFLOW,
- CNT_N_SCORED, CNT_N_COMPONENTS) = range(8)
-N_COUNTERS = 8
+ CNT_N_SCORED, CNT_N_COMPONENTS, CNT_N_MERGED) = range(9)
+N_COUNTERS = 16
 
 #: every symbol include/ddhf.h declares
 EXPORTS = ["ddhf_create", "ddhf_workspace_bytes", "ddhf_window", "ddhf_window_host",
@@ -37,7 +37,7 @@ class DdhfConfig(C.Structure):
         ("f_min_hz", C.c_double), ("df_hz", C.c_double), ("n_freq", C.c_int32),
         ("f0_min_hz", C.c_double), ("f0_step_hz", C.c_double), ("n_f0", C.c_int32),
         ("n_harm", C.c_int32), ("half_bw_bins", C.c_int32), ("h_min", C.c_int32),
-        ("n_min", C.c_int32), ("a_min", C.c_int32),
+        ("n_min", C.c_int32), ("a_min", C.c_int32), ("merge_alpha", C.c_float),
         ("tau_sf", C.c_float), ("tau_comb", C.c_float), ("sf_eps", C.c_float),
         ("k_lo", C.c_int32),
         ("max_events", C.c_int64), ("max_active", C.c_int32), ("max_boxes", C.c_int32),
@@ -49,13 +49,13 @@ class DdhfConfig(C.Structure):
 class DdhfOutputs(C.Structure):
     _fields_ = [(n, C.c_void_p) for n in
                 ("row_ptr", "csr_ev", "active_idx", "power", "sf", "score", "f0_idx", "mask",
-                 "labels", "boxes", "counters", "comb_debug")]
+                 "labels", "boxes", "counters", "merged_boxes", "comb_debug")]
 
 
 class DdhfHostOutputs(C.Structure):
     _fields_ = [(n, C.c_void_p) for n in
                 ("row_ptr", "csr_ev", "active_idx", "power", "sf", "score", "f0_idx", "mask",
-                 "labels", "boxes", "counters")]
+                 "labels", "boxes", "counters", "merged_boxes")]
 
 
 _lib = None
@@ -115,6 +115,7 @@ def make_config(params: dict[str, Any], *, max_events: int, max_active: int | No
                  "n_f0", "n_harm", "half_bw_bins", "h_min", "n_min", "a_min", "tau_sf", "tau_comb",
                  "sf_eps", "k_lo"):
         setattr(c, name, params[name])
+    c.merge_alpha = float(params.get("merge_alpha", 0.0))
     c.max_events = int(max_events)
     c.max_active = int(max_active if max_active is not None else params["width"] * params["height"])
     c.max_boxes = int(max_boxes)
@@ -231,10 +232,11 @@ class Detector:
         self.labels = z(self.np_, torch.int32) if want_labels else None
         self.boxes = z(c.max_boxes * 6, torch.int32)
         self.counters = z(N_COUNTERS, torch.int32)
+        self.merged_boxes = z(c.max_boxes * 6, torch.int32) if c.merge_alpha > 0 else None
         self.comb_debug = z(c.max_active * c.n_f0 * 3, torch.float32) if want_debug else None
         o = DdhfOutputs()
         for name in ("row_ptr", "csr_ev", "active_idx", "power", "sf", "score", "f0_idx", "mask",
-                     "labels", "boxes", "counters", "comb_debug"):
+                     "labels", "boxes", "counters", "merged_boxes", "comb_debug"):
             t = getattr(self, name)
             setattr(o, name, None if t is None else t.data_ptr())
         self.out = o
@@ -278,6 +280,9 @@ class Detector:
             mask=self.mask.cpu().numpy().reshape(H, W),
             boxes=self.boxes[: n_box * 6].cpu().numpy().view(BOX_DTYPE).reshape(-1),
         )
+        if self.merged_boxes is not None:
+            n_m = int(cnt[CNT_N_MERGED])
+            res["merged_boxes"] = self.merged_boxes[: n_m * 6].cpu().numpy().view(BOX_DTYPE).reshape(-1)
         if self.labels is not None:
             res["labels"] = self.labels.cpu().numpy().reshape(H, W)
         if self.power is not None:

@@ -93,6 +93,8 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
         return fail(nullptr, DDHF_E_INVAL, "ddhf_create: k_lo / sf_eps out of range");
     if (c.max_events < 1 || c.max_events >= (1ll << 31) || c.max_active < 1 || c.max_boxes < 1)
         return fail(nullptr, DDHF_E_INVAL, "ddhf_create: capacities out of range");
+    if (c.merge_alpha > 0.f && c.max_boxes > 8192)
+        return fail(nullptr, DDHF_E_INVAL, "ddhf_create: box merge (merge_alpha > 0) supports max_boxes <= 8192");
 
     ddhf_handle *h = new (std::nothrow) ddhf_handle();
     if (!h) return fail(nullptr, DDHF_E_NOMEM, "ddhf_create: out of host memory");
@@ -156,7 +158,7 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
         delete h;
         return fail(nullptr, DDHF_E_CUDA, msg);
     }
-    if (ingest_configure() != cudaSuccess) {
+    if (ingest_configure() != cudaSuccess || (c.merge_alpha > 0.f && ccl_configure(c.max_boxes) != cudaSuccess)) {
         const std::string msg = std::string("ddhf_create: ") + cudaGetErrorString(cudaGetLastError());
         cudaFree(h->d_cand);
         delete h;
@@ -291,6 +293,8 @@ extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n
     cp.rec = reinterpret_cast<int32_t *>(ws + h->off_rec);
     cp.tile_sum = reinterpret_cast<int32_t *>(ws + h->off_ctiles);
     cp.boxes = out->boxes; cp.counters = out->counters;
+    cp.merged = (c.merge_alpha > 0.f) ? out->merged_boxes : nullptr;
+    cp.merge_alpha = c.merge_alpha;
 
     int launches = 0;
     if (timing) cudaEventRecord(h->ev[0], st);
@@ -346,6 +350,7 @@ extern "C" int ddhf_window_host(ddhf_handle *h, const ddhf_event *h_events, int6
         HB_CHECK(cudaMalloc(&h->hb_out.mask, np));
         HB_CHECK(cudaMalloc(&h->hb_out.labels, sizeof(int32_t) * np));
         HB_CHECK(cudaMalloc(&h->hb_out.boxes, sizeof(ddhf_box) * static_cast<size_t>(c.max_boxes)));
+        HB_CHECK(cudaMalloc(&h->hb_out.merged_boxes, sizeof(ddhf_box) * static_cast<size_t>(c.max_boxes)));
         HB_CHECK(cudaMalloc(&h->hb_out.counters, sizeof(int32_t) * DDHF_N_COUNTERS));
         h->hb_out.power = nullptr;
         h->hb_out.comb_debug = nullptr;
@@ -378,6 +383,8 @@ extern "C" int ddhf_window_host(ddhf_handle *h, const ddhf_event *h_events, int6
     if (out->active_idx && n_act) HB_CHECK(cudaMemcpyAsync(out->active_idx, dev.active_idx, sizeof(int32_t) * n_act, cudaMemcpyDeviceToHost, st));
     if (out->power && n_act) HB_CHECK(cudaMemcpyAsync(out->power, dev.power, sizeof(float) * n_act * c.n_freq, cudaMemcpyDeviceToHost, st));
     if (out->boxes && n_box) HB_CHECK(cudaMemcpyAsync(out->boxes, dev.boxes, sizeof(ddhf_box) * n_box, cudaMemcpyDeviceToHost, st));
+    const size_t n_mrg = static_cast<size_t>(cnt[DDHF_CNT_N_MERGED]);
+    if (out->merged_boxes && n_mrg) HB_CHECK(cudaMemcpyAsync(out->merged_boxes, dev.merged_boxes, sizeof(ddhf_box) * n_mrg, cudaMemcpyDeviceToHost, st));
     HB_CHECK(cudaStreamSynchronize(st));
     return DDHF_OK;
 }
@@ -416,6 +423,7 @@ extern "C" int ddhf_host_submit(ddhf_handle *h, const ddhf_event *h_events, int6
             PIPE_CHECK(cudaMalloc(&s.out.mask, np));
             PIPE_CHECK(cudaMalloc(&s.out.labels, sizeof(int32_t) * np));
             PIPE_CHECK(cudaMalloc(&s.out.boxes, sizeof(ddhf_box) * static_cast<size_t>(c.max_boxes)));
+            PIPE_CHECK(cudaMalloc(&s.out.merged_boxes, sizeof(ddhf_box) * static_cast<size_t>(c.max_boxes)));
             PIPE_CHECK(cudaMalloc(&s.out.counters, sizeof(int32_t) * DDHF_N_COUNTERS));
             PIPE_CHECK(cudaEventCreateWithFlags(&s.copied, cudaEventDisableTiming));
             PIPE_CHECK(cudaEventCreateWithFlags(&s.done, cudaEventDisableTiming));
@@ -434,6 +442,7 @@ extern "C" int ddhf_host_submit(ddhf_handle *h, const ddhf_event *h_events, int6
     if (out->counters) PIPE_CHECK(cudaMemcpyAsync(out->counters, d.counters, sizeof(int32_t) * DDHF_N_COUNTERS, cudaMemcpyDeviceToHost, st));
     if (out->mask) PIPE_CHECK(cudaMemcpyAsync(out->mask, d.mask, np, cudaMemcpyDeviceToHost, st));
     if (out->boxes) PIPE_CHECK(cudaMemcpyAsync(out->boxes, d.boxes, sizeof(ddhf_box) * static_cast<size_t>(c.max_boxes), cudaMemcpyDeviceToHost, st));
+    if (out->merged_boxes) PIPE_CHECK(cudaMemcpyAsync(out->merged_boxes, d.merged_boxes, sizeof(ddhf_box) * static_cast<size_t>(c.max_boxes), cudaMemcpyDeviceToHost, st));
     if (out->sf) PIPE_CHECK(cudaMemcpyAsync(out->sf, d.sf, sizeof(float) * np, cudaMemcpyDeviceToHost, st));
     if (out->score) PIPE_CHECK(cudaMemcpyAsync(out->score, d.score, sizeof(float) * np, cudaMemcpyDeviceToHost, st));
     if (out->f0_idx) PIPE_CHECK(cudaMemcpyAsync(out->f0_idx, d.f0_idx, sizeof(int32_t) * np, cudaMemcpyDeviceToHost, st));
@@ -470,11 +479,11 @@ extern "C" int ddhf_destroy(ddhf_handle *h)
     if (h->hb_ws) cudaFree(h->hb_ws);
     void *bufs[] = {h->hb_out.row_ptr, h->hb_out.csr_ev, h->hb_out.active_idx, h->hb_out.power,
                     h->hb_out.sf, h->hb_out.score, h->hb_out.f0_idx, h->hb_out.mask,
-                    h->hb_out.labels, h->hb_out.boxes, h->hb_out.counters};
+                    h->hb_out.labels, h->hb_out.boxes, h->hb_out.counters, h->hb_out.merged_boxes};
     for (void *b : bufs) if (b) cudaFree(b);
     for (auto &s : h->pipe) {
         void *pb[] = {s.events, s.ws, s.out.row_ptr, s.out.csr_ev, s.out.active_idx, s.out.sf, s.out.score,
-                      s.out.f0_idx, s.out.mask, s.out.labels, s.out.boxes, s.out.counters};
+                      s.out.f0_idx, s.out.mask, s.out.labels, s.out.boxes, s.out.counters, s.out.merged_boxes};
         for (void *b : pb) if (b) cudaFree(b);
         if (s.copied) cudaEventDestroy(s.copied);
         if (s.done) cudaEventDestroy(s.done);

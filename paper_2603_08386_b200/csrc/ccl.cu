@@ -15,6 +15,7 @@
 //   k_ccl_label     parent[i] = root (labels; -1 off the mask); box record of the root updated
 //   k_ccl_count     per tile of 4096 pixels: roots, and roots whose box passes A_min
 //   k_ccl_emit      ordered compaction of the passing roots into boxes[] (ascending label)
+//   k_box_merge     (optional) eq. 12: boxes with close centres merged into the final detections
 #include "ddhf_internal.cuh"
 
 namespace ddhf {
@@ -202,7 +203,98 @@ __global__ void __launch_bounds__(1024) k_ccl_emit(CclParams p, int n_tiles)
     }
 }
 
+// ---- a9: box merge, eq. 12 ---------------------------------------------------
+// "two boxes ... are merged if dist(c1, c2) < alpha max(w1, h1, w2, h2)".  Readings R27-R29: box
+// centres, the rule evaluated on the boxes that entered the step, merging transitive.  A handful of
+// boxes: one CTA, union-find over box indices in shared memory (root = smallest index = smallest
+// label, since boxes[] is ascending by label), all pairs tested in double precision with the same
+// expression as the oracle.
+constexpr int kMergeThreads = 256;
+
+__device__ __forceinline__ int mg_find(volatile int *par, int x)
+{
+    int p = par[x];
+    while (p != x) { x = p; p = par[x]; }
+    return x;
+}
+
+__global__ void __launch_bounds__(kMergeThreads) k_box_merge(CclParams p)
+{
+    extern __shared__ int s_par[];                       // [n] parents, then [n][5] merged records
+    __shared__ int s_out;
+    const int n = min(p.counters[DDHF_CNT_N_BOXES], p.max_boxes);
+    int *s_rec = s_par + n;
+    for (int i = threadIdx.x; i < n; i += kMergeThreads) s_par[i] = i;
+    if (threadIdx.x == 0) s_out = 0;
+    __syncthreads();
+    const double alpha = static_cast<double>(p.merge_alpha);
+    const long long n_pairs = static_cast<long long>(n) * (n - 1) / 2;
+    for (long long q = threadIdx.x; q < n_pairs; q += kMergeThreads) {
+        // pair (i, j), i < j, from the linear index q = j (j - 1) / 2 + i
+        int j = static_cast<int>((1.0 + sqrt(1.0 + 8.0 * static_cast<double>(q))) * 0.5);
+        while (static_cast<long long>(j) * (j - 1) / 2 > q) --j;
+        while (static_cast<long long>(j + 1) * j / 2 <= q) ++j;
+        const int i = static_cast<int>(q - static_cast<long long>(j) * (j - 1) / 2);
+        const ddhf_box a = p.boxes[i], b = p.boxes[j];
+        const double cxa = 0.5 * (a.x0 + a.x1), cya = 0.5 * (a.y0 + a.y1);
+        const double cxb = 0.5 * (b.x0 + b.x1), cyb = 0.5 * (b.y0 + b.y1);
+        const double dist = sqrt((cxa - cxb) * (cxa - cxb) + (cya - cyb) * (cya - cyb));
+        double m = a.x1 - a.x0 + 1;
+        if (a.y1 - a.y0 + 1 > m) m = a.y1 - a.y0 + 1;
+        if (b.x1 - b.x0 + 1 > m) m = b.x1 - b.x0 + 1;
+        if (b.y1 - b.y0 + 1 > m) m = b.y1 - b.y0 + 1;
+        if (dist < alpha * m) {
+            int x = i, y = j;
+            while (true) {                               // unite: larger root under the smaller
+                x = mg_find(s_par, x);
+                y = mg_find(s_par, y);
+                if (x == y) break;
+                if (x < y) { const int t = x; x = y; y = t; }
+                const int old = atomicMin(&s_par[x], y);
+                if (old == x) break;
+                x = old;
+            }
+        }
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < n; i += kMergeThreads) {
+        int *c = s_rec + 5 * i;
+        c[0] = 0x7fffffff; c[1] = 0x7fffffff; c[2] = -1; c[3] = -1; c[4] = 0;
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < n; i += kMergeThreads) {
+        const int r = mg_find(s_par, i);
+        const ddhf_box b = p.boxes[i];
+        int *c = s_rec + 5 * r;
+        atomicMin(c + 0, b.x0);
+        atomicMin(c + 1, b.y0);
+        atomicMax(c + 2, b.x1);
+        atomicMax(c + 3, b.y1);
+        atomicAdd(c + 4, b.n_pix);
+    }
+    __syncthreads();
+    // ordered emit: roots in ascending index (= ascending label); one thread walks them (n is small)
+    if (threadIdx.x == 0) {
+        int k = 0;
+        for (int i = 0; i < n; ++i) {
+            if (s_par[i] != i) continue;
+            const int *c = s_rec + 5 * i;
+            ddhf_box b;
+            b.x0 = c[0]; b.y0 = c[1]; b.x1 = c[2]; b.y1 = c[3]; b.n_pix = c[4];
+            b.label = p.boxes[i].label;
+            p.merged[k++] = b;
+        }
+        p.counters[DDHF_CNT_N_MERGED] = k;
+    }
+}
+
 }  // namespace
+
+cudaError_t ccl_configure(int max_boxes)
+{
+    return cudaFuncSetAttribute(k_box_merge, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                static_cast<int>(static_cast<size_t>(max_boxes) * 6 * sizeof(int)));
+}
 
 int launch_ccl(const CclParams &p, cudaStream_t st)
 {
@@ -213,6 +305,9 @@ int launch_ccl(const CclParams &p, cudaStream_t st)
     k_ccl_label<<<g256, 256, 0, st>>>(p); ++launches;
     k_ccl_count<<<n_tiles, 1024, 0, st>>>(p); ++launches;
     k_ccl_emit<<<n_tiles, 1024, 0, st>>>(p, n_tiles); ++launches;
+    if (p.merged != nullptr) {
+        k_box_merge<<<1, kMergeThreads, static_cast<size_t>(p.max_boxes) * 6 * sizeof(int), st>>>(p); ++launches;
+    }
     return launches;
 }
 

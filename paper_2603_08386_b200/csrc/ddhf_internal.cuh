@@ -110,6 +110,8 @@ struct CclParams {
     int32_t *tile_sum;           // [<= 1024] boxes that pass A_min per tile of 4096 pixels
     ddhf_box *boxes;
     int32_t *counters;
+    ddhf_box *merged;            // optional: eq. 12 detections
+    float merge_alpha;
 };
 
 // kernel-set entry points (host functions that enqueue on `st`); each returns the number
@@ -121,6 +123,7 @@ int ingest_chunk_tiles();                    // tiles per scan chunk
 int launch_ndft(const NdftParams &p, int n_freq, int sm_count, cudaStream_t st, cudaEvent_t between);
                                              // `between` (optional) is recorded after the NDFT kernel, before the scoring kernel
 int launch_ccl(const CclParams &p, cudaStream_t st);
+cudaError_t ccl_configure(int max_boxes);    // shared memory of the box-merge kernel
 int ndft_bins_per_lane(int n_freq);          // 8, 16, 32 or 64
 int ndft_tn(int n_freq);                     // offset pairs per centre for that kernel
 size_t ndft_smem_bytes(int n_freq);

@@ -73,7 +73,7 @@ def preset(cfg: int) -> dict[str, Any]:
     bound (L234).  Table 2's own finals are in ``paper_table2()``.
     """
     common = dict(h_min=4, n_min=6, a_min=9, tau_sf=0.5, tau_comb=6.0, sf_eps=1e-12, k_lo=1,
-                  f_min_hz=0.0)
+                  f_min_hz=0.0, merge_alpha=19.05)          # alpha of eq. 12: Table 2 (L235)
     if cfg == 1:
         p = dict(width=64, height=64, window_us=20_000, df_hz=10.0, n_freq=201,
                  f0_min_hz=100.0, f0_step_hz=10.0, n_f0=31, n_harm=5, half_bw_bins=5)

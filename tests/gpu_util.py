@@ -28,6 +28,7 @@ def run_gpu(params, events, t0, window_us, *, score_all=False, want_power=True, 
     if timing:
         res["stage_ms"] = det.stage_ms()
     res["launches"] = binding.ddhf_launches_per_window(det.h)
+    res["merge_alpha"] = float(params.get("merge_alpha", 0.0))
     det.close()
     return res
 
@@ -103,6 +104,19 @@ def check_maps(gpu, orc, params, *, score_all, oracle_mod=None, orc_power=None):
     return edge
 
 
+def check_merged_boxes(gpu, oracle_mod, alpha):
+    """Eq. 12 detections vs the oracle's merge of the GPU's own boxes (exact: same expression in
+    double precision on both sides)."""
+    if "merged_boxes" not in gpu:
+        return
+    import numpy as _np
+    want = oracle_mod.merge_boxes(gpu["boxes"], float(_np.float32(alpha)))
+    got = gpu["merged_boxes"]
+    assert len(got) == len(want), (len(got), len(want))
+    for k in ("x0", "y0", "x1", "y1", "n_pix", "label"):
+        assert _np.array_equal(got[k], want[k]), f"merged_boxes.{k} differ"
+
+
 def check_boxes_against_oracle_ccl(gpu, oracle_mod, a_min, max_boxes=4096):
     """GPU CCL/boxes vs the oracle's CCL run on the GPU's own mask (exact)."""
     labels, boxes, total = oracle_mod.ccl_boxes(gpu["mask"], a_min, max_boxes=max_boxes)
@@ -111,3 +125,5 @@ def check_boxes_against_oracle_ccl(gpu, oracle_mod, a_min, max_boxes=4096):
     assert gpu["n_boxes_total"] == total and gpu["n_boxes"] == len(boxes)
     for k in ("x0", "y0", "x1", "y1", "n_pix", "label"):
         assert np.array_equal(gpu["boxes"][k], boxes[k]), f"boxes.{k} differ"
+    if gpu.get("merge_alpha", 0) > 0:
+        check_merged_boxes(gpu, oracle_mod, gpu["merge_alpha"])

@@ -67,7 +67,7 @@ int main(void) {
 def test_header_compiles_as_c_and_cpp(tmp_path):
     for comp, ext in (("gcc", "c"), ("g++", "cpp")):
         f = tmp_path / f"t.{ext}"
-        f.write_text('#include "ddhf.h"\nint main(void) { return DDHF_N_COUNTERS == 8 ? 0 : 1; }\n')
+        f.write_text('#include "ddhf.h"\nint main(void) { return DDHF_N_COUNTERS == 16 ? 0 : 1; }\n')
         subprocess.check_call([comp, "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), str(f),
                                "-o", str(tmp_path / f"t_{ext}")])
 

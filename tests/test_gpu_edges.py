@@ -188,7 +188,7 @@ def test_host_buffer_entry_point_matches_device_path():
         active_idx=np.zeros(NP, np.int32), power=np.zeros((NP, cfg.n_freq), np.float32),
         sf=np.zeros(NP, np.float32), score=np.zeros(NP, np.float32), f0_idx=np.zeros(NP, np.int32),
         mask=np.zeros(NP, np.uint8), labels=np.zeros(NP, np.int32),
-        boxes=np.zeros(cfg.max_boxes, binding.BOX_DTYPE), counters=np.zeros(8, np.int32))
+        boxes=np.zeros(cfg.max_boxes, binding.BOX_DTYPE), counters=np.zeros(16, np.int32))
     out = binding.DdhfHostOutputs()
     for k, v in host.items():
         setattr(out, k, v.ctypes.data)
@@ -230,7 +230,7 @@ def test_pipelined_host_submit_wait_matches_device_path():
                  score=torch.zeros(NP, dtype=torch.float32).pin_memory(),
                  labels=torch.zeros(NP, dtype=torch.int32).pin_memory(),
                  boxes=torch.zeros(cfg.max_boxes * 6, dtype=torch.int32).pin_memory(),
-                 counters=torch.zeros(8, dtype=torch.int32).pin_memory())
+                 counters=torch.zeros(16, dtype=torch.int32).pin_memory())
         o = binding.DdhfHostOutputs()
         for k, v in t.items():
             setattr(o, k, v.data_ptr())
@@ -271,3 +271,24 @@ def test_fma_probe_reports_plausible_peak():
     scalar, packed = binding.ddhf_fma_peak_probe(5.0)
     print(f"FMA probe: scalar {scalar:.1f} TFLOP/s, packed {packed:.1f} TFLOP/s")
     assert 20.0 < max(scalar, packed) < 90.0
+
+
+@pytest.mark.parametrize("alpha", [0.6, 1.5, 19.05])
+def test_box_merge_many_boxes(oracle, alpha):
+    """Eq. 12 on a few hundred boxes: a lenient threshold setting turns every active noise pixel
+    cluster into a box; merged detections must equal the oracle's merge of the same boxes."""
+    w = wl.make(2)
+    prm = dict(w.params, n_min=2, tau_sf=0.99, tau_comb=0.5, a_min=1, merge_alpha=alpha)
+    gpu = gu.run_gpu(prm, w.events, 0, w.window_us)
+    assert gpu["n_boxes"] > 100
+    gu.check_merged_boxes(gpu, oracle, alpha)
+    assert 1 <= len(gpu["merged_boxes"]) <= gpu["n_boxes"]
+    if alpha > 10:
+        assert len(gpu["merged_boxes"]) < gpu["n_boxes"]
+
+
+def test_box_merge_disabled_leaves_output_alone(oracle):
+    w = wl.make(1)
+    prm = dict(w.params, merge_alpha=0.0)
+    gpu = gu.run_gpu(prm, w.events, 0, w.window_us)
+    assert "merged_boxes" not in gpu and int(gpu["counters"][8]) == 0
