@@ -99,6 +99,8 @@ def load_workload(name: str):
         return workloads.make(5, n_windows=100)
     if name == "cfg3":
         return workloads.make(3)
+    if name == "paper":                       # the paper's operating point on the config-4 scene
+        return workloads.paper_native()
     if name == "cfg4q":                       # quarter-scale config 4 (for quick checks)
         return workloads.make(4, scale=0.5)
     raise SystemExit(f"unknown workload {name}")

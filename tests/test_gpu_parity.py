@@ -171,6 +171,18 @@ def test_config3_score_all_overflows_the_scoring_queue(oracle):
 
 
 @pytest.mark.slow
+def test_paper_operating_point_1280x720_sampled(oracle):
+    """33.3 ms frame, integer modes (df = 1/T), Table 2 finals on the config-4 scene: every active
+    pixel passes SF <= 0.89, so every active pixel is scored (queue overflow path included)."""
+    w = wl.paper_native()
+    gpu, wp, wsf, ws = _sampled_compare(oracle, w, w.params, w.events, 0, 300, score_all=False, seed=3)
+    gu.check_merged_boxes(gpu, oracle, w.params["merge_alpha"])
+    print(f"paper point: events {gpu['n_in']}, active {gpu['n_active']}, scored {gpu['n_scored']}, "
+          f"mask {gpu['mask'].sum()}, boxes {gpu['n_boxes']}, detections {len(gpu['merged_boxes'])}, "
+          f"power {wp:.2e}, sf {wsf:.2e}, score {ws:.2e}")
+
+
+@pytest.mark.slow
 def test_config4_full_size_sampled(oracle):
     """BASELINE.json's 1280x720 / 10 M event window in the launch configuration bench.py times."""
     w = wl.make(4)
