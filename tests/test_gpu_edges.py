@@ -99,6 +99,21 @@ def test_grid_shapes(oracle, nf, klo, fmin):
     gu.check_maps(gpu, orc, prm, score_all=True, oracle_mod=oracle, orc_power=orc["power"])
 
 
+def test_large_sensor_2048_bin_digits(oracle):
+    """2048 x 1100 pixels (21-bit pixel index): the partition runs with 2048-bin digits and the
+    1-CTA-per-SM shared-memory layout; unsorted input with a hot corner and bad events."""
+    W, H, T = 2048, 1100, 30_000
+    ev = wl.random_window(77, W, H, 300_000, T, hot_fraction=0.3, out_of_range=0.02, time_sorted=False)
+    prm = dict(SMALL, width=W, height=H, n_min=4)
+    orc = oracle.window(prm, ev, 0, T)
+    gpu = gu.run_gpu(prm, ev, 0, T, max_active=orc["n_active"] + 8)
+    gu.check_csr(gpu, orc)
+    assert gpu["n_active"] > 1000
+    assert gu.power_error(gpu["power"], orc["power"]) <= gu.POWER_TOL
+    gu.check_maps(gpu, orc, prm, score_all=False, oracle_mod=oracle, orc_power=orc["power"])
+    gu.check_boxes_against_oracle_ccl(gpu, oracle, prm["a_min"])
+
+
 def test_capacity_truncation(oracle):
     w = wl.make(1)
     prm = dict(w.params, n_min=1, a_min=1, tau_sf=2.0, tau_comb=0.0)    # every active pixel is a detection
