@@ -126,9 +126,7 @@ int launch_ccl(const CclParams &p, cudaStream_t st);
 cudaError_t ccl_configure(int max_boxes);    // shared memory of the box-merge kernel
 int ndft_bins_per_lane(int n_freq);          // 8, 16, 32 or 64
 int ndft_tn(int n_freq);                     // offset pairs per centre for that kernel
-size_t ndft_smem_bytes(int n_freq);
 int ndft_padded_bins(int n_freq);            // row length of the deferred-scoring queue
 int ndft_band_size(int n_freq, int r0, int r1);   // sort capacity needed, 0 if unsupported
-cudaError_t ndft_configure();                // opt in to large dynamic shared memory
 
 }  // namespace ddhf
