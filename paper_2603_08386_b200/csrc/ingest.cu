@@ -26,9 +26,15 @@ namespace ddhf {
 
 namespace {
 
-constexpr int kTileThreads = 512;
+#ifndef DDHF_TILE_THREADS
+#define DDHF_TILE_THREADS 512
+#endif
+constexpr int kTileThreads = DDHF_TILE_THREADS;
 constexpr int kTileWarps = kTileThreads / 32;
-constexpr int kTileEv = 16;                          // events per thread
+#ifndef DDHF_TILE_EV
+#define DDHF_TILE_EV 16
+#endif
+constexpr int kTileEv = DDHF_TILE_EV;                // events per thread
 constexpr int kTile = kTileThreads * kTileEv;        // 8192 events per tile
 constexpr int kWarpSpan = 32 * kTileEv;              // consecutive events owned by one warp
 constexpr int kChunkTiles = 8;                       // tiles per scan chunk
@@ -284,8 +290,11 @@ struct PartSmem {
     static size_t bytes(int bins) { return static_cast<size_t>(bins) * (8 + 2 * kTileWarps) + 4u * kStageWords; }
 };
 
+#ifndef DDHF_PART_BLOCKS
+#define DDHF_PART_BLOCKS (kTileThreads >= 512 ? 2 : 4)
+#endif
 template <int PASS>
-__global__ void __launch_bounds__(kTileThreads, 2) k_part(IngestParams p)
+__global__ void __launch_bounds__(kTileThreads, DDHF_PART_BLOCKS) k_part(IngestParams p)
 {
     extern __shared__ uint32_t s_raw[];
     __shared__ int s_ntile;
@@ -366,10 +375,10 @@ __global__ void __launch_bounds__(kTileThreads, 2) k_part(IngestParams p)
         __shared__ uint32_t s_ws[kTileWarps + 1];
         const int per = (bins + kTileThreads - 1) / kTileThreads;
         const int bb = threadIdx.x * per;
-        uint32_t tot[4];                                       // per <= 4 (bins <= 2048)
+        uint32_t tot[8];                                       // per <= 8 (bins <= 2048, >= 256 threads)
         uint32_t sum = 0;
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
+        for (int j = 0; j < 8; ++j) {
             tot[j] = 0;
             const int b = bb + j;
             if (j < per && b < bins) {
@@ -405,7 +414,7 @@ __global__ void __launch_bounds__(kTileThreads, 2) k_part(IngestParams p)
         __syncthreads();
         uint32_t off = inc - sum + s_ws[wid];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
+        for (int j = 0; j < 8; ++j) {
             const int b = bb + j;
             if (j < per && b < bins) {
                 s_binoff[b] = off;
