@@ -114,6 +114,31 @@ def test_large_sensor_2048_bin_digits(oracle):
     gu.check_boxes_against_oracle_ccl(gpu, oracle, prm["a_min"])
 
 
+def test_longest_window_keeps_phase_exact(oracle):
+    """window_us = 2^31 - 1 (35.8 minutes): f t reaches 1e7 cycles at 5 kHz.  The 64-bit fixed-point
+    phase constants keep 2^-32 turns, so the power error stays at the level of short windows
+    (a float32 phase would be off by whole cycles)."""
+    T = (1 << 31) - 1
+    rng = np.random.default_rng(31)
+    n_pix, per = 150, 24
+    px = rng.choice(48 * 40, size=n_pix, replace=False)
+    x = np.repeat(px % 48, per)
+    y = np.repeat(px // 48, per)
+    t = rng.integers(0, T, size=n_pix * per, dtype=np.int64)
+    pol = rng.integers(0, 2, size=n_pix * per).astype(np.int16) * 2 - 1
+    ev = np.zeros(n_pix * per, dtype=wl.EVENT_DTYPE)
+    ev["x"], ev["y"], ev["p"], ev["t"] = x, y, pol, t
+    ev = ev[np.argsort(ev["t"], kind="stable")]
+    prm = dict(wl.preset(4), width=48, height=40, n_min=6)
+    orc = oracle.window(prm, ev, 0, T)
+    gpu = gu.run_gpu(prm, ev, 0, T)
+    gu.check_csr(gpu, orc)
+    assert gpu["n_active"] == n_pix
+    err = gu.power_error(gpu["power"], orc["power"])
+    assert err <= 2e-5, err
+    gu.check_maps(gpu, orc, prm, score_all=False, oracle_mod=oracle, orc_power=orc["power"])
+
+
 def test_capacity_truncation(oracle):
     w = wl.make(1)
     prm = dict(w.params, n_min=1, a_min=1, tau_sf=2.0, tau_comb=0.0)    # every active pixel is a detection
