@@ -210,3 +210,25 @@ def test_config5_streaming_windows(oracle):
     det.close()
     lo, n, t0 = w.window_slice(1)
     _sampled_compare(oracle, w, w.params, w.events[lo:lo + n], t0, 200, score_all=False, seed=1)
+
+
+@pytest.mark.slow
+def test_config4_bench_launch_configuration(oracle):
+    """bench.py runs config 4 without the spectra output, without labels and with max_active = 1
+    (active_idx truncated).  That launch configuration must give bit-identical maps, boxes and
+    detections to the configuration test_config4_full_size_sampled checks against the oracle."""
+    from paper_2603_08386_b200 import binding
+    w = wl.make(4)
+    ref = gu.run_gpu(w.params, w.events, 0, w.window_us, want_power=True)
+    det = binding.Detector(w.params, max_events=len(w.events), timing=True, want_power=False,
+                           want_labels=False, max_active=1)
+    d_ev = det.upload(w.events)
+    det.window(d_ev, len(w.events), 0, w.window_us)
+    got = det.results()
+    det.close()
+    assert got["overflow"] & 1 and got["n_active"] == ref["n_active"]       # truncation is flagged, count is not capped
+    for k in ("row_ptr", "csr_ev", "sf", "score", "f0_idx", "mask", "boxes", "merged_boxes"):
+        same = (np.array_equal(got[k], ref[k], equal_nan=True) if got[k].dtype.kind == "f"
+                else np.array_equal(got[k], ref[k]))
+        assert same, k
+    assert got["n_scored"] == ref["n_scored"] and got["n_boxes"] == ref["n_boxes"]
