@@ -1,4 +1,5 @@
-// ndft.cu -- a4-a7: per-pixel NDFT power spectrum with the scoring fused into its epilogue.
+// ndft.cu -- a4-a7: per-pixel NDFT power spectrum and spectral flatness (k_ndft_score) and the
+// harmonic-comb score of the pixels that pass the SF filter (k_comb_deferred).
 //
 //   a4  X_j = sum_k w_k exp(-2 pi i f_j t_k),  P_j = |X_j|^2          (eq. 6)
 //   a5  SF = geometric mean / arithmetic mean of P                  (eq. 7)
@@ -21,13 +22,17 @@
 //   is no recurrence along frequency or time, hence no drift to resync.
 // * Phases are exact 32-bit fixed point "turns": hi32(G * t) with G = 2^64 f 1e-6, so a
 //   5 kHz x 0.1 s = 500-cycle phase keeps 2^-32 turn resolution before it reaches the SFU.
-// * The spectrum never goes back to HBM for scoring: P stays in registers and in the warp's
-//   shared-memory slice; the optional compact spectrum output is a streaming store.
+// * Power and spectral flatness are the kernel's epilogue, straight from the accumulators; the
+//   optional compact spectrum output is a streaming store.  A pixel that needs the comb score
+//   queues its spectrum (8 KB) for k_comb_deferred, which runs the latency-bound scoring code at
+//   an occupancy this 168-register kernel cannot offer; when the queue is full the same
+//   comb_score() runs in place, so the result does not depend on the path.
 // * The complement median of every candidate is an order statistic of the full spectrum
 //   in a narrow rank band [r0, r1] known at create time.  The band is isolated by a few
-//   counting passes over the register-resident spectrum, sorted once per pixel in registers
-//   (bitonic), and each candidate then only corrects the rank for its own excluded bins
-//   (prefix counts from warp ballots + a bitmask of excluded in-band positions).
+//   counting passes over the spectrum, sorted once per pixel in registers (bitonic), and each
+//   candidate then only corrects the rank for its own excluded bins (prefix counts from warp
+//   ballots + a bitmask of excluded in-band positions).  Window maxima of eq. 8 come from a
+//   table of forward block maxima built by warp shuffles.
 #include "ddhf_internal.cuh"
 
 namespace ddhf {
