@@ -65,7 +65,7 @@ struct NdftParams {
     // deferred comb scoring: spectra of the pixels to score are queued and scored by k_comb_deferred
     float *spill;                // [spill_cap][padded n_freq]
     SpillRec *spill_rec;         // [spill_cap]
-    int32_t *spill_count;        // rows requested (may exceed spill_cap: the excess is scored in place)
+    int32_t *spill_count;        // [0] rows requested (may exceed spill_cap: the excess is scored in place), [1] rows taken by k_comb_deferred
     int32_t spill_cap;
     ScoreParams sp;
 };
@@ -86,7 +86,7 @@ struct IngestParams {
     int32_t chunk_words;         // words of chunk1 + chunk2 (zeroed every window)
     int32_t *bin_base1, *bin_base2;   // [bins]
     int32_t *bin_tot;            // [bins] scratch of k_binscan
-    int32_t *scan_done;          // [2] CTAs of k_binscan<1>, <2> that have finished
+    int32_t *scan_done;          // [4] CTAs of k_binscan<1>, <2> that have finished; [2], [3]: scoring queue producer / consumer counts
     int32_t *active_idx;
     WorkItem *work;
     int32_t *tile_sum, *tile_act;   // [n_tiles]

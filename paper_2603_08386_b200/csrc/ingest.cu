@@ -88,7 +88,7 @@ __global__ void k_init(IngestParams p)
             p.class_cnt[threadIdx.x] = 0;
             p.class_cur[threadIdx.x] = 0;
         }
-        if (threadIdx.x == 0) { *p.work_cursor = 0ull; p.scan_done[0] = 0; p.scan_done[1] = 0; p.scan_done[2] = 0; }
+        if (threadIdx.x == 0) { *p.work_cursor = 0ull; p.scan_done[0] = 0; p.scan_done[1] = 0; p.scan_done[2] = 0; p.scan_done[3] = 0; }
     }
 }
 

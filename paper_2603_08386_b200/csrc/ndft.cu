@@ -775,8 +775,13 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 4) k_comb_deferred(NdftParam
     uint32_t *scr = wsm + L::P_WORDS;
     const ScoreParams &sp = p.sp;
     const int n_rows = min(*p.spill_count, p.spill_cap);
-    const int n_warps = gridDim.x * kScoreWarps;
-    for (int row = blockIdx.x * kScoreWarps + wid; row < n_rows; row += n_warps) {
+    // rows are handed out one at a time (their cost varies with the band search): spill_count[1]
+    // is the consumer cursor, zeroed with the producer count by the ingest stage
+    while (true) {
+        int row = 0;
+        if (lane == 0) row = atomicAdd(p.spill_count + 1, 1);
+        row = __shfl_sync(kFull, row, 0);
+        if (row >= n_rows) break;
         const SpillRec r = p.spill_rec[row];
         const float *src = p.spill + static_cast<size_t>(row) * L::NB + lane;
         float preg[NBL];
