@@ -1,0 +1,58 @@
+"""Randomised GPU parity: random sensor sizes, grids, comb parameters, event mixes (hot pixels,
+out-of-range events, unsorted input) against the oracle, every stage.  DDHF_FUZZ_SEEDS=n runs
+n seeds instead of the default dozen."""
+import os
+
+import numpy as np
+import pytest
+
+from paper_2603_08386_b200 import workloads as wl
+
+import gpu_util as gu
+
+pytestmark = pytest.mark.gpu
+
+N_SEEDS = int(os.environ.get("DDHF_FUZZ_SEEDS", "12"))
+
+
+def _case(seed):
+    rng = np.random.default_rng([2603, 8386, 777, seed])
+    W, H = int(rng.integers(8, 200)), int(rng.integers(8, 160))
+    T = int(rng.choice([5_000, 20_000, 100_000, 1_000_000]))
+    n = int(rng.integers(0, 60_000))
+    nf = int(rng.choice([8, 40, 64, 130, 256, 300, 512, 700, 1024, 1500, 2048]))
+    f_hi = float(rng.choice([500.0, 2000.0, 5000.0]))
+    fmin = float(rng.choice([0.0, 0.0, 37.5]))
+    df = (f_hi - fmin) / nf
+    klo = int(rng.integers(0, 3)) if fmin == 0 else 0
+    d = int(rng.integers(0, 4)) if nf >= 64 else 0
+    n_harm = int(rng.integers(1, 7)) if nf >= 64 else 1
+    f0_min = max(fmin + (d + klo + 2) * df, 20.0)
+    prm = dict(width=W, height=H, window_us=T, f_min_hz=fmin, df_hz=df, n_freq=nf, k_lo=klo,
+               f0_min_hz=f0_min, f0_step_hz=float(rng.choice([0.5, 2.0, 7.0])) * df,
+               n_f0=int(rng.integers(1, 100)), n_harm=n_harm, half_bw_bins=d,
+               h_min=int(rng.integers(1, n_harm + 1)), n_min=int(rng.integers(1, 8)),
+               a_min=int(rng.integers(1, 12)), tau_sf=float(rng.uniform(0.3, 0.95)),
+               tau_comb=float(rng.uniform(1.5, 8.0)), sf_eps=1e-12,
+               merge_alpha=float(rng.choice([0.0, 1.0, 19.05])))
+    ev = wl.random_window(1000 + seed, W, H, n, T, hot_fraction=float(rng.choice([0.0, 0.3, 0.8])),
+                          out_of_range=float(rng.choice([0.0, 0.05])), time_sorted=bool(rng.integers(0, 2)))
+    return prm, ev, T, bool(rng.integers(0, 2))
+
+
+@pytest.mark.parametrize("seed", range(N_SEEDS))
+def test_random_configuration(oracle, seed):
+    from paper_2603_08386_b200 import binding
+    prm, ev, T, score_all = _case(seed)
+    try:
+        gpu = gu.run_gpu(prm, ev, 0, T, score_all=score_all)
+    except binding.DdhfError as e:
+        # a configuration the library refuses at create time (comb windows too wide for the band
+        # sorter) is not a parity case; anything else is a failure
+        assert "band sorter" in str(e), str(e)
+        pytest.skip(str(e))
+    orc = oracle.window(prm, ev, 0, T, score_all=score_all)
+    gu.check_csr(gpu, orc)
+    assert gu.power_error(gpu["power"], orc["power"], gu.active_counts(orc)) <= gu.POWER_TOL
+    gu.check_maps(gpu, orc, prm, score_all=score_all, oracle_mod=oracle, orc_power=orc["power"])
+    gu.check_boxes_against_oracle_ccl(gpu, oracle, prm["a_min"])
