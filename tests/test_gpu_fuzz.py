@@ -56,3 +56,27 @@ def test_random_configuration(oracle, seed):
     assert gu.power_error(gpu["power"], orc["power"], gu.active_counts(orc)) <= gu.POWER_TOL
     gu.check_maps(gpu, orc, prm, score_all=score_all, oracle_mod=oracle, orc_power=orc["power"])
     gu.check_boxes_against_oracle_ccl(gpu, oracle, prm["a_min"])
+
+
+@pytest.mark.parametrize("seed", range(max(N_SEEDS // 2, 4)))
+def test_random_bucketing_at_scale(oracle, seed):
+    """CSR only, larger inputs: sensors up to 4 Mi pixels (digit widths from 6+6 to 11+11 bits), up to
+    3 M events, several partition tiles with a ragged tail, skewed pixels, bad events, any order."""
+    rng = np.random.default_rng([2603, 8386, 778, seed])
+    W = int(rng.choice([64, 300, 640, 1280, 2048]))
+    H = int(rng.choice([64, 200, 480, 720, 2048]))
+    n = int(rng.choice([1, 8191, 8192, 8193, 100_000, 1_000_003, 3_000_000]))
+    T = int(rng.choice([1000, 100_000, (1 << 31) - 1]))
+    ev = wl.random_window(2000 + seed, W, H, n, T, hot_fraction=float(rng.choice([0.0, 0.5, 0.95])),
+                          out_of_range=float(rng.choice([0.0, 0.1])), time_sorted=bool(rng.integers(0, 2)))
+    t0 = int(rng.choice([0, 0, -12345]))
+    ev["t"] += t0
+    prm = dict(wl.preset(1), width=W, height=H, n_min=int(rng.integers(1, 5)))
+    gpu = gu.run_gpu(prm, ev, t0, T, want_power=False, max_active=16)
+    row_ptr, csr, dropped = oracle.bucket(ev, W, H, t0, T)
+    assert gpu["n_dropped"] == dropped and gpu["n_in"] == len(csr)
+    assert np.array_equal(gpu["row_ptr"], row_ptr), "row_ptr differs"
+    assert np.array_equal(gpu["csr_ev"], csr), "csr_ev differs"
+    cnt = np.diff(row_ptr)
+    assert gpu["n_active"] == int((cnt >= prm["n_min"]).sum())
+    assert np.array_equal(gpu["active_idx"], np.flatnonzero(cnt >= prm["n_min"])[:16])
