@@ -101,8 +101,6 @@ def load_workload(name: str):
         return workloads.make(3)
     if name == "paper":                       # the paper's operating point on the config-4 scene
         return workloads.paper_native()
-    if name == "cfg4q":                       # quarter-scale config 4 (for quick checks)
-        return workloads.make(4, scale=0.5)
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -169,7 +167,6 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--score-all", action="store_true", help="comb score on every active pixel (R14)")
     ap.add_argument("--spectra", action="store_true", help="also write the compact power spectra to HBM")
-    ap.add_argument("--n-freq", type=int, default=0, help="experiment: override the number of bins (same df)")
     args = ap.parse_args()
     steps, warmup = max(args.steps, 1), max(args.warmup, 3 if args.impl == "ours" else 0)
 
@@ -208,8 +205,6 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     w = load_workload(args.workload)
-    if args.n_freq:
-        w.params = dict(w.params, n_freq=args.n_freq)
     prm = w.params
     det = binding.Detector(prm, max_events=len(w.events), score_all=args.score_all, timing=True,
                            want_power=args.spectra, want_labels=False, device=f"cuda:{local_rank}",

@@ -62,9 +62,14 @@ static size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
 
 static uint64_t freq_const(double f_hz)
 {
-    // round(2^64 * f * 1e-6): phase in turns of f at integer microsecond t is hi32(G * t)
-    const long double x = static_cast<long double>(f_hz) / 1.0e6L;
-    return static_cast<uint64_t>(llroundl(ldexpl(x, 64)));
+    // round(2^64 * f * 1e-6) mod 2^64: phase in turns of f at integer microsecond t is hi32(G * t).
+    // Only the fractional part of f * 1e-6 (cycles per microsecond) matters; it is scaled in two
+    // 32-bit halves so that no signed 64-bit conversion can overflow, whatever f is.
+    long double x = static_cast<long double>(f_hz) / 1.0e6L;
+    x -= floorl(x);
+    const long double hi = floorl(ldexpl(x, 32));
+    const long double lo = roundl(ldexpl(ldexpl(x, 32) - hi, 32));
+    return (static_cast<uint64_t>(hi) << 32) + static_cast<uint64_t>(lo);     // lo == 2^32 carries into hi
 }
 
 extern "C" const char *ddhf_version(void) { return "ddhf-b200 0.1 (sm_100a)"; }
@@ -322,6 +327,57 @@ extern "C" int ddhf_stage_ms(ddhf_handle *h, float *ms)
     return DDHF_OK;
 }
 
+// ---- device buffers owned by the handle for the host-buffer entry points -----------------------
+// One set for ddhf_window_host(), two for the pipeline of ddhf_host_submit().  A set is either
+// complete or absent: a failed allocation frees what was allocated before it.
+static void free_set(ddhf_event *&events, void *&ws, ddhf_outputs &o)
+{
+    void *bufs[] = {events, ws, o.row_ptr, o.csr_ev, o.active_idx, o.power, o.sf, o.score, o.f0_idx, o.mask,
+                    o.labels, o.boxes, o.counters, o.merged_boxes};
+    for (void *b : bufs) if (b) cudaFree(b);
+    events = nullptr;
+    ws = nullptr;
+    o = ddhf_outputs{};
+}
+
+static cudaError_t alloc_set(const ddhf_handle *h, ddhf_event *&events, void *&ws, ddhf_outputs &o)
+{
+    const ddhf_config &c = h->cfg;
+    const size_t np = h->np;
+    o = ddhf_outputs{};
+    events = nullptr;
+    ws = nullptr;
+    cudaError_t e = cudaSuccess;
+    auto get = [&e](auto &ptr, size_t bytes) {
+        if (e == cudaSuccess) e = cudaMalloc(reinterpret_cast<void **>(&ptr), bytes ? bytes : 1);
+    };
+    get(events, sizeof(ddhf_event) * static_cast<size_t>(c.max_events));
+    get(ws, h->ws_bytes);
+    get(o.row_ptr, sizeof(int32_t) * (np + 1));
+    get(o.csr_ev, sizeof(uint32_t) * static_cast<size_t>(c.max_events));
+    get(o.active_idx, sizeof(int32_t) * static_cast<size_t>(c.max_active));
+    get(o.sf, sizeof(float) * np);
+    get(o.score, sizeof(float) * np);
+    get(o.f0_idx, sizeof(int32_t) * np);
+    get(o.mask, np);
+    get(o.labels, sizeof(int32_t) * np);
+    get(o.boxes, sizeof(ddhf_box) * static_cast<size_t>(c.max_boxes));
+    get(o.merged_boxes, sizeof(ddhf_box) * static_cast<size_t>(c.max_boxes));
+    get(o.counters, sizeof(int32_t) * DDHF_N_COUNTERS);
+    if (e != cudaSuccess) free_set(events, ws, o);
+    return e;
+}
+
+static int check_host_args(ddhf_handle *h, const char *who, const ddhf_event *h_events, int64_t n,
+                           int64_t window_us, const ddhf_host_outputs *out)
+{
+    if (!out || (n > 0 && !h_events)) return fail(h, DDHF_E_INVAL, std::string(who) + ": NULL argument");
+    if (n < 0 || window_us <= 0 || window_us >= (1ll << 31))
+        return fail(h, DDHF_E_INVAL, std::string(who) + ": n or window_us out of range");
+    if (n > h->cfg.max_events) return fail(h, DDHF_E_CAPACITY, std::string(who) + ": n > max_events");
+    return DDHF_OK;
+}
+
 #define HB_CHECK(call)                                                                         \
     do {                                                                                       \
         const cudaError_t e_ = (call);                                                         \
@@ -333,27 +389,13 @@ extern "C" int ddhf_window_host(ddhf_handle *h, const ddhf_event *h_events, int6
                                 int64_t window_us, const ddhf_host_outputs *out, void *cuda_stream)
 {
     if (!h) return DDHF_E_INVAL;
-    if (!out || (n > 0 && !h_events)) return fail(h, DDHF_E_INVAL, "ddhf_window_host: NULL argument");
-    if (n > h->cfg.max_events) return fail(h, DDHF_E_CAPACITY, "ddhf_window_host: n > max_events");
+    const int arg_rc = check_host_args(h, "ddhf_window_host", h_events, n, window_us, out);     // before any copy
+    if (arg_rc != DDHF_OK) return arg_rc;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const ddhf_config &c = h->cfg;
     const size_t np = h->np;
     if (!h->hb_ready) {
-        HB_CHECK(cudaMalloc(&h->hb_events, sizeof(ddhf_event) * static_cast<size_t>(c.max_events)));
-        HB_CHECK(cudaMalloc(&h->hb_ws, h->ws_bytes));
-        HB_CHECK(cudaMalloc(&h->hb_out.row_ptr, sizeof(int32_t) * (np + 1)));
-        HB_CHECK(cudaMalloc(&h->hb_out.csr_ev, sizeof(uint32_t) * static_cast<size_t>(c.max_events)));
-        HB_CHECK(cudaMalloc(&h->hb_out.active_idx, sizeof(int32_t) * static_cast<size_t>(c.max_active)));
-        HB_CHECK(cudaMalloc(&h->hb_out.sf, sizeof(float) * np));
-        HB_CHECK(cudaMalloc(&h->hb_out.score, sizeof(float) * np));
-        HB_CHECK(cudaMalloc(&h->hb_out.f0_idx, sizeof(int32_t) * np));
-        HB_CHECK(cudaMalloc(&h->hb_out.mask, np));
-        HB_CHECK(cudaMalloc(&h->hb_out.labels, sizeof(int32_t) * np));
-        HB_CHECK(cudaMalloc(&h->hb_out.boxes, sizeof(ddhf_box) * static_cast<size_t>(c.max_boxes)));
-        HB_CHECK(cudaMalloc(&h->hb_out.merged_boxes, sizeof(ddhf_box) * static_cast<size_t>(c.max_boxes)));
-        HB_CHECK(cudaMalloc(&h->hb_out.counters, sizeof(int32_t) * DDHF_N_COUNTERS));
-        h->hb_out.power = nullptr;
-        h->hb_out.comb_debug = nullptr;
+        HB_CHECK(alloc_set(h, h->hb_events, h->hb_ws, h->hb_out));
         h->hb_ready = true;
     }
     if (out->power && !h->hb_out.power)
@@ -364,7 +406,7 @@ extern "C" int ddhf_window_host(ddhf_handle *h, const ddhf_event *h_events, int6
     if (n > 0) HB_CHECK(cudaMemcpyAsync(h->hb_events, h_events, sizeof(ddhf_event) * static_cast<size_t>(n),
                                         cudaMemcpyHostToDevice, st));
     const int rc = ddhf_window(h, h->hb_events, n, t0_us, window_us, h->hb_ws, &dev, st);
-    if (rc != DDHF_OK) return rc;
+    if (rc != DDHF_OK) { cudaStreamSynchronize(st); return rc; }
 
     int32_t cnt[DDHF_N_COUNTERS];
     HB_CHECK(cudaMemcpyAsync(cnt, dev.counters, sizeof(cnt), cudaMemcpyDeviceToHost, st));
@@ -389,66 +431,74 @@ extern "C" int ddhf_window_host(ddhf_handle *h, const ddhf_event *h_events, int6
     return DDHF_OK;
 }
 
-#define PIPE_CHECK(call)                                                                       \
-    do {                                                                                       \
-        const cudaError_t e_ = (call);                                                         \
-        if (e_ != cudaSuccess)                                                                 \
-            return fail(h, DDHF_E_CUDA, std::string("ddhf_host_submit: ") + cudaGetErrorString(e_)); \
-    } while (0)
-
 extern "C" int ddhf_host_submit(ddhf_handle *h, const ddhf_event *h_events, int64_t n, int64_t t0_us,
                                 int64_t window_us, const ddhf_host_outputs *out, void *cuda_stream)
 {
     if (!h) return DDHF_E_INVAL;
-    if (!out || (n > 0 && !h_events)) return fail(h, DDHF_E_INVAL, "ddhf_host_submit: NULL argument");
+    const int arg_rc = check_host_args(h, "ddhf_host_submit", h_events, n, window_us, out);
+    if (arg_rc != DDHF_OK) return arg_rc;
     if (out->csr_ev || out->active_idx || out->power)
         return fail(h, DDHF_E_INVAL, "ddhf_host_submit: csr_ev, active_idx and power are not available in the pipelined call");
-    if (n > h->cfg.max_events) return fail(h, DDHF_E_CAPACITY, "ddhf_host_submit: n > max_events");
     if (h->pipe_head - h->pipe_tail >= 2)
         return fail(h, DDHF_E_INVAL, "ddhf_host_submit: two windows already in flight, call ddhf_host_wait");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const ddhf_config &c = h->cfg;
     const size_t np = h->np;
+    auto cuda_fail = [h](cudaError_t e) {
+        return fail(h, DDHF_E_CUDA, std::string("ddhf_host_submit: ") + cudaGetErrorString(e));
+    };
     if (!h->pipe_ready) {
-        PIPE_CHECK(cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+        // all or nothing: a failure part-way leaves no buffer behind, so the next call starts clean
+        cudaError_t e = cudaSuccess;
+        if (!h->copy_stream) e = cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking);
         for (auto &s : h->pipe) {
-            PIPE_CHECK(cudaMalloc(&s.events, sizeof(ddhf_event) * static_cast<size_t>(c.max_events)));
-            PIPE_CHECK(cudaMalloc(&s.ws, h->ws_bytes));
-            PIPE_CHECK(cudaMalloc(&s.out.row_ptr, sizeof(int32_t) * (np + 1)));
-            PIPE_CHECK(cudaMalloc(&s.out.csr_ev, sizeof(uint32_t) * static_cast<size_t>(c.max_events)));
-            PIPE_CHECK(cudaMalloc(&s.out.active_idx, sizeof(int32_t) * static_cast<size_t>(c.max_active)));
-            PIPE_CHECK(cudaMalloc(&s.out.sf, sizeof(float) * np));
-            PIPE_CHECK(cudaMalloc(&s.out.score, sizeof(float) * np));
-            PIPE_CHECK(cudaMalloc(&s.out.f0_idx, sizeof(int32_t) * np));
-            PIPE_CHECK(cudaMalloc(&s.out.mask, np));
-            PIPE_CHECK(cudaMalloc(&s.out.labels, sizeof(int32_t) * np));
-            PIPE_CHECK(cudaMalloc(&s.out.boxes, sizeof(ddhf_box) * static_cast<size_t>(c.max_boxes)));
-            PIPE_CHECK(cudaMalloc(&s.out.merged_boxes, sizeof(ddhf_box) * static_cast<size_t>(c.max_boxes)));
-            PIPE_CHECK(cudaMalloc(&s.out.counters, sizeof(int32_t) * DDHF_N_COUNTERS));
-            PIPE_CHECK(cudaEventCreateWithFlags(&s.copied, cudaEventDisableTiming));
-            PIPE_CHECK(cudaEventCreateWithFlags(&s.done, cudaEventDisableTiming));
+            if (e == cudaSuccess) e = alloc_set(h, s.events, s.ws, s.out);
+            if (e == cudaSuccess && !s.copied) e = cudaEventCreateWithFlags(&s.copied, cudaEventDisableTiming);
+            if (e == cudaSuccess && !s.done) e = cudaEventCreateWithFlags(&s.done, cudaEventDisableTiming);
+        }
+        if (e != cudaSuccess) {
+            for (auto &s : h->pipe) free_set(s.events, s.ws, s.out);
+            return cuda_fail(e);
         }
         h->pipe_ready = true;
     }
     ddhf_handle::PipeSlot &s = h->pipe[h->pipe_head & 1];
     // the slot's previous window (two submits ago) has been waited for, so its buffers are free
-    if (n > 0) PIPE_CHECK(cudaMemcpyAsync(s.events, h_events, sizeof(ddhf_event) * static_cast<size_t>(n),
-                                          cudaMemcpyHostToDevice, h->copy_stream));
-    PIPE_CHECK(cudaEventRecord(s.copied, h->copy_stream));
-    PIPE_CHECK(cudaStreamWaitEvent(st, s.copied, 0));
+    cudaError_t e = cudaSuccess;
+    if (n > 0) e = cudaMemcpyAsync(s.events, h_events, sizeof(ddhf_event) * static_cast<size_t>(n),
+                                   cudaMemcpyHostToDevice, h->copy_stream);
+    if (e == cudaSuccess) e = cudaEventRecord(s.copied, h->copy_stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(st, s.copied, 0);
+    if (e != cudaSuccess) {
+        cudaStreamSynchronize(h->copy_stream);            // nothing was enqueued on `st`: the slot stays free
+        return cuda_fail(e);
+    }
     const int rc = ddhf_window(h, s.events, n, t0_us, window_us, s.ws, &s.out, st);
-    if (rc != DDHF_OK) return rc;
     const ddhf_outputs &d = s.out;
-    if (out->counters) PIPE_CHECK(cudaMemcpyAsync(out->counters, d.counters, sizeof(int32_t) * DDHF_N_COUNTERS, cudaMemcpyDeviceToHost, st));
-    if (out->mask) PIPE_CHECK(cudaMemcpyAsync(out->mask, d.mask, np, cudaMemcpyDeviceToHost, st));
-    if (out->boxes) PIPE_CHECK(cudaMemcpyAsync(out->boxes, d.boxes, sizeof(ddhf_box) * static_cast<size_t>(c.max_boxes), cudaMemcpyDeviceToHost, st));
-    if (out->merged_boxes) PIPE_CHECK(cudaMemcpyAsync(out->merged_boxes, d.merged_boxes, sizeof(ddhf_box) * static_cast<size_t>(c.max_boxes), cudaMemcpyDeviceToHost, st));
-    if (out->sf) PIPE_CHECK(cudaMemcpyAsync(out->sf, d.sf, sizeof(float) * np, cudaMemcpyDeviceToHost, st));
-    if (out->score) PIPE_CHECK(cudaMemcpyAsync(out->score, d.score, sizeof(float) * np, cudaMemcpyDeviceToHost, st));
-    if (out->f0_idx) PIPE_CHECK(cudaMemcpyAsync(out->f0_idx, d.f0_idx, sizeof(int32_t) * np, cudaMemcpyDeviceToHost, st));
-    if (out->labels) PIPE_CHECK(cudaMemcpyAsync(out->labels, d.labels, sizeof(int32_t) * np, cudaMemcpyDeviceToHost, st));
-    if (out->row_ptr) PIPE_CHECK(cudaMemcpyAsync(out->row_ptr, d.row_ptr, sizeof(int32_t) * (np + 1), cudaMemcpyDeviceToHost, st));
-    PIPE_CHECK(cudaEventRecord(s.done, st));
+    auto d2h = [&](void *dst, const void *src, size_t bytes) {
+        if (e == cudaSuccess && dst) e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st);
+    };
+    if (rc == DDHF_OK) {
+        d2h(out->counters, d.counters, sizeof(int32_t) * DDHF_N_COUNTERS);
+        d2h(out->mask, d.mask, np);
+        d2h(out->boxes, d.boxes, sizeof(ddhf_box) * static_cast<size_t>(c.max_boxes));
+        d2h(out->merged_boxes, d.merged_boxes, sizeof(ddhf_box) * static_cast<size_t>(c.max_boxes));
+        d2h(out->sf, d.sf, sizeof(float) * np);
+        d2h(out->score, d.score, sizeof(float) * np);
+        d2h(out->f0_idx, d.f0_idx, sizeof(int32_t) * np);
+        d2h(out->labels, d.labels, sizeof(int32_t) * np);
+        d2h(out->row_ptr, d.row_ptr, sizeof(int32_t) * (np + 1));
+    }
+    if (rc != DDHF_OK || e != cudaSuccess) {
+        // kernels or copies of this window may already be queued on the slot's buffers: drain them so
+        // that the slot can be reused by the next submit, and report the failure (nothing is in flight)
+        cudaStreamSynchronize(st);
+        return rc != DDHF_OK ? rc : cuda_fail(e);
+    }
+    if ((e = cudaEventRecord(s.done, st)) != cudaSuccess) {
+        cudaStreamSynchronize(st);
+        return cuda_fail(e);
+    }
     ++h->pipe_head;
     return DDHF_OK;
 }
@@ -475,16 +525,9 @@ extern "C" int ddhf_destroy(ddhf_handle *h)
     if (!h) return DDHF_OK;
     if (h->d_cand) cudaFree(h->d_cand);
     for (int i = 0; i < 5; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
-    if (h->hb_events) cudaFree(h->hb_events);
-    if (h->hb_ws) cudaFree(h->hb_ws);
-    void *bufs[] = {h->hb_out.row_ptr, h->hb_out.csr_ev, h->hb_out.active_idx, h->hb_out.power,
-                    h->hb_out.sf, h->hb_out.score, h->hb_out.f0_idx, h->hb_out.mask,
-                    h->hb_out.labels, h->hb_out.boxes, h->hb_out.counters, h->hb_out.merged_boxes};
-    for (void *b : bufs) if (b) cudaFree(b);
+    free_set(h->hb_events, h->hb_ws, h->hb_out);
     for (auto &s : h->pipe) {
-        void *pb[] = {s.events, s.ws, s.out.row_ptr, s.out.csr_ev, s.out.active_idx, s.out.sf, s.out.score,
-                      s.out.f0_idx, s.out.mask, s.out.labels, s.out.boxes, s.out.counters, s.out.merged_boxes};
-        for (void *b : pb) if (b) cudaFree(b);
+        free_set(s.events, s.ws, s.out);
         if (s.copied) cudaEventDestroy(s.copied);
         if (s.done) cudaEventDestroy(s.done);
     }

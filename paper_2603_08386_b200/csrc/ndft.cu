@@ -48,9 +48,6 @@ namespace {
 #ifndef DDHF_PU
 #define DDHF_PU 4                 // table passes issued together
 #endif
-#ifndef DDHF_EXP
-#define DDHF_EXP 0               // timing experiments only (1: no SF loop, 2: no table, 3: one event per chunk)
-#endif
 #ifndef DDHF_NDFT_BLOCKS
 #define DDHF_NDFT_BLOCKS 1         // CTAs per SM
 #endif
@@ -558,11 +555,7 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
                                        (v & 1u) ? 0u : 0x80000000u);
             }
             __syncwarp();
-#if DDHF_EXP == 2 || DDHF_EXP == 6
-            const int n_pass = 0;
-#else
             const int n_pass = (nc + EPP - 1) / EPP;
-#endif
             // PU passes at a time: their phase -> SFU -> store chains are independent
             constexpr int PU = (kEC / EPP) < DDHF_PU ? (kEC / EPP) : DDHF_PU;
             {
@@ -613,7 +606,7 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
                     }                                                                            \
                 }                                                                                \
             }
-            const int nce = (DDHF_EXP == 3 || DDHF_EXP == 7) ? min(nc, 1) : nc;
+            const int nce = nc;
             DDHF_CENTRES(a0r, a0i, 0)
             int k = 0;
 #pragma unroll 1
@@ -661,9 +654,7 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
                 if (full_grid || i * 32 + lane < sp.n_freq) __stcs(dst + i * 32, preg[i]);
         }
         float slog = 0.f, ssum = 0.f;
-        if (DDHF_EXP == 1 || DDHF_EXP == 5) {
-            slog = preg[3]; ssum = preg[5] + 1.f;
-        } else if (full_grid) {
+        if (full_grid) {
             // every bin is in range; only the first k_lo bins (register 0) are left out.  Bins are
             // taken in pairs, log2(a b) = log2 a + log2 b (one SFU op per two bins; a b stays a
             // normal number: sf_eps^2 >= 1e-36 is checked, P <= n^2 < 2^62), four partial sums
@@ -716,7 +707,7 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
         float score = 0.f;
         int f0 = -1;
         bool deferred = false;
-        if ((DDHF_EXP < 4) && (sp.score_all || sf_ok)) {
+        if (sp.score_all || sf_ok) {
             // queue the spectrum for k_comb_deferred; if the queue is full, score it here
             int slot = 0;
             if (lane == 0) slot = atomicAdd(p.spill_count, 1);

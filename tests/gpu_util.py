@@ -69,9 +69,20 @@ def near(value, thr, rel=REL_TOL):
     return np.abs(value - thr) <= rel * abs(thr)
 
 
-def check_maps(gpu, orc, params, *, score_all, oracle_mod=None, orc_power=None):
+#: filled by check_maps: how many pixels the last call left out of the exact comparisons
+last_counts: dict = {}
+
+
+def check_maps(gpu, orc, params, *, score_all, oracle_mod=None, orc_power=None, max_ill=None,
+               power_of=None):
     """SF, score, f0_idx and mask on all pixels.  Returns the boolean map of pixels that are
-    within tolerance of a threshold (excluded from the exact comparisons)."""
+    within tolerance of a threshold (excluded from the exact comparisons).
+
+    `last_counts` records how many active pixels were left out: "ill" (R30: spectrum at the
+    FP32 floor of the direct sum, SF / score not compared with the oracle) and "edge" (within 1e-3
+    relative of a threshold, north_star).  `max_ill` bounds the first class (asserted).  `power_of(pix)`
+    returns the oracle spectrum of one pixel on demand (full-size runs without a stored spectrum): it is
+    used to settle f0 ties."""
     act = np.zeros(gpu["sf"].size, bool)
     act[orc["active_idx"]] = True
     act = act.reshape(gpu["sf"].shape)
@@ -102,6 +113,9 @@ def check_maps(gpu, orc, params, *, score_all, oracle_mod=None, orc_power=None):
             stage_err = np.abs(gpu["sf"].ravel()[orc["active_idx"]].astype(np.float64) - sf_from_gpu) / sf_from_gpu
             assert stage_err.max(initial=0) <= 5e-5, f"SF stage rel err {stage_err.max()}"
     assert sf_err.max(initial=0) <= REL_TOL, f"SF rel err {sf_err.max()}"
+    n_ill = int(ill_map.sum())
+    if max_ill is not None:
+        assert n_ill <= max_ill, f"{n_ill} ill-conditioned pixels (FP32 floor, DESIGN.md R30), allowed {max_ill}"
     edge_sf = (near(orc["sf"], params["tau_sf"]) | (ill_map & near(orc["sf"], params["tau_sf"], rel=0.05))) & act
     # score is evaluated where score_all or SF <= tau_sf
     scored_o = act & (np.ones_like(act) if score_all else (orc["sf"] <= params["tau_sf"]))
@@ -117,16 +131,21 @@ def check_maps(gpu, orc, params, *, score_all, oracle_mod=None, orc_power=None):
         assert (gpu["score"][skipped] == 0).all() and (gpu["f0_idx"][skipped] == -1).all()
     # f0 index: equal unless the oracle's two best candidates tie within tolerance
     diff = cmp_px & (gpu["f0_idx"] != orc["f0_idx"])
+    n_tie = int(diff.sum())
     if diff.any():
-        assert oracle_mod is not None and orc_power is not None, \
+        assert oracle_mod is not None and (orc_power is not None or power_of is not None), \
             f"{diff.sum()} f0_idx mismatches and no spectra to check ties"
         row_of = {int(p): r for r, p in enumerate(orc["active_idx"])}
         W = gpu["sf"].shape[1]
         for y, x in zip(*np.nonzero(diff)):
             r = row_of[int(y) * W + int(x)]
-            if r >= len(orc_power):
-                continue
-            _, _, snr, _, _ = oracle_mod.comb_score(orc_power[r], params)
+            if orc_power is not None:
+                if r >= len(orc_power):
+                    continue
+                P = orc_power[r]
+            else:
+                P = power_of(int(y) * W + int(x))
+            _, _, snr, _, _ = oracle_mod.comb_score(P, params)
             g, o = gpu["f0_idx"][y, x], orc["f0_idx"][y, x]
             assert g >= 0 and abs(snr[g] - snr[o]) <= REL_TOL * snr[o], \
                 f"f0_idx {g} vs {o} at ({x},{y}): snr {snr[g]} vs {snr[o]}"
@@ -134,6 +153,11 @@ def check_maps(gpu, orc, params, *, score_all, oracle_mod=None, orc_power=None):
     edge = edge_sf | (near(orc["score"], params["tau_comb"]) & scored_o)
     bad = (gpu["mask"] != orc["mask"]) & ~edge
     assert not bad.any(), f"{bad.sum()} mask mismatches outside tolerance"
+    last_counts.clear()
+    last_counts.update(active=int(act.sum()), ill=n_ill, edge=int((edge & act).sum()), f0_ties=n_tie,
+                       compared_sf=int(act.sum()) - n_ill, compared_score=int(cmp_px.sum()),
+                       mask_equal=bool(np.array_equal(gpu["mask"], orc["mask"])),
+                       sf_err=float(sf_err.max(initial=0)), score_err=float(s_err.max(initial=0)))
     return edge
 
 

@@ -10,7 +10,7 @@ import gpu_util as gu
 pytestmark = pytest.mark.gpu
 
 
-def _full_compare(oracle, w, params, *, score_all, events=None, t0=None):
+def _full_compare(oracle, w, params, *, score_all, events=None, t0=None, max_ill=None):
     ev = w.events if events is None else events
     t0 = w.t0_us if t0 is None else t0
     orc = oracle.window(params, ev, t0, w.window_us, score_all=score_all, want_power=True)
@@ -19,7 +19,9 @@ def _full_compare(oracle, w, params, *, score_all, events=None, t0=None):
     gu.check_csr(gpu, orc)
     err = gu.power_error(gpu["power"], orc["power"])
     assert err <= gu.POWER_TOL, f"power error / peak = {err}"
-    gu.check_maps(gpu, orc, params, score_all=score_all, oracle_mod=oracle, orc_power=orc["power"])
+    gu.check_maps(gpu, orc, params, score_all=score_all, oracle_mod=oracle, orc_power=orc["power"],
+                  max_ill=max_ill)
+    print("  left out of the exact comparisons:", gu.last_counts)
     gu.check_boxes_against_oracle_ccl(gpu, oracle, params["a_min"])
     if np.array_equal(gpu["mask"], orc["mask"]):
         assert np.array_equal(gpu["boxes"], orc["boxes"].view(gpu["boxes"].dtype))
@@ -31,7 +33,7 @@ def _full_compare(oracle, w, params, *, score_all, events=None, t0=None):
 def test_config1_full(oracle, n_min, score_all):
     w = wl.make(1)
     prm = dict(w.params, n_min=n_min)
-    gpu, orc, err = _full_compare(oracle, w, prm, score_all=score_all)
+    gpu, orc, err = _full_compare(oracle, w, prm, score_all=score_all, max_ill=0 if n_min >= 6 else None)
     assert gpu["mask"].sum() >= 40            # the rotor patch is found
     print(f"cfg1 n_min={n_min} score_all={score_all}: power err/peak {err:.2e}, "
           f"active {gpu['n_active']}, scored {gpu['n_scored']}, mask {gpu['mask'].sum()}")
@@ -41,7 +43,7 @@ def test_config1_full(oracle, n_min, score_all):
 def test_config2_full(oracle, n_min, score_all):
     w = wl.make(2)
     prm = dict(w.params, n_min=n_min)
-    gpu, orc, err = _full_compare(oracle, w, prm, score_all=score_all)
+    gpu, orc, err = _full_compare(oracle, w, prm, score_all=score_all, max_ill=0 if n_min >= 6 else None)
     print(f"cfg2 n_min={n_min} score_all={score_all}: power err/peak {err:.2e}, "
           f"active {gpu['n_active']}, scored {gpu['n_scored']}, mask {gpu['mask'].sum()}")
 
@@ -89,7 +91,7 @@ def test_paper_native_grid(oracle):
 def test_config4_quarter_scale(oracle):
     """Config-4 scene on a 320x180 sensor: heavy-tailed rows, several size classes."""
     w = wl.make(4, scale=0.25)
-    gpu, orc, err = _full_compare(oracle, w, w.params, score_all=False)
+    gpu, orc, err = _full_compare(oracle, w, w.params, score_all=False, max_ill=0)
     assert np.diff(orc["row_ptr"]).max() > 500          # a long row is present
     print(f"cfg4/16: events {len(w.events)}, active {gpu['n_active']}, power err/peak {err:.2e}, "
           f"scored {gpu['n_scored']}, mask {gpu['mask'].sum()}, boxes {gpu['n_boxes']}")
@@ -232,3 +234,72 @@ def test_config4_bench_launch_configuration(oracle):
                 else np.array_equal(got[k], ref[k]))
         assert same, k
     assert got["n_scored"] == ref["n_scored"] and got["n_boxes"] == ref["n_boxes"]
+
+
+# ---------------------------------------------------------------------------------------------
+# Full-size windows against the WHOLE oracle window (north_star: "oracle-matching spectra and
+# detections on all five configs"): every pixel's SF, score, f0 index and mask, the boxes and the
+# merged detections; only the spectra stay sampled (tests above).  The oracle needs 10-30 s per
+# window on the box's host cores.
+# ---------------------------------------------------------------------------------------------
+def _whole_window_compare(oracle, w, params, ev, t0, *, score_all, name):
+    import time
+    t = time.perf_counter()
+    orc = oracle.window(params, ev, t0, w.window_us, score_all=score_all, want_power=False)
+    t_orc = time.perf_counter() - t
+    gpu = gu.run_gpu(params, ev, t0, w.window_us, score_all=score_all, want_power=False)
+    gu.check_csr(gpu, orc)
+
+    def power_of(pix):
+        seg = orc["csr_ev"][orc["row_ptr"][pix]:orc["row_ptr"][pix + 1]]
+        return oracle.ndft_power(seg >> 1, np.where(seg & 1, 1.0, -1.0), params["f_min_hz"],
+                                 params["df_hz"], params["n_freq"])
+
+    # no spectra are stored, so no pixel is excused as ill-conditioned: every active pixel's SF and
+    # every scored pixel's score is held to 1e-3 (DESIGN.md section 6 claims none needs the excuse
+    # on configs 1-5 with k_lo = 1)
+    edge = gu.check_maps(gpu, orc, params, score_all=score_all, oracle_mod=oracle, power_of=power_of)
+    c = dict(gu.last_counts)
+    assert c["ill"] == 0
+    # CCL / boxes / eq. 12 detections: the GPU's on its own mask are exact against the oracle's CCL of
+    # that mask; with the threshold-band pixels forced to the oracle's decision the mask IS the
+    # oracle's (checked above), and when no pixel needed forcing the boxes must be the oracle's too
+    gu.check_boxes_against_oracle_ccl(gpu, oracle, params["a_min"])
+    forced = np.where(edge, orc["mask"], gpu["mask"])
+    assert np.array_equal(forced, orc["mask"])
+    n_forced = int((gpu["mask"] != orc["mask"]).sum())
+    if n_forced == 0:
+        assert np.array_equal(gpu["boxes"], orc["boxes"].view(gpu["boxes"].dtype))
+        if "merged_boxes" in gpu:
+            want = oracle.merge_boxes(orc["boxes"].view(gpu["boxes"].dtype), float(np.float32(params["merge_alpha"])))
+            assert np.array_equal(gpu["merged_boxes"], want.view(gpu["merged_boxes"].dtype))
+    print(f"{name}: events {gpu['n_in']}, active {c['active']}, scored {gpu['n_scored']}, mask {int(gpu['mask'].sum())}, "
+          f"boxes {gpu['n_boxes']}, detections {len(gpu.get('merged_boxes', []))}; whole-window oracle {t_orc:.1f} s; "
+          f"SF err {c['sf_err']:.2e}, score err {c['score_err']:.2e}; pixels inside a 1e-3 threshold band {c['edge']}, "
+          f"mask pixels that needed forcing {n_forced}, f0 ties {c['f0_ties']}, ill-conditioned 0")
+    return gpu, orc
+
+
+@pytest.mark.slow
+def test_config3_whole_window(oracle):
+    w = wl.make(3)
+    _whole_window_compare(oracle, w, w.params, w.events, 0, score_all=False, name="cfg3 whole window")
+
+
+@pytest.mark.slow
+def test_config4_whole_window(oracle):
+    w = wl.make(4)
+    _whole_window_compare(oracle, w, w.params, w.events, 0, score_all=False, name="cfg4 whole window")
+
+
+@pytest.mark.slow
+def test_config5_whole_window(oracle):
+    w = wl.make(5, n_windows=3)
+    lo, n, t0 = w.window_slice(1)
+    _whole_window_compare(oracle, w, w.params, w.events[lo:lo + n], t0, score_all=False, name="cfg5 window 1")
+
+
+@pytest.mark.slow
+def test_paper_point_whole_window(oracle):
+    w = wl.paper_native()
+    _whole_window_compare(oracle, w, w.params, w.events, 0, score_all=False, name="paper point whole window")
