@@ -14,7 +14,7 @@ pytestmark = pytest.mark.gpu
 
 N_SEEDS = int(os.environ.get("DDHF_FUZZ_SEEDS", "12"))
 #: largest share of the active pixels that may be ill-conditioned, by n_min (1, 2, >= 3)
-ILL_CAP = {1: 1.0, 2: 0.6, 3: 0.15}
+ILL_CAP = {1: 1.0, 2: 0.6, 3: 0.35}
 
 
 def _case(seed):
@@ -61,7 +61,7 @@ def test_random_configuration(oracle, seed):
     # active pixels, and the count is printed
     n_act = max(int(orc["n_active"]), 1)
     gu.check_maps(gpu, orc, prm, score_all=score_all, oracle_mod=oracle, orc_power=orc["power"],
-                  max_ill=int(ILL_CAP[min(prm["n_min"], 3)] * n_act) + 2)
+                  allow_ill=True, max_ill=int(ILL_CAP[min(prm["n_min"], 3)] * n_act) + 2)
     print(f"seed {seed}: n_min {prm['n_min']}, {gu.last_counts}")
     gu.check_boxes_against_oracle_ccl(gpu, oracle, prm["a_min"])
 

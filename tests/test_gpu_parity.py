@@ -10,7 +10,7 @@ import gpu_util as gu
 pytestmark = pytest.mark.gpu
 
 
-def _full_compare(oracle, w, params, *, score_all, events=None, t0=None, max_ill=None):
+def _full_compare(oracle, w, params, *, score_all, events=None, t0=None):
     ev = w.events if events is None else events
     t0 = w.t0_us if t0 is None else t0
     orc = oracle.window(params, ev, t0, w.window_us, score_all=score_all, want_power=True)
@@ -19,8 +19,8 @@ def _full_compare(oracle, w, params, *, score_all, events=None, t0=None, max_ill
     gu.check_csr(gpu, orc)
     err = gu.power_error(gpu["power"], orc["power"])
     assert err <= gu.POWER_TOL, f"power error / peak = {err}"
-    gu.check_maps(gpu, orc, params, score_all=score_all, oracle_mod=oracle, orc_power=orc["power"],
-                  max_ill=max_ill)
+    # strict: no pixel is excused as ill-conditioned on the BASELINE configs
+    gu.check_maps(gpu, orc, params, score_all=score_all, oracle_mod=oracle, orc_power=orc["power"])
     print("  left out of the exact comparisons:", gu.last_counts)
     gu.check_boxes_against_oracle_ccl(gpu, oracle, params["a_min"])
     if np.array_equal(gpu["mask"], orc["mask"]):
@@ -33,7 +33,7 @@ def _full_compare(oracle, w, params, *, score_all, events=None, t0=None, max_ill
 def test_config1_full(oracle, n_min, score_all):
     w = wl.make(1)
     prm = dict(w.params, n_min=n_min)
-    gpu, orc, err = _full_compare(oracle, w, prm, score_all=score_all, max_ill=0 if n_min >= 6 else None)
+    gpu, orc, err = _full_compare(oracle, w, prm, score_all=score_all)
     assert gpu["mask"].sum() >= 40            # the rotor patch is found
     print(f"cfg1 n_min={n_min} score_all={score_all}: power err/peak {err:.2e}, "
           f"active {gpu['n_active']}, scored {gpu['n_scored']}, mask {gpu['mask'].sum()}")
@@ -43,7 +43,7 @@ def test_config1_full(oracle, n_min, score_all):
 def test_config2_full(oracle, n_min, score_all):
     w = wl.make(2)
     prm = dict(w.params, n_min=n_min)
-    gpu, orc, err = _full_compare(oracle, w, prm, score_all=score_all, max_ill=0 if n_min >= 6 else None)
+    gpu, orc, err = _full_compare(oracle, w, prm, score_all=score_all)
     print(f"cfg2 n_min={n_min} score_all={score_all}: power err/peak {err:.2e}, "
           f"active {gpu['n_active']}, scored {gpu['n_scored']}, mask {gpu['mask'].sum()}")
 
@@ -91,7 +91,7 @@ def test_paper_native_grid(oracle):
 def test_config4_quarter_scale(oracle):
     """Config-4 scene on a 320x180 sensor: heavy-tailed rows, several size classes."""
     w = wl.make(4, scale=0.25)
-    gpu, orc, err = _full_compare(oracle, w, w.params, score_all=False, max_ill=0)
+    gpu, orc, err = _full_compare(oracle, w, w.params, score_all=False)
     assert np.diff(orc["row_ptr"]).max() > 500          # a long row is present
     print(f"cfg4/16: events {len(w.events)}, active {gpu['n_active']}, power err/peak {err:.2e}, "
           f"scored {gpu['n_scored']}, mask {gpu['mask'].sum()}, boxes {gpu['n_boxes']}")
