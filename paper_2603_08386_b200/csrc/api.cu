@@ -1,5 +1,6 @@
 // api.cu -- the C ABI of include/ddhf.h: handle, constant tables, workspace layout, the
 // per-window launch sequence and the host-buffer (end-to-end) variant.
+#include <algorithm>
 #include <math.h>
 #include <stdio.h>
 #include <string.h>
@@ -26,7 +27,9 @@ struct ddhf_handle {
     int spill_cap = 0;
     ScoreParams sp{};
     uint64_t g_f0 = 0, g_d = 0, g_h = 0;
-    CandTable *d_cand = nullptr;
+    unsigned char *d_tables = nullptr;      // comb tables (num_tab | piece_tab | meta)
+    int band_size = 0;
+    int ndft_blocks_per_sm = 1, score_blocks_per_sm = 1;
     // workspace offsets (bytes)
     size_t off_cnt = 0, off_pairs = 0, off_work = 0, off_tiles = 0, off_class = 0, off_cursor = 0, off_thist = 0, off_chunk = 0, off_binbase = 0, off_spill = 0, off_spillrec = 0,
            off_parent = 0, off_rec = 0, off_ctiles = 0, ws_bytes = 0;
@@ -112,68 +115,114 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
         return fail(nullptr, DDHF_E_CUDA, "ddhf_create: no CUDA device");
     }
 
-    // ---- comb tables (R7-R10): harmonic centres, validity prefix, union intervals, rank ----
-    std::vector<CandTable> tab(c.n_f0);
+    // ---- comb tables (R7-R10): harmonic centres, validity prefix, union of the windows, median rank ------
     const int nb = c.n_freq - c.k_lo, d = c.half_bw_bins;
-    int r0 = 1 << 30, r1 = -1;
+    const int nbl = ndft_bins_per_lane(c.n_freq);
+    const int cpad = (c.n_f0 + 31) / 32 * 32;
+    const int wlen = 2 * d + 1;
+    int s_lvl = 0;
+    while (s_lvl < 5 && (2 << s_lvl) <= wlen) ++s_lvl;               // 2^s_lvl <= min(wlen, 32)
+    const int blk = 1 << s_lvl;
+    if (wlen > 2 * blk) {
+        delete h;
+        return fail(nullptr, DDHF_E_INVAL, "ddhf_create: half_bw_bins must be <= 31 (harmonic window <= 63 bins)");
+    }
+    auto padk = [nbl](long long k) { return static_cast<uint32_t>(k + k / nbl); };
+    struct Cand { int mv = 0, rank = 0, n_excl = 0; std::vector<int> kc; std::vector<std::pair<int, int>> pieces; };
+    std::vector<Cand> cand(c.n_f0);
+    int r0 = 1 << 30, r1 = -1, max_pieces = 1;
     for (int ci = 0; ci < c.n_f0; ++ci) {
-        CandTable &t = tab[ci];
-        memset(&t, 0, sizeof(t));
+        Cand &t = cand[ci];
         const double f0 = c.f0_min_hz + ci * c.f0_step_hz;
-        int mv = 0;
         for (int m = 1; m <= c.n_harm; ++m) {
             const long long km = static_cast<long long>(floor((m * f0 - c.f_min_hz) / c.df_hz + 0.5));
             if (km - d < c.k_lo || km + d > c.n_freq - 1) break;
-            t.kc[m - 1] = static_cast<int16_t>(km);
-            mv = m;
+            t.kc.push_back(static_cast<int>(km));
         }
+        int mv = static_cast<int>(t.kc.size());
         if (mv < c.h_min) continue;
-        int ni = 0, n_excl = 0;
+        // union of the windows as disjoint intervals (centres rise with m), cut into pieces of <= 32 bins
+        std::vector<std::pair<int, int>> iv;
+        int n_excl = 0;
         for (int m = 0; m < mv; ++m) {
             const int lo = t.kc[m] - d, hi = t.kc[m] + d;
-            if (ni > 0 && lo <= t.hi[ni - 1]) {
-                if (hi > t.hi[ni - 1]) { n_excl += hi - t.hi[ni - 1]; t.hi[ni - 1] = static_cast<int16_t>(hi); }
+            if (!iv.empty() && lo <= iv.back().second) {
+                if (hi > iv.back().second) { n_excl += hi - iv.back().second; iv.back().second = hi; }
             } else {
-                t.lo[ni] = static_cast<int16_t>(lo);
-                t.hi[ni] = static_cast<int16_t>(hi);
+                iv.emplace_back(lo, hi);
                 n_excl += hi - lo + 1;
-                ++ni;
             }
         }
         const int n_comp = nb - n_excl;
         if (n_comp <= 0) continue;
-        t.m_valid = static_cast<int16_t>(mv);
-        t.n_int = static_cast<int16_t>(ni);
-        t.n_excl = static_cast<int16_t>(n_excl);
-        t.rank = static_cast<int16_t>((n_comp - 1) / 2);
-        r0 = t.rank < r0 ? t.rank : r0;
-        r1 = t.rank + n_excl > r1 ? t.rank + n_excl : r1;
+        for (const auto &q : iv)
+            for (int s = q.first; s <= q.second; s += 32)
+                t.pieces.emplace_back(s, std::min(32, q.second - s + 1));
+        t.mv = mv;
+        t.n_excl = n_excl;
+        t.rank = (n_comp - 1) / 2;
+        r0 = std::min(r0, t.rank);
+        r1 = std::max(r1, t.rank + n_excl);
+        max_pieces = std::max(max_pieces, static_cast<int>(t.pieces.size()));
     }
     if (r1 < 0) { r0 = 0; r1 = 0; }
-    if (ndft_band_size(c.n_freq, r0, r1) == 0) {
+    const int band_size = ndft_band_size(c.n_freq, r0, r1);
+    if (band_size == 0 || max_pieces > kMaxPieces) {
         delete h;
         return fail(nullptr, DDHF_E_INVAL,
                     "ddhf_create: harmonic windows exclude too many bins for the band sorter "
-                    "(n_harm * (2 half_bw_bins + 1) too large for n_freq)");
+                    "(the union of a candidate's windows must stay below about 900 of 2048 bins; "
+                    "n_harm * (2 half_bw_bins + 1) too large for n_freq)");
     }
-    if (cudaMalloc(&h->d_cand, sizeof(CandTable) * c.n_f0) != cudaSuccess ||
-        cudaMemcpy(h->d_cand, tab.data(), sizeof(CandTable) * c.n_f0, cudaMemcpyHostToDevice) != cudaSuccess) {
+    {
+        // one device buffer: num_tab [n_harm][cpad] u32 | piece_tab [max_pieces][cpad] uint2 | meta [cpad] uint4
+        // rows padded to a multiple of 8 (the kernel reads the tables 8 rows at a time, unconditionally)
+        const size_t n_num = static_cast<size_t>((c.n_harm + 7) / 8 * 8) * cpad, n_pc = static_cast<size_t>((max_pieces + 7) / 8 * 8) * cpad;
+        const size_t off_pc = align_up(n_num * sizeof(uint32_t), 16), off_meta = align_up(off_pc + n_pc * sizeof(uint2), 16);
+        const size_t bytes = off_meta + static_cast<size_t>(cpad) * sizeof(uint4);
+        std::vector<unsigned char> host(bytes, 0);
+        uint32_t *num_tab = reinterpret_cast<uint32_t *>(host.data());
+        uint2 *piece_tab = reinterpret_cast<uint2 *>(host.data() + off_pc);
+        uint4 *meta = reinterpret_cast<uint4 *>(host.data() + off_meta);
+        for (int ci = 0; ci < c.n_f0; ++ci) {
+            const Cand &t = cand[ci];
+            if (t.mv == 0) continue;
+            for (int m = 0; m < t.mv; ++m)
+                num_tab[static_cast<size_t>(m) * cpad + ci] = padk(t.kc[m] - d) | (padk(t.kc[m] + d - blk + 1) << 16);
+            for (size_t q = 0; q < t.pieces.size(); ++q) {
+                const int len = t.pieces[q].second;
+                piece_tab[q * cpad + ci] = make_uint2(len >= 32 ? 0xffffffffu : ((1u << len) - 1u),
+                                                      static_cast<uint32_t>(t.pieces[q].first));
+            }
+            const float inv_mv = 1.0f / static_cast<float>(t.mv);
+            uint32_t inv_bits;
+            memcpy(&inv_bits, &inv_mv, 4);
+            meta[ci] = make_uint4(static_cast<uint32_t>(t.mv) | (static_cast<uint32_t>(t.pieces.size()) << 16),
+                                  static_cast<uint32_t>(t.rank) | (static_cast<uint32_t>(t.n_excl) << 16), inv_bits, 0u);
+        }
+        if (cudaMalloc(&h->d_tables, bytes) != cudaSuccess ||
+            cudaMemcpy(h->d_tables, host.data(), bytes, cudaMemcpyHostToDevice) != cudaSuccess) {
+            const std::string msg = std::string("ddhf_create: ") + cudaGetErrorString(cudaGetLastError());
+            if (h->d_tables) cudaFree(h->d_tables);
+            delete h;
+            return fail(nullptr, DDHF_E_CUDA, msg);
+        }
+        h->sp.num_tab = reinterpret_cast<const uint32_t *>(h->d_tables);
+        h->sp.piece_tab = reinterpret_cast<const uint2 *>(h->d_tables + off_pc);
+        h->sp.meta = reinterpret_cast<const uint4 *>(h->d_tables + off_meta);
+    }
+    h->band_size = band_size;
+    if (ingest_configure() != cudaSuccess || (c.merge_alpha > 0.f && ccl_configure(c.max_boxes) != cudaSuccess) ||
+        ndft_configure(c.n_freq, band_size, cpad, &h->ndft_blocks_per_sm, &h->score_blocks_per_sm) != cudaSuccess) {
         const std::string msg = std::string("ddhf_create: ") + cudaGetErrorString(cudaGetLastError());
-        if (h->d_cand) cudaFree(h->d_cand);
+        cudaFree(h->d_tables);
         delete h;
         return fail(nullptr, DDHF_E_CUDA, msg);
     }
-    if (ingest_configure() != cudaSuccess || (c.merge_alpha > 0.f && ccl_configure(c.max_boxes) != cudaSuccess)) {
-        const std::string msg = std::string("ddhf_create: ") + cudaGetErrorString(cudaGetLastError());
-        cudaFree(h->d_cand);
-        delete h;
-        return fail(nullptr, DDHF_E_CUDA, msg);
-    }
-    h->sp.n_freq = c.n_freq; h->sp.k_lo = c.k_lo; h->sp.n_f0 = c.n_f0; h->sp.half_bw = d;
-    h->sp.r0 = r0; h->sp.r1 = r1;
+    h->sp.n_freq = c.n_freq; h->sp.k_lo = c.k_lo; h->sp.n_f0 = c.n_f0; h->sp.n_harm = c.n_harm; h->sp.half_bw = d;
+    h->sp.s_lvl = s_lvl; h->sp.r0 = r0; h->sp.r1 = r1; h->sp.cpad = cpad; h->sp.max_pieces = max_pieces;
     h->sp.tau_sf = c.tau_sf; h->sp.tau_comb = c.tau_comb; h->sp.sf_eps = c.sf_eps;
     h->sp.score_all = (c.flags & DDHF_FLAG_SCORE_ALL) ? 1 : 0;
-    h->sp.cand = h->d_cand;
 
     // ---- fixed-point frequency constants of the factorised NDFT ------------------------------
     const int tn = ndft_tn(c.n_freq);
@@ -201,7 +250,7 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
         const size_t ev_tiles = (static_cast<size_t>(c.max_events) + ingest_tile_events() - 1) / ingest_tile_events();
         const size_t ev_chunks = (ev_tiles + ingest_chunk_tiles() - 1) / ingest_chunk_tiles();
         if (2 * ev_chunks * bins >= (1ull << 31)) {
-            cudaFree(h->d_cand);
+            cudaFree(h->d_tables);
             delete h;
             return fail(nullptr, DDHF_E_INVAL, "ddhf_create: max_events too large for this sensor size");
         }
@@ -214,6 +263,7 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
     // pixels beyond the capacity are scored in place by the NDFT kernel)
     h->spill_cap = h->np < 32768 ? h->np : 32768;
     if (c.max_scored > 0) h->spill_cap = c.max_scored < h->np ? c.max_scored : h->np;
+    if (!ndft_scores_in_place(c.n_freq, band_size)) h->spill_cap = h->np;      // every pixel must fit in the queue
     h->off_spill = o;      o = align_up(o + sizeof(float) * static_cast<size_t>(h->spill_cap) * ndft_padded_bins(c.n_freq));
     h->off_spillrec = o;   o = align_up(o + sizeof(SpillRec) * static_cast<size_t>(h->spill_cap));
     h->off_parent = o;     o = align_up(o + sizeof(int32_t) * h->np);
@@ -305,7 +355,8 @@ extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n
     if (timing) cudaEventRecord(h->ev[0], st);
     launches += launch_ingest(ip, st);
     if (timing) cudaEventRecord(h->ev[1], st);
-    launches += launch_ndft(np, c.n_freq, h->sm_count, st, timing ? h->ev[2] : nullptr);
+    launches += launch_ndft(np, c.n_freq, h->band_size, h->sm_count * h->ndft_blocks_per_sm,
+                            h->sm_count * h->score_blocks_per_sm, st, timing ? h->ev[2] : nullptr);
     if (timing) cudaEventRecord(h->ev[3], st);
     launches += launch_ccl(cp, st);
     if (timing) { cudaEventRecord(h->ev[4], st); h->timed_once = true; }
@@ -523,7 +574,7 @@ extern "C" int ddhf_fma_peak_probe(float ms_target, float *tflops_out, void *cud
 extern "C" int ddhf_destroy(ddhf_handle *h)
 {
     if (!h) return DDHF_OK;
-    if (h->d_cand) cudaFree(h->d_cand);
+    if (h->d_tables) cudaFree(h->d_tables);
     for (int i = 0; i < 5; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
     free_set(h->hb_events, h->hb_ws, h->hb_out);
     for (auto &s : h->pipe) {

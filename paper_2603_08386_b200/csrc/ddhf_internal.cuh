@@ -11,6 +11,7 @@ namespace ddhf {
 
 constexpr int kMaxHarm = 16;       // n_harm limit
 constexpr int kMaxF0 = 256;        // n_f0 limit
+constexpr int kMaxPieces = 64;     // pieces of <= 32 bins of one candidate's excluded set
 constexpr int kNumClasses = 12;    // work-list size classes (by log2 of the row length)
 constexpr int kScanTile = 4096;    // elements per scan tile (1024 threads x 4)
 
@@ -22,24 +23,24 @@ struct __align__(16) WorkItem {
     int32_t arow;        // row of the compact outputs (index into active_idx)
 };
 
-// Per-candidate comb tables, built on the host at create time (readings R7-R10).
-struct CandTable {
-    int16_t m_valid;             // valid harmonics (0 = candidate skipped)
-    int16_t n_int;               // disjoint intervals of the union of the windows
-    int16_t rank;                // 0-based rank of the lower median in the complement
-    int16_t n_excl;              // bins in the union
-    int16_t kc[kMaxHarm];        // centre bin of harmonic m (index m-1)
-    int16_t lo[kMaxHarm];        // union intervals, inclusive
-    int16_t hi[kMaxHarm];
-};
-
-struct ScoreParams {
-    int32_t n_freq, k_lo, n_f0, half_bw;
+// Constants of the SF / comb stages (a5-a7) and the per-candidate tables, built on the host at create
+// time (readings R7-R10).  Tables are padded to `cpad` candidates (a multiple of 32) so that a warp
+// reads them without range checks; layout [row][cpad], candidate fastest (coalesced per lane).
+struct CombParams {
+    int32_t n_freq, k_lo, n_f0, n_harm, half_bw;
+    int32_t s_lvl;               // block maxima of 2^s_lvl bins, 2^s_lvl <= min(2 half_bw + 1, 32)
     int32_t r0, r1;              // full-spectrum rank band that holds every complement median
+    int32_t cpad, max_pieces;
     float tau_sf, tau_comb, sf_eps;
     int32_t score_all;
-    const CandTable *cand;       // DEVICE [n_f0]
+    const uint32_t *num_tab;     // DEVICE [n_harm][cpad]: padded indices of the two block maxima that cover the
+                                 // window of harmonic m (lo | hi << 16); 0 beyond M_valid
+    const uint2 *piece_tab;      // DEVICE [max_pieces][cpad]: the union of the windows in pieces of <= 32 bins,
+                                 // {mask of the piece's length, first bin}; mask 0 beyond the candidate's pieces
+    const uint4 *meta;           // DEVICE [cpad]: {M_valid | n_pieces << 16, rank of the lower median in the
+                                 // complement | n_excl << 16, float bits of 1 / M_valid, 0}; M_valid 0 = skipped
 };
+typedef CombParams ScoreParams;
 
 // One row of the deferred-scoring queue (a pixel that passed the SF filter).
 struct __align__(16) SpillRec {
@@ -120,7 +121,7 @@ int launch_ingest(const IngestParams &p, cudaStream_t st);
 cudaError_t ingest_configure();              // opt in to large dynamic shared memory
 int ingest_tile_events();                    // events per partition tile
 int ingest_chunk_tiles();                    // tiles per scan chunk
-int launch_ndft(const NdftParams &p, int n_freq, int sm_count, cudaStream_t st, cudaEvent_t between);
+int launch_ndft(const NdftParams &p, int n_freq, int band_size, int grid_ndft, int grid_score, cudaStream_t st, cudaEvent_t between);
                                              // `between` (optional) is recorded after the NDFT kernel, before the scoring kernel
 int launch_ccl(const CclParams &p, cudaStream_t st);
 cudaError_t ccl_configure(int max_boxes);    // shared memory of the box-merge kernel
@@ -128,5 +129,8 @@ int ndft_bins_per_lane(int n_freq);          // 8, 16, 32 or 64
 int ndft_tn(int n_freq);                     // offset pairs per centre for that kernel
 int ndft_padded_bins(int n_freq);            // row length of the deferred-scoring queue
 int ndft_band_size(int n_freq, int r0, int r1);   // sort capacity needed, 0 if unsupported
+cudaError_t ndft_configure(int n_freq, int band_size, int cpad, int *blocks_per_sm, int *score_blocks_per_sm);
+                                             // opt in to the kernels' dynamic shared memory on the current device
+bool ndft_scores_in_place(int n_freq, int band_size);   // whether the NDFT kernel can score a pixel itself when the queue is full
 
 }  // namespace ddhf

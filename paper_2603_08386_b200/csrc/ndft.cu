@@ -33,7 +33,7 @@
 //   candidate then only corrects the rank for its own excluded bins (prefix counts from warp
 //   ballots + a bitmask of excluded in-band positions).  Window maxima of eq. 8 come from a
 //   table of forward block maxima built by warp shuffles.
-#include "ddhf_internal.cuh"
+#include "comb.cuh"
 
 namespace ddhf {
 
@@ -54,25 +54,23 @@ namespace {
 constexpr int kWarps = DDHF_NDFT_WARPS;
 constexpr int kEC = 32;            // events per table chunk
 constexpr unsigned kFull = 0xffffffffu;
-constexpr uint32_t kInvalidKey = 0x7fffffffu;
 
+// Per-warp shared memory of k_ndft_score: the phasor table / phase words of the event loop and the
+// staged CSR events; the scoring scratch of comb.cuh (in-place scoring, only when the deferred queue is
+// full) aliases the table.  INPLACE = false (band sorter of 1024 values): the queue holds every pixel.
 template <int TM, int TN, int BS>
 struct Layout {
     static constexpr int NBL = TM * 2 * TN;                 // bins per lane
     static constexpr int NB = NBL * 32;                     // padded spectrum length
-    static constexpr int P_WORDS = NB + NBL;                // P_s[j + (j >> 5)]
+    static constexpr bool INPLACE = BS <= 512;
     static constexpr int TAB_WORDS = kEC * TN * 2 + kEC * 4;
-    // scoring scratch (aliases the phasor table)
-    static constexpr int BAL_WORDS = 4 * (NBL + 1);         // belw, inbw, belc, inbc
-    static constexpr int BAND_WORDS = BS;                   // bandv
-    static constexpr int SORT_WORDS = BS;                   // sortv
-    static constexpr int POS_WORDS = BS / 2;                // posb (u16)
-    static constexpr int MASK_WORDS = BS;                   // maskw[BS/32][32]
-    static constexpr int SCORE_WORDS = BAL_WORDS + BAND_WORDS + SORT_WORDS + POS_WORDS + MASK_WORDS;
-    static constexpr int SCRATCH_WORDS = (SCORE_WORDS > TAB_WORDS ? SCORE_WORDS : TAB_WORDS);
     static constexpr int EV_WORDS = 2 * kEC;                // staged CSR events, double buffered
-    static constexpr int WARP_WORDS = ((P_WORDS + SCRATCH_WORDS + EV_WORDS + 3) / 4) * 4;
-    static constexpr size_t SMEM_BYTES = static_cast<size_t>(WARP_WORDS) * 4 * kWarps;
+    __host__ __device__ static constexpr int scratch_words(int cpad)
+    {
+        return INPLACE && CombSmem<NBL, BS>::words(cpad) > TAB_WORDS ? CombSmem<NBL, BS>::words(cpad) : TAB_WORDS;
+    }
+    __host__ __device__ static constexpr int warp_words(int cpad) { return ((scratch_words(cpad) + EV_WORDS + 3) / 4) * 4; }
+    static size_t smem_bytes(int cpad) { return static_cast<size_t>(warp_words(cpad)) * 4 * kWarps; }
 };
 
 __device__ __forceinline__ uint32_t phase_u32(uint64_t g, uint32_t t)
@@ -91,8 +89,6 @@ __device__ __forceinline__ void sincos_u32(uint32_t ph, float &s, float &c)
     s = __sinf(r);
     c = __cosf(r);
 }
-
-__device__ __forceinline__ int pad(int j) { return j + (j >> 5); }
 
 // The work list is ordered by descending row length.  Warps take items from both ends: "head"
 // warps the long rows (FMA-pipe bound), "tail" warps the short ones (dominated by the
@@ -135,348 +131,6 @@ __device__ __forceinline__ WorkItem make_item()
     return w;
 }
 
-template <int E>
-__device__ __forceinline__ void bitonic_sort_regs(float (&x)[E], int lane)
-{
-    constexpr int N = E * 32;
-#pragma unroll
-    for (int k = 2; k <= N; k <<= 1) {
-#pragma unroll
-        for (int j = k >> 1; j > 0; j >>= 1) {
-            if (j < E) {
-#pragma unroll
-                for (int r = 0; r < E; ++r) {
-                    if ((r & j) == 0) {
-                        const bool asc = (k < E) ? ((r & k) == 0)
-                                                 : (k == N ? true : ((lane & (k / E)) == 0));
-                        const float a = x[r], b = x[r | j];
-                        const float lo = fminf(a, b), hi = fmaxf(a, b);
-                        x[r] = asc ? lo : hi;
-                        x[r | j] = asc ? hi : lo;
-                    }
-                }
-            } else {
-                const int lm = j / E;
-                const bool asc = (k == N) ? true : ((lane & (k / E)) == 0);
-                const bool lower = (lane & lm) == 0;
-                const bool take_min = (lower == asc);
-#pragma unroll
-                for (int r = 0; r < E; ++r) {
-                    const float o = __shfl_xor_sync(kFull, x[r], lm);
-                    x[r] = take_min ? fminf(x[r], o) : fmaxf(x[r], o);
-                }
-            }
-        }
-    }
-}
-
-// Next trial key of the band-limit search.  [lo, hi] brackets the wanted key, cLo / cHi are
-// #{key < lo}, #{key < hi}.  Without a finite upper bound: exponential-tail model through
-// (lo, cLo); otherwise linear interpolation of the rank in value space, with a plain bisection
-// of the key interval every third step so that the search always converges.
-__device__ __forceinline__ uint32_t next_pivot(uint32_t lo, uint32_t hi, int cLo, int cHi, float target,
-                                               int it, float nbf)
-{
-    uint32_t piv;
-    if (hi > 0x7f7fffffu) {
-        float g = 4.f;
-        if (cLo > 0)
-            g = __logf(fmaxf(1.f - target / nbf, 1e-6f)) / __logf(fmaxf(1.f - static_cast<float>(cLo) / nbf, 1e-6f));
-        g = fminf(fmaxf(g, 1.0625f), 16.f);
-        piv = __float_as_uint(fmaxf(__uint_as_float(lo), 1e-30f) * g);
-    } else if ((it % 3) == 2 || cHi <= cLo) {
-        piv = lo + ((hi - lo) >> 1);
-    } else {
-        const float vlo = __uint_as_float(lo), vhi = __uint_as_float(hi);
-        const float fr = (target - static_cast<float>(cLo)) / static_cast<float>(cHi - cLo);
-        piv = __float_as_uint(vlo + (vhi - vlo) * fminf(fmaxf(fr, 0.02f), 0.98f));
-    }
-    return min(max(piv, lo + 1u), hi - 1u);
-}
-
-// ----------------------------------------------------------------------------------------
-// a6: comb score of one pixel.  preg: the lane's NBL powers (bins lane + 32 i); P_s: the same
-// spectrum in the warp's shared memory, bin j at P_s[j + (j >> 5)] (overwritten);
-// returns (score, f0 index) on every lane.
-// ----------------------------------------------------------------------------------------
-template <int TM, int TN, int BS>
-__device__ __forceinline__ void comb_score(const float (&preg)[TM * 2 * TN], float *P_s, uint32_t *scr,
-                                           const ScoreParams &sp, float mean_p, int lane,
-                                           float &score_out, int &f0_out, float *dbg)
-{
-    using L = Layout<TM, TN, BS>;
-    constexpr int NBL = L::NBL;
-    constexpr int E = BS / 32;
-    uint32_t *belw = scr;
-    uint32_t *inbw = belw + (NBL + 1);
-    uint32_t *belc = inbw + (NBL + 1);
-    uint32_t *inbc = belc + (NBL + 1);
-    float *bandv = reinterpret_cast<float *>(inbc + (NBL + 1));
-    float *sortv = bandv + BS;
-    unsigned short *posb = reinterpret_cast<unsigned short *>(sortv + BS);
-    uint32_t *maskw = reinterpret_cast<uint32_t *>(sortv + BS) + BS / 2;
-
-    const int nb = sp.n_freq - sp.k_lo;
-    const int r0 = sp.r0, r1 = sp.r1;
-    const int slack = (BS - (r1 - r0 + 1)) / 2;
-
-    // The spectrum is read back from the warp's shared-memory copy in rolled loops: this part
-    // runs on a small share of the pixels, and compact code matters more here than registers.
-    uint32_t *K = reinterpret_cast<uint32_t *>(P_s);     // keys: K[33 i + lane]
-    // invalid bins (below k_lo, or padding past n_freq) never take part in the order statistics
-#pragma unroll 1
-    for (int i = 0; i < NBL; ++i) {
-        const int j = i * 32 + lane;
-        if (j < sp.k_lo || j >= sp.n_freq) K[i * 33 + lane] = kInvalidKey;
-        if (i == 0 && sp.k_lo <= 32) i = max(0, (sp.n_freq >> 5) - 1);        // only the ends can be invalid
-    }
-    __syncwarp();
-
-    // ---- A: band limits by counting passes over the spectrum -------------------------------
-    // find Lkey with  r0 - slack <= #{key < Lkey} <= r0   and Ukey with
-    // r1 + 1 <= #{key < Ukey} <= r1 + 1 + slack; on heavy ties the search converges to the
-    // exact order statistic and the tied bins are split by their order in the spectrum.
-    uint32_t loL = 0u, hiL = 0x7f800001u, loU = 0u, hiU = 0x7f800001u;
-    int cntLo_L = 0, cntLo_U = 0;          // #{key < loL}, #{key < loU}
-    int cntHi_L = nb, cntHi_U = nb;        // #{key < hiL}, #{key < hiU}
-    const float nbf = static_cast<float>(nb);
-    const float tgtL = r0 - 0.5f * slack, tgtU = r1 + 1 + 0.5f * slack;
-    bool doneL = false, doneU = false, exactL = false, exactU = false;
-    // first pivots: exponential-spectrum guess around the mean power
-    uint32_t pivL, pivU;
-    {
-        const float qL = fminf(fmaxf((r0 - 0.5f * slack) / nb, 0.01f), 0.98f);
-        const float qU = fminf(fmaxf((r1 + 1 + 0.5f * slack) / nb, 0.02f), 0.99f);
-        pivL = __float_as_uint(fmaxf(-mean_p * __logf(1.f - qL), 0.f));
-        pivU = __float_as_uint(fmaxf(-mean_p * __logf(1.f - qU), 0.f));
-        pivL = min(max(pivL, 1u), 0x7f800000u);
-        pivU = min(max(pivU, 1u), 0x7f800000u);
-    }
-    int cntL = 0, cntU = 0;
-#pragma unroll 1
-    for (int it = 0; it < 120 && !(doneL && doneU); ++it) {
-        int cl = 0, cu = 0;
-#pragma unroll 8
-        for (int i = 0; i < NBL; ++i) {
-            const uint32_t key = K[i * 33 + lane];
-            cl += (key < pivL);
-            cu += (key < pivU);
-        }
-        cl = __reduce_add_sync(kFull, cl);
-        cu = __reduce_add_sync(kFull, cu);
-        if (!doneL) {
-            if (cl > r0) {
-                hiL = pivL;
-                cntHi_L = cl;
-            } else {
-                loL = pivL;
-                cntLo_L = cl;
-                if (cl >= r0 - slack) { doneL = true; cntL = cl; }
-            }
-            if (!doneL) {
-                if (hiL - loL <= 1u) { doneL = true; exactL = true; cntL = cntLo_L; }
-                else pivL = next_pivot(loL, hiL, cntLo_L, cntHi_L, tgtL, it, nbf);
-            }
-        }
-        if (!doneU) {
-            if (cu >= r1 + 1) {
-                hiU = pivU;
-                cntHi_U = cu;
-                if (cu <= r1 + 1 + slack) { doneU = true; cntU = cu; }
-            } else {
-                loU = pivU;
-                cntLo_U = cu;
-            }
-            if (!doneU) {
-                if (hiU - loU <= 1u) { doneU = true; exactU = true; cntU = cntLo_U; }
-                else pivU = next_pivot(loU, hiU, cntLo_U, cntHi_U, tgtU, it, nbf);
-            }
-        }
-    }
-    const uint32_t Lkey = exactL ? loL : pivL;
-    const uint32_t Ukey = exactU ? loU : pivU;
-    const int tL = exactL ? (r0 - cntL) : 0;           // tied bins at Lkey that count as "below"
-    const int tU = exactU ? (r1 + 1 - cntU) : 0;       // tied bins at Ukey that are still in band
-    const int cntL_eff = cntL + tL;
-    const int cntU_eff = cntU + tU;
-    const int nband = cntU_eff - cntL_eff;
-
-    // ---- B + C: below / in-band flags as ballots (bit l of word i <-> bin 32 i + l), running
-    // popcounts, and the in-band powers compacted in bin order -------------------------------
-    {
-        const uint32_t lt = (1u << lane) - 1u;
-        int runL = 0, runU = 0, runB = 0, runI = 0;
-        const bool ties = (tL | tU) != 0;
-#pragma unroll 2
-        for (int i = 0; i < NBL; ++i) {
-            const uint32_t key = K[i * 33 + lane];
-            bool below = key < Lkey, leu = key < Ukey;
-            if (ties) {
-                const uint32_t mL = __ballot_sync(kFull, key == Lkey);
-                const uint32_t mU = __ballot_sync(kFull, key == Ukey);
-                const int trL = runL + __popc(mL & lt), trU = runU + __popc(mU & lt);
-                runL += __popc(mL);
-                runU += __popc(mU);
-                below = below || (key == Lkey && trL < tL);
-                leu = leu || (key == Ukey && trU < tU);
-            }
-            const bool inb = leu && !below;
-            const uint32_t wb = __ballot_sync(kFull, below);
-            const uint32_t wi = __ballot_sync(kFull, inb);
-            if (lane == 0) {
-                belw[i] = wb; inbw[i] = wi;
-                belc[i] = runB; inbc[i] = runI;
-            }
-            if (inb) {
-                const int ib = runI + __popc(wi & lt);
-                if (ib < BS) bandv[ib] = __uint_as_float(key);
-            }
-            runB += __popc(wb);
-            runI += __popc(wi);
-        }
-        if (lane == 0) {
-            belw[NBL] = 0; inbw[NBL] = 0;
-            belc[NBL] = cntL_eff; inbc[NBL] = nband;
-        }
-    }
-    __syncwarp();
-
-    // ---- D: sort the band (ascending) in registers -----------------------------------------
-    {
-        float x[E];
-#pragma unroll
-        for (int r = 0; r < E; ++r) {
-            const int idx = lane * E + r;
-            x[r] = (idx < nband) ? bandv[idx] : __int_as_float(0x7f800000);
-        }
-        bitonic_sort_regs<E>(x, lane);
-#pragma unroll
-        for (int r = 0; r < E; ++r) sortv[lane * E + r] = x[r];
-    }
-    __syncwarp();
-
-    // ---- E: sorted position of every band element (unique; ties ordered by bin) -------------
-    for (int ib = lane; ib < nband; ib += 32) {
-        const float v = bandv[ib];
-        int lo = 0, hi = nband;                 // first index with sortv >= v
-        while (lo < hi) {
-            const int mid = (lo + hi) >> 1;
-            if (sortv[mid] < v) lo = mid + 1; else hi = mid;
-        }
-        int pos = lo;
-        if (lo + 1 < nband && sortv[lo + 1] == v) {      // tied values: earlier bins first
-            for (int q = 0; q < ib; ++q) pos += (bandv[q] == v);
-        }
-        posb[ib] = static_cast<unsigned short>(pos);
-    }
-    __syncwarp();
-
-    // ---- W: forward block maxima M[k] = max P[k .. k + blk - 1], blk = 2^s <= min(2d+1, 32), by
-    // s doubling steps on the register copy (bin k + sh lives sh lanes further, in register i or
-    // i + 1); written over the spectrum, which only the window maxima of eq. 8 still need ------
-    const int d = sp.half_bw;
-    const int wlen = 2 * d + 1;
-    const int s_lvl = min(31 - __clz(wlen), 5);
-    const int blk = 1 << s_lvl;
-    {
-        float mreg[NBL];
-#pragma unroll
-        for (int i = 0; i < NBL; ++i) mreg[i] = preg[i];
-#pragma unroll 1
-        for (int t = 0; t < s_lvl; ++t) {
-            const int sh = 1 << t;
-            const int src = (lane + sh) & 31;
-            const bool wrap = lane + sh >= 32;
-#pragma unroll
-            for (int i = 0; i < NBL; ++i) {
-                const float a = __shfl_sync(kFull, mreg[i], src);
-                const float b = (i + 1 < NBL) ? __shfl_sync(kFull, mreg[i + 1], src) : 0.f;
-                mreg[i] = fmaxf(mreg[i], wrap ? b : a);
-            }
-        }
-#pragma unroll
-        for (int i = 0; i < NBL; ++i) P_s[i * 33 + lane] = mreg[i];
-    }
-    __syncwarp();
-
-    // ---- F: one candidate per lane ------------------------------------------------------------
-    float best = 0.f;
-    int best_c = 0x7fffffff;
-    for (int c0 = 0; c0 < sp.n_f0; c0 += 32) {
-        const int c = c0 + lane;
-        float snr = 0.f, num = 0.f, med = 0.f;
-        bool valid = false;
-        if (c < sp.n_f0) {
-            const CandTable *ct = sp.cand + c;
-            const int mv = ct->m_valid;
-            if (mv > 0) {
-                valid = true;
-                // eq. 8: mean over valid harmonics of the window maximum
-                for (int m = 0; m < mv; ++m) {
-                    const int kc = ct->kc[m];
-                    float mx = 0.f;
-                    for (int off = 0; off < wlen; off += blk)
-                        mx = fmaxf(mx, P_s[pad(min(kc - d + off, kc + d - blk + 1))]);
-                    num += mx;
-                }
-                num = num / static_cast<float>(mv);
-                // eq. 9-10: lower median of the complement
-#pragma unroll
-                for (int w = 0; w < BS / 32; ++w) maskw[w * 32 + lane] = 0u;
-                int e_low = 0;
-                const int ni = ct->n_int;
-                for (int q = 0; q < ni; ++q) {
-                    const int lo = ct->lo[q], hi1 = ct->hi[q] + 1;
-                    const int wl = lo >> 5, wh = hi1 >> 5;
-                    const uint32_t ml = (1u << (lo & 31)) - 1u, mh = (1u << (hi1 & 31)) - 1u;
-                    e_low += static_cast<int>(belc[wh] + __popc(belw[wh] & mh)) -
-                             static_cast<int>(belc[wl] + __popc(belw[wl] & ml));
-                    const int ib0 = inbc[wl] + __popc(inbw[wl] & ml);
-                    const int ib1 = inbc[wh] + __popc(inbw[wh] & mh);
-                    for (int ib = ib0; ib < ib1; ++ib) {
-                        const int pos = posb[ib];
-                        maskw[(pos >> 5) * 32 + lane] |= 1u << (pos & 31);
-                    }
-                }
-                int j = static_cast<int>(ct->rank) - (cntL_eff - e_low);   // rank inside the band's complement
-                j = max(j, 0);
-                int a = nband - 1;
-#pragma unroll 1
-                for (int w = 0; w < BS / 32; ++w) {
-                    uint32_t z = ~maskw[w * 32 + lane];
-                    const int nz = __popc(z);
-                    if (j < nz) {
-                        for (int q = 0; q < j; ++q) z &= z - 1u;            // drop j lowest set bits
-                        a = w * 32 + (__ffs(z) - 1);
-                        break;
-                    }
-                    j -= nz;
-                }
-                a = min(a, max(nband - 1, 0));
-                med = sortv[a];
-                snr = num / fmaxf(med, sp.sf_eps);
-            }
-        }
-        if (dbg != nullptr && c < sp.n_f0) {
-            dbg[c * 3 + 0] = snr;
-            dbg[c * 3 + 1] = num;
-            dbg[c * 3 + 2] = med;
-        }
-        if (valid && (best_c == 0x7fffffff || snr > best)) { best = snr; best_c = c; }
-        __syncwarp();
-    }
-    // eq. 11: max over candidates, first maximum wins
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        const float ob = __shfl_xor_sync(kFull, best, o);
-        const int oc = __shfl_xor_sync(kFull, best_c, o);
-        const bool take = (oc != 0x7fffffff) && (best_c == 0x7fffffff || ob > best || (ob == best && oc < best_c));
-        if (take) { best = ob; best_c = oc; }
-    }
-    score_out = (best_c == 0x7fffffff) ? 0.f : best;
-    f0_out = (best_c == 0x7fffffff) ? -1 : best_c;
-}
-
 // ----------------------------------------------------------------------------------------
 // The fused kernel.
 // ----------------------------------------------------------------------------------------
@@ -492,9 +146,8 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
     constexpr int NBL = L::NBL;
     extern __shared__ __align__(16) uint32_t smem_raw[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    uint32_t *wsm = smem_raw + wid * L::WARP_WORDS;
-    float *P_s = reinterpret_cast<float *>(wsm);
-    uint32_t *scr = wsm + L::P_WORDS;
+    const int cpad = p.sp.cpad;
+    uint32_t *scr = smem_raw + wid * L::warp_words(cpad);
     float2 *btab = reinterpret_cast<float2 *>(scr);                 // [kEC][TN]
     uint4 *phs = reinterpret_cast<uint4 *>(scr + kEC * TN * 2);     // [kEC]
 
@@ -507,7 +160,7 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
     // dynamic work queue with one item of look-ahead: the next work item is loaded while the
     // current pixel is being processed, and its first events are staged in shared memory by
     // cp.async (no register holds data in flight, so nothing waits on a spill)
-    uint32_t *ev_s = scr + L::SCRATCH_WORDS;                        // [2][kEC]
+    uint32_t *ev_s = scr + L::scratch_words(cpad);                  // [2][kEC]
     int evb = 0;                                                    // staging buffer in use
     const bool head = (wid % 3) < DDHF_NDFT_HEAD_WARPS;
     int claim_left = 0;                                             // items of the current claim not yet started
@@ -722,13 +375,23 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
                     r.pix = it.pix; r.arow = has_row ? it.arow : -1; r.mean_p = mean_p; r._pad = 0;
                     p.spill_rec[slot] = r;
                 }
-            } else {
+            } else if (L::INPLACE) {
+                // the queue is full: score here.  comb_score() wants the lane's bins contiguous
+                // (NBL lane + i); they are strided (32 i + lane) in the accumulators: transpose through
+                // the scratch (bin k at k + k / NBL, conflict-free both ways)
+                float *T = reinterpret_cast<float *>(scr);
+                __syncwarp();
 #pragma unroll
-                for (int i = 0; i < NBL; ++i) P_s[i * 33 + lane] = preg[i];        // == pad(32 i + lane)
+                for (int i = 0; i < NBL; ++i) {
+                    const int k = i * 32 + lane;
+                    T[k + k / NBL] = preg[i];
+                }
                 __syncwarp();
                 float *dbg = (p.comb_debug != nullptr && has_row)
                                  ? p.comb_debug + static_cast<size_t>(it.arow) * sp.n_f0 * 3 : nullptr;
-                comb_score<TM, TN, BS>(preg, P_s, scr, sp, mean_p, lane, score, f0, dbg);
+                const float2 r = comb_score_from_smem<NBL, L::INPLACE ? BS : 256>(scr, sp, mean_p, lane, dbg);
+                score = r.x;
+                f0 = __float_as_int(r.y);
                 if (lane == 0) atomicAdd(p.n_scored, 1);
             }
         }
@@ -753,18 +416,15 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
 // ----------------------------------------------------------------------------------------
 constexpr int kScoreWarps = 4;
 
-template <int TM, int TN, int BS>
+template <int NBL, int BS>
 __global__ void __launch_bounds__(kScoreWarps * 32, 4) k_comb_deferred(NdftParams p)
 {
-    using L = Layout<TM, TN, BS>;
-    constexpr int NBL = L::NBL;
-    constexpr int WORDS = ((L::P_WORDS + L::SCORE_WORDS + 3) / 4) * 4;
+    using S = CombSmem<NBL, BS>;
+    constexpr int NB = NBL * 32;
     extern __shared__ __align__(16) uint32_t smem_raw[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    uint32_t *wsm = smem_raw + wid * WORDS;
-    float *P_s = reinterpret_cast<float *>(wsm);
-    uint32_t *scr = wsm + L::P_WORDS;
     const ScoreParams &sp = p.sp;
+    uint32_t *scr = smem_raw + wid * S::words(sp.cpad);
     const int n_rows = min(*p.spill_count, p.spill_cap);
     // rows are handed out one at a time (their cost varies with the band search): spill_count[1]
     // is the consumer cursor, zeroed with the producer count by the ingest stage
@@ -774,18 +434,19 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 4) k_comb_deferred(NdftParam
         row = __shfl_sync(kFull, row, 0);
         if (row >= n_rows) break;
         const SpillRec r = p.spill_rec[row];
-        const float *src = p.spill + static_cast<size_t>(row) * L::NB + lane;
+        // the lane's NBL consecutive bins: NBL / 4 128-bit loads (the row is read exactly once)
+        const float4 *src = reinterpret_cast<const float4 *>(p.spill + static_cast<size_t>(row) * NB + NBL * lane);
         float preg[NBL];
 #pragma unroll
-        for (int i = 0; i < NBL; ++i) preg[i] = __ldcs(src + i * 32);
-#pragma unroll
-        for (int i = 0; i < NBL; ++i) P_s[i * 33 + lane] = preg[i];
-        __syncwarp();
+        for (int i = 0; i < NBL / 4; ++i) {
+            const float4 v = __ldcs(src + i);
+            preg[4 * i] = v.x; preg[4 * i + 1] = v.y; preg[4 * i + 2] = v.z; preg[4 * i + 3] = v.w;
+        }
         float score;
         int f0;
         float *dbg = (p.comb_debug != nullptr && r.arow >= 0)
                          ? p.comb_debug + static_cast<size_t>(r.arow) * sp.n_f0 * 3 : nullptr;
-        comb_score<TM, TN, BS>(preg, P_s, scr, sp, r.mean_p, lane, score, f0, dbg);
+        comb_score<NBL, BS>(preg, scr, sp, r.mean_p, lane, score, f0, dbg);
         if (lane == 0) {
             // the pixel is in the queue because SF <= tau_sf or score_all; the mask needs both
             const bool sf_ok = p.sf[r.pix] <= sp.tau_sf;
@@ -799,29 +460,36 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 4) k_comb_deferred(NdftParam
 }
 
 template <int TM, int TN, int BS, bool FULL>
-int launch_one(const NdftParams &p, int sm_count, cudaStream_t st, cudaEvent_t between)
+int launch_one(const NdftParams &p, int grid_ndft, int grid_score, cudaStream_t st, cudaEvent_t between)
 {
     using L = Layout<TM, TN, BS>;
-    static bool configured = false;
-    static int blocks_per_sm = 1, score_blocks_per_sm = 1;
-    constexpr size_t score_smem = static_cast<size_t>(((L::P_WORDS + L::SCORE_WORDS + 3) / 4) * 4) * 4 * kScoreWarps;
-    if (!configured) {
-        cudaFuncSetAttribute(k_ndft_score<TM, TN, BS, FULL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             static_cast<int>(L::SMEM_BYTES));
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&blocks_per_sm, k_ndft_score<TM, TN, BS, FULL>,
-                                                      kWarps * 32, L::SMEM_BYTES);
-        if (blocks_per_sm < 1) blocks_per_sm = 1;
-        cudaFuncSetAttribute(k_comb_deferred<TM, TN, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             static_cast<int>(score_smem));
-        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&score_blocks_per_sm, k_comb_deferred<TM, TN, BS>,
-                                                      kScoreWarps * 32, score_smem);
-        if (score_blocks_per_sm < 1) score_blocks_per_sm = 1;
-        configured = true;
-    }
-    k_ndft_score<TM, TN, BS, FULL><<<sm_count * blocks_per_sm, kWarps * 32, L::SMEM_BYTES, st>>>(p);
+    const size_t score_smem = static_cast<size_t>(CombSmem<L::NBL, BS>::words(p.sp.cpad)) * 4 * kScoreWarps;
+    k_ndft_score<TM, TN, BS, FULL><<<grid_ndft, kWarps * 32, L::smem_bytes(p.sp.cpad), st>>>(p);
     if (between) cudaEventRecord(between, st);
-    k_comb_deferred<TM, TN, BS><<<sm_count * score_blocks_per_sm, kScoreWarps * 32, score_smem, st>>>(p);
+    k_comb_deferred<L::NBL, BS><<<grid_score, kScoreWarps * 32, score_smem, st>>>(p);
     return 2;
+}
+
+template <int TM, int TN, int BS, bool FULL>
+cudaError_t configure_one(int cpad, int *blocks_per_sm, int *score_blocks_per_sm)
+{
+    using L = Layout<TM, TN, BS>;
+    const size_t smem = L::smem_bytes(cpad);
+    const size_t score_smem = static_cast<size_t>(CombSmem<L::NBL, BS>::words(cpad)) * 4 * kScoreWarps;
+    cudaError_t e = cudaFuncSetAttribute(k_ndft_score<TM, TN, BS, FULL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         static_cast<int>(smem));
+    if (e != cudaSuccess) return e;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, k_ndft_score<TM, TN, BS, FULL>, kWarps * 32, smem);
+    if (e != cudaSuccess) return e;
+    if (*blocks_per_sm < 1) return cudaErrorLaunchOutOfResources;
+    e = cudaFuncSetAttribute(k_comb_deferred<L::NBL, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             static_cast<int>(score_smem));
+    if (e != cudaSuccess) return e;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(score_blocks_per_sm, k_comb_deferred<L::NBL, BS>,
+                                                      kScoreWarps * 32, score_smem);
+    if (e != cudaSuccess) return e;
+    if (*score_blocks_per_sm < 1) return cudaErrorLaunchOutOfResources;
+    return cudaSuccess;
 }
 
 }  // namespace
@@ -844,36 +512,67 @@ int ndft_tn(int n_freq)
 
 int ndft_band_size(int n_freq, int r0, int r1)
 {
+    // sort capacity: the rank band [r0, r1] plus room for the band-limit search to land in (16 ranks on
+    // either side at least); a spectrum that fits the smallest sorter is sorted whole
     const int need = r1 - r0 + 1;
     const int nb = ndft_bins_per_lane(n_freq) * 32;
-    if (need + 16 <= 256 || nb <= 256) return (need <= 256) ? 256 : 0;
-    if (need + 32 <= 512 || nb <= 512) return (need <= 512) ? 512 : 0;
-    if (nb >= 2048 && need <= 1024) return 1024;
+    if (nb <= 256 || need + 32 <= 256) return (need <= 256) ? 256 : 0;
+    if (nb <= 512 || need + 64 <= 512) return (need <= 512) ? 512 : 0;
+    if (nb <= 1024 || need + 128 <= 1024) return (need <= 1024) ? 1024 : 0;
     return 0;
 }
 
+bool ndft_scores_in_place(int n_freq, int band_size) { (void)n_freq; return band_size <= 512; }
+
 namespace {
 
-template <int TM, int TN, int BS>
-int launch_full(const NdftParams &p, bool full, int sm_count, cudaStream_t st, cudaEvent_t between)
+// one dispatch for configure and launch: f.template operator()<TM, TN, BS>()
+template <typename F>
+auto dispatch(int n_freq, int bs, F &&f)
 {
-    return full ? launch_one<TM, TN, BS, true>(p, sm_count, st, between)
-                : launch_one<TM, TN, BS, false>(p, sm_count, st, between);
+    const int nbl = ndft_bins_per_lane(n_freq);
+    if (nbl == 8) return f.template operator()<1, 4, 256>();
+    if (nbl == 16) return bs == 256 ? f.template operator()<1, 8, 256>() : f.template operator()<1, 8, 512>();
+    if (nbl == 32) return bs == 256 ? f.template operator()<1, 16, 256>()
+                        : bs == 512 ? f.template operator()<1, 16, 512>() : f.template operator()<1, 16, 1024>();
+    return bs == 256 ? f.template operator()<2, 16, 256>()
+         : bs == 512 ? f.template operator()<2, 16, 512>() : f.template operator()<2, 16, 1024>();
 }
+
+struct ConfigureFn {
+    int cpad; int *b1, *b2;
+    template <int TM, int TN, int BS> cudaError_t operator()() const
+    {
+        cudaError_t e = configure_one<TM, TN, BS, true>(cpad, b1, b2);
+        if (e != cudaSuccess) return e;
+        int x, y;
+        e = configure_one<TM, TN, BS, false>(cpad, &x, &y);
+        if (e == cudaSuccess) { *b1 = x < *b1 ? x : *b1; *b2 = y < *b2 ? y : *b2; }
+        return e;
+    }
+};
+
+struct LaunchFn {
+    const NdftParams &p; bool full; int g1, g2; cudaStream_t st; cudaEvent_t between;
+    template <int TM, int TN, int BS> int operator()() const
+    {
+        return full ? launch_one<TM, TN, BS, true>(p, g1, g2, st, between)
+                    : launch_one<TM, TN, BS, false>(p, g1, g2, st, between);
+    }
+};
 
 }  // namespace
 
-int launch_ndft(const NdftParams &p, int n_freq, int sm_count, cudaStream_t st, cudaEvent_t between)
+cudaError_t ndft_configure(int n_freq, int band_size, int cpad, int *blocks_per_sm, int *score_blocks_per_sm)
+{
+    return dispatch(n_freq, band_size, ConfigureFn{cpad, blocks_per_sm, score_blocks_per_sm});
+}
+
+int launch_ndft(const NdftParams &p, int n_freq, int band_size, int grid_ndft, int grid_score, cudaStream_t st,
+                cudaEvent_t between)
 {
     const bool full = (n_freq == ndft_bins_per_lane(n_freq) * 32) && (p.sp.k_lo <= 32);
-    const int nbl = ndft_bins_per_lane(n_freq);
-    const int bs = ndft_band_size(n_freq, p.sp.r0, p.sp.r1);
-    if (nbl == 8) return launch_full<1, 4, 256>(p, full, sm_count, st, between);
-    if (nbl == 16) return bs == 256 ? launch_full<1, 8, 256>(p, full, sm_count, st, between) : launch_full<1, 8, 512>(p, full, sm_count, st, between);
-    if (nbl == 32) return bs == 256 ? launch_full<1, 16, 256>(p, full, sm_count, st, between) : launch_full<1, 16, 512>(p, full, sm_count, st, between);
-    if (bs == 256) return launch_full<2, 16, 256>(p, full, sm_count, st, between);
-    if (bs == 512) return launch_full<2, 16, 512>(p, full, sm_count, st, between);
-    return launch_full<2, 16, 1024>(p, full, sm_count, st, between);
+    return dispatch(n_freq, band_size, LaunchFn{p, full, grid_ndft, grid_score, st, between});
 }
 
 }  // namespace ddhf
