@@ -268,15 +268,18 @@ __global__ void __launch_bounds__(1024) k_binscan(IngestParams p)
 // find each other by one ballot per digit bit (MATCH.ANY is far slower on sm_100); the lowest lane
 // of a group writes the group's count.  Kept out of line so that the common conflict-free step
 // does not pay for it.
-__device__ __noinline__ uint32_t rank_by_ballots(bool ok, uint32_t d, uint32_t c, int lane, unsigned short *my_cnt)
+__device__ __noinline__ uint32_t rank_by_ballots(bool ok, uint32_t d, uint32_t c, int lane, unsigned short *my_cnt, int nbits)
 {
     const uint32_t lt = (1u << lane) - 1u;
     uint32_t peers = __ballot_sync(kFullMask, ok);
 #pragma unroll
     for (int k = 0; k < 11; ++k) {
-        const bool bit = (d >> k) & 1u;
-        const uint32_t bal = __ballot_sync(kFullMask, bit);
-        peers &= bit ? bal : ~bal;
+        if (k < nbits) {                                   // warp-uniform: only the digit's own bits are voted on
+            int m;                                         // 0 or -1: bit k of the digit, sign-extended
+            asm("bfe.s32 %0, %1, %2, 1;" : "=r"(m) : "r"(d), "r"(k));
+            const uint32_t bal = __ballot_sync(kFullMask, m != 0);
+            peers &= ~(bal ^ static_cast<uint32_t>(m));    // lanes whose bit k equals mine
+        }
     }
     if (ok && (peers & lt) == 0u) my_cnt[d] = static_cast<unsigned short>(c + __popc(peers));
     __syncwarp();
@@ -365,7 +368,7 @@ __global__ void __launch_bounds__(kTileThreads, DDHF_PART_BLOCKS) k_part(IngestP
         __syncwarp();
         const bool lost = ok && (static_cast<uint32_t>(my_cnt[d]) >> 11) != static_cast<uint32_t>(lane);
         uint32_t rank = c;
-        if (__any_sync(kFullMask, lost)) rank = rank_by_ballots(ok, d, c, lane, my_cnt);
+        if (__any_sync(kFullMask, lost)) rank = rank_by_ballots(ok, d, c, lane, my_cnt, bits);
         key[s] = ok ? (d | (rank << 16)) : 0xffffffffu;
     }
     __syncthreads();
