@@ -22,8 +22,7 @@ struct ddhf_handle {
     int sm_count = 0;
     int n_tiles = 0;
     int launches = 0;
-    int bits1 = 1, bits2 = 1;
-    int chunk_words = 0;
+    int bl = 5, nb = 1, hbits = 1;          // ingest digit split (ingest_plan)
     int spill_cap = 0;
     ScoreParams sp{};
     uint64_t g_f0 = 0, g_d = 0, g_h = 0;
@@ -31,7 +30,7 @@ struct ddhf_handle {
     int band_size = 0;
     int ndft_blocks_per_sm = 1, score_blocks_per_sm = 1;
     // workspace offsets (bytes)
-    size_t off_cnt = 0, off_pairs = 0, off_work = 0, off_tiles = 0, off_class = 0, off_cursor = 0, off_thist = 0, off_chunk = 0, off_binbase = 0, off_spill = 0, off_spillrec = 0,
+    size_t off_cnt = 0, off_items = 0, off_scratch = 0, off_work = 0, off_tiles = 0, off_class = 0, off_cursor = 0, off_runs = 0, off_bkt = 0, off_rows = 0, off_spill = 0, off_spillrec = 0,
            off_parent = 0, off_rec = 0, off_ctiles = 0, ws_bytes = 0;
     cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     bool timed_once = false;
@@ -235,29 +234,25 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
     h->n_tiles = (h->np + kScanTile - 1) / kScanTile;
     size_t o = 0;
     h->off_cnt = o;        o = align_up(o + sizeof(int32_t) * h->np);
-    h->off_pairs = o;      o = align_up(o + sizeof(uint64_t) * static_cast<size_t>(c.max_events));
+    {
+        // tile slots of the bucket-sorted items: 4-byte items in slots of ingest_tile_stride(true), 8-byte in (false)
+        const size_t ev_tiles = (static_cast<size_t>(c.max_events) + ingest_tile_events() - 1) / ingest_tile_events();
+        const size_t a = 4u * ingest_tile_stride(true), b = 8u * ingest_tile_stride(false);
+        h->off_items = o;  o = align_up(o + ev_tiles * (a > b ? a : b));
+    }
+    h->off_scratch = o;    o = align_up(o + sizeof(uint64_t) * static_cast<size_t>(c.max_events));
     h->off_work = o;       o = align_up(o + sizeof(WorkItem) * static_cast<size_t>(h->np));
     h->off_tiles = o;      o = align_up(o + sizeof(int32_t) * 4 * 1024);
     h->off_class = o;      o = align_up(o + sizeof(int32_t) * 2 * kNumClasses);
     h->off_cursor = o;     o = align_up(o + 256);
     {
-        // stable radix partition on the pixel index: two digits of ceil(bits/2) / floor(bits/2) bits
-        int bits = 2;
-        while ((1ll << bits) < np) ++bits;
-        h->bits1 = (bits + 1) / 2;
-        h->bits2 = bits - h->bits1;
-        const size_t bins = static_cast<size_t>(1) << h->bits1;
+        // stable two-level sort on the pixel index (ingest.cu): run table of the tiles, bucket totals and
+        // bases, chunk table of the buckets that need more than one chunk (at most 2 n / capacity + nb rows)
+        ingest_plan(h->np, &h->bl, &h->nb, &h->hbits);
         const size_t ev_tiles = (static_cast<size_t>(c.max_events) + ingest_tile_events() - 1) / ingest_tile_events();
-        const size_t ev_chunks = (ev_tiles + ingest_chunk_tiles() - 1) / ingest_chunk_tiles();
-        if (2 * ev_chunks * bins >= (1ull << 31)) {
-            cudaFree(h->d_tables);
-            delete h;
-            return fail(nullptr, DDHF_E_INVAL, "ddhf_create: max_events too large for this sensor size");
-        }
-        h->chunk_words = static_cast<int>(2 * ev_chunks * bins);
-        h->off_thist = o;   o = align_up(o + sizeof(int32_t) * ev_tiles * bins);
-        h->off_chunk = o;   o = align_up(o + sizeof(int32_t) * static_cast<size_t>(h->chunk_words));
-        h->off_binbase = o; o = align_up(o + sizeof(int32_t) * 3 * bins);
+        h->off_runs = o;    o = align_up(o + sizeof(uint32_t) * ev_tiles * static_cast<size_t>(h->nb));
+        h->off_bkt = o;     o = align_up(o + sizeof(int32_t) * 3 * (static_cast<size_t>(h->nb) + 2));
+        h->off_rows = o;    o = align_up(o + sizeof(int32_t) * (2 * ev_tiles + h->nb + 2) * (4 + (static_cast<size_t>(1) << h->bl)));
     }
     // deferred-scoring queue: spectra of the pixels that pass the SF filter (32 Ki rows at most;
     // pixels beyond the capacity are scored in place by the NDFT kernel)
@@ -306,7 +301,7 @@ extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n
     ip.n_min = c.n_min; ip.max_active = c.max_active;
     ip.cnt = reinterpret_cast<int32_t *>(ws + h->off_cnt);
     ip.row_ptr = out->row_ptr; ip.csr_ev = out->csr_ev;
-    ip.pairs = reinterpret_cast<uint64_t *>(ws + h->off_pairs);
+    ip.items = ws + h->off_items; ip.scratch = ws + h->off_scratch;
     ip.active_idx = out->active_idx;
     ip.work = reinterpret_cast<WorkItem *>(ws + h->off_work);
     int32_t *tiles = reinterpret_cast<int32_t *>(ws + h->off_tiles);
@@ -316,15 +311,14 @@ extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n
     ip.counters = out->counters;
     ip.sf = out->sf; ip.score = out->score; ip.f0_idx = out->f0_idx; ip.mask = out->mask;
     ip.work_cursor = reinterpret_cast<unsigned long long *>(ws + h->off_cursor);
-    ip.bits1 = h->bits1; ip.bits2 = h->bits2;
-    ip.tile_hist = reinterpret_cast<int32_t *>(ws + h->off_thist);
-    ip.chunk1 = reinterpret_cast<int32_t *>(ws + h->off_chunk);
-    ip.chunk2 = ip.chunk1 + h->chunk_words / 2;
-    ip.chunk_words = h->chunk_words;
-    ip.bin_base1 = reinterpret_cast<int32_t *>(ws + h->off_binbase);
-    ip.bin_base2 = ip.bin_base1 + (1 << h->bits1);
-    ip.bin_tot = ip.bin_base2 + (1 << h->bits1);
-    ip.scan_done = reinterpret_cast<int32_t *>(ws + h->off_cursor + 16);     // [2], followed by the spill counter
+    ip.bl = h->bl; ip.vb = 32 - h->bl; ip.nb = h->nb; ip.hbits = h->hbits;
+    ip.compact = (2 * window_us <= (1ll << ip.vb)) ? 1 : 0;               // value = (t - t0) << 1 | polarity
+    ip.run_tab = reinterpret_cast<uint32_t *>(ws + h->off_runs);
+    ip.bkt_total = reinterpret_cast<int32_t *>(ws + h->off_bkt);
+    ip.bkt_base = ip.bkt_total + h->nb + 2;
+    ip.bkt_order = ip.bkt_base + h->nb + 2;
+    ip.chunk_rows = reinterpret_cast<int32_t *>(ws + h->off_rows);
+    ip.sync = reinterpret_cast<int32_t *>(ws + h->off_cursor + 16);       // [8]; the scoring queue counts are sync[2..3]
 
     ip.ccl_parent = cp_parent;
 

@@ -80,14 +80,17 @@ struct IngestParams {
     int32_t *cnt;                // [np] per-pixel histogram
     int32_t *row_ptr;            // [np+1]
     uint32_t *csr_ev;
-    uint64_t *pairs;             // [max_events] (pixel << 32 | csr value) after partition pass 1
-    int32_t bits1, bits2;        // digit widths of the two partition passes (low, high)
-    int32_t *tile_hist;          // [ev_tiles][bins] digit histogram of every 8192-event tile
-    int32_t *chunk1, *chunk2;    // [ev_chunks][bins] per pass; chunk2 follows chunk1 in memory
-    int32_t chunk_words;         // words of chunk1 + chunk2 (zeroed every window)
-    int32_t *bin_base1, *bin_base2;   // [bins]
-    int32_t *bin_tot;            // [bins] scratch of k_binscan
-    int32_t *scan_done;          // [4] CTAs of k_binscan<1>, <2> that have finished; [2], [3]: scoring queue producer / consumer counts
+    // stable two-level sort on pixel = bucket << bl | low (ingest.cu)
+    int32_t bl, vb;              // low-digit bits; value bits of a compact item (32 - bl)
+    int32_t nb, hbits;           // buckets (<= 1023); bits of the tile sort digit (holds nb + 1 values)
+    int32_t compact;             // items of 4 bytes (low << vb | value): 2 * window < 2^vb
+    void *items;                 // [ev_tiles][tile stride] 4- or 8-byte items: every tile sorted by bucket, runs 16-byte aligned
+    void *scratch;               // [max_events] sorted chunks of the buckets that need more than one
+    uint32_t *run_tab;           // [ev_tiles][nb] run of every bucket inside its tile: first item | length << 16
+    int32_t *bkt_order;          // [nb] buckets by descending size class
+    int32_t *bkt_total, *bkt_base;   // [nb + 2] events per bucket; exclusive scan (bkt_base[nb] = n_in)
+    int32_t *chunk_rows;         // [max_rows][4 + 2^bl] chunk table of the multi-chunk buckets
+    int32_t *sync;               // [8] 0: tiles finished, 1: chunk rows handed out, 2-3: scoring queue counts
     int32_t *active_idx;
     WorkItem *work;
     int32_t *tile_sum, *tile_act;   // [n_tiles]
@@ -119,8 +122,10 @@ struct CclParams {
 // of kernels it launched
 int launch_ingest(const IngestParams &p, cudaStream_t st);
 cudaError_t ingest_configure();              // opt in to large dynamic shared memory
-int ingest_tile_events();                    // events per partition tile
-int ingest_chunk_tiles();                    // tiles per scan chunk
+int ingest_tile_events();                    // events per sort tile
+int ingest_tile_stride(bool compact);        // items per tile slot of IngestParams::items (run padding included)
+size_t ingest_tile_smem(int nb);             // dynamic shared memory of k_tile_sort
+void ingest_plan(int np, int *bl, int *nb, int *hbits);   // digit split for a sensor of np pixels
 int launch_ndft(const NdftParams &p, int n_freq, int band_size, int grid_ndft, int grid_score, cudaStream_t st, cudaEvent_t between);
                                              // `between` (optional) is recorded after the NDFT kernel, before the scoring kernel
 int launch_ccl(const CclParams &p, cudaStream_t st);

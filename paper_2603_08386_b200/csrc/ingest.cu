@@ -5,39 +5,40 @@
 // pixels with fewer than n_min events are discarded (L137).  Readings R19 (half-open
 // window, bad coordinates dropped and counted) and R20 (input order inside a row).
 //
-// The bucketing is a two-pass least-significant-digit radix partition on the pixel index
-// (digits of ceil(bits/2) and floor(bits/2) bits, at most 2048 bins), each pass stable, so
-// that events of one pixel keep their input order and csr_ev is bit-reproducible with no
-// atomics deciding any position:
+// The bucketing is a stable two-level sort on the pixel index, pixel = bucket << bL | low,
+// at most 1023 buckets, that reads the 16-byte events exactly once:
 //
-//   pass 1   k_dhist<1>   one CTA per tile of 8192 events: per-pixel histogram (global
-//                         atomics, order-free), per-tile digit histogram M[tile][bin]
-//            k_binscan<1> bin-major exclusive scan of the tile histograms (per 8-tile chunk)
-//            k_part<1>    re-reads the tile, ranks every event inside its (tile, bin) group in
-//                         input order (warp match + per-warp counters + cross-warp scan) and
-//                         writes (value, pixel) pairs at base + rank
-//   pass 2   the same three kernels on the pairs with the high digit; the output is csr_ev.
+//   k_tile_sort    one CTA per tile of 8192 events: decode, filter, and sort the tile by bucket
+//                  in shared memory; the tile goes back to HBM in that order as 4-byte
+//                  (low << vb | value) or 8-byte items, with the start of every bucket's run
+//                  inside the tile (u16 [tile][bucket]).  Bucket totals by integer atomics; the
+//                  last CTA turns them into bucket bases.
+//   k_bucket_sort  one CTA per bucket: gathers the bucket's runs from all tiles in tile order
+//                  (= input order), sorts them by the low digit in shared memory and writes
+//                  csr_ev and the per-pixel counts.  Buckets larger than the CTA's capacity go
+//                  through in chunks (two loops over the chunks: count, then place).
 //
-// HBM traffic per event: 16 B read twice (histogram, partition 1), 8 B written and read twice,
-// 4 B written; the tile histograms add 4 B x bins per 8192 events.
+// Both sorts are least-significant-digit counting sorts of at most 5 bits per sub-pass with
+// THREAD-PRIVATE counters: thread t owns K consecutive items and its own column of the
+// counter matrix [digit][thread], so counting needs no atomics, no ballots and no match
+// instructions, and the rank of an item is a plain exclusive scan of that matrix in
+// (digit, thread) order -- input order inside a digit by construction.  No atomic decides any
+// position, so csr_ev is bit-reproducible (R20).  The ballot-ranking partition this replaces
+// spent 160-185 warp instructions per 32 events and per digit (profiles/r2_ingest_primitives.md);
+// a 5-bit sub-pass here costs about 25.
+//
+// HBM traffic per event: 16 B read, 4 B (8 B when the value does not fit beside the low digit)
+// written and read, 4 B written; the run table adds 2 B x buckets per 8192 events.
 #include "ddhf_internal.cuh"
 
 namespace ddhf {
 
 namespace {
 
-#ifndef DDHF_TILE_THREADS
-#define DDHF_TILE_THREADS 512
-#endif
-constexpr int kTileThreads = DDHF_TILE_THREADS;
-constexpr int kTileWarps = kTileThreads / 32;
-#ifndef DDHF_TILE_EV
-#define DDHF_TILE_EV 16
-#endif
-constexpr int kTileEv = DDHF_TILE_EV;                // events per thread
-constexpr int kTile = kTileThreads * kTileEv;        // 8192 events per tile
-constexpr int kWarpSpan = 32 * kTileEv;              // consecutive events owned by one warp
-constexpr int kChunkTiles = 8;                       // tiles per scan chunk
+constexpr int kNT = 512;                       // threads per CTA of both sort kernels
+constexpr int kTile = 8192;                    // events per tile of k_tile_sort (16 per thread)
+constexpr int kCntStride = kNT + kNT / 32;     // words per counter row (one pad word per 32)
+constexpr int kCntWords = 16 * kCntStride;     // 32 digits, two 16-bit counters per word
 constexpr unsigned kFullMask = 0xffffffffu;
 
 struct Ev {
@@ -69,390 +70,610 @@ __device__ __forceinline__ int size_class(int n)
     return min(kNumClasses - 1, max(0, bl - 3));
 }
 
-// ---- k_init: per-pixel maps for inactive pixels, zeroed histograms and counters ---------
+// ---- k_init: per-pixel maps for inactive pixels, zeroed totals and counters ---------------
 __global__ void k_init(IngestParams p)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < p.np) {
-        p.cnt[i] = 0;
         p.sf[i] = __int_as_float(0x7fc00000);   // NaN: pixel not active
         p.score[i] = 0.f;
         p.f0_idx[i] = -1;
         p.mask[i] = 0;
         p.ccl_parent[i] = 0x7fffffff;           // no parent yet
     }
-    for (int k = i; k < p.chunk_words; k += gridDim.x * blockDim.x) p.chunk1[k] = 0;   // chunk1, chunk2
+    if (i <= p.nb + 1) { p.bkt_total[i] = 0; p.bkt_base[i] = 0; p.bkt_order[i] = i; }   // identity order: no tile ran
     if (blockIdx.x == 0) {
         if (threadIdx.x < DDHF_N_COUNTERS) p.counters[threadIdx.x] = 0;
         if (threadIdx.x < kNumClasses) {
             p.class_cnt[threadIdx.x] = 0;
             p.class_cur[threadIdx.x] = 0;
         }
-        if (threadIdx.x == 0) { *p.work_cursor = 0ull; p.scan_done[0] = 0; p.scan_done[1] = 0; p.scan_done[2] = 0; p.scan_done[3] = 0; }
+        if (threadIdx.x < 8) p.sync[threadIdx.x] = 0;
+        if (threadIdx.x == 0) *p.work_cursor = 0ull;
     }
 }
 
-// ---- k_dhist: digit histogram of one tile; pass 2 also counts[pix] += n (a1) ---------------
-// The per-pixel histogram is taken in pass 2: its input is sorted by the low digit, so a tile
-// holds very few distinct low digits and the counts of (low digit, high digit) = pixel can be
-// pre-aggregated in shared memory; only the non-zero sums go to global memory as atomics.
-constexpr int kLoSpan = 4;     // distinct low digits per tile that are aggregated in shared memory
+// ---- the counting-sort sub-pass --------------------------------------------------------------
+// Shared-memory positions are padded so that both access patterns are conflict-free: "blocked"
+// (thread t reads its K consecutive items) and "striped" (consecutive threads, consecutive items).
+template <typename T> __device__ __forceinline__ int pad_pos(int e);
+template <> __device__ __forceinline__ int pad_pos<uint32_t>(int e) { return e + (e >> 5); }
+template <> __device__ __forceinline__ int pad_pos<uint64_t>(int e) { return e + (e >> 4); }
 
-template <int PASS>
-__global__ void __launch_bounds__(kTileThreads) k_dhist(IngestParams p)
+template <typename T> __device__ __forceinline__ uint32_t digit_of(T it, int shift, uint32_t mask);
+template <> __device__ __forceinline__ uint32_t digit_of<uint32_t>(uint32_t it, int shift, uint32_t mask)
 {
-    extern __shared__ uint32_t s_hist[];            // [bins] (+ [kLoSpan][bins] in pass 2)
-    __shared__ int s_drop;
-    const int bits = (PASS == 1) ? p.bits1 : p.bits2;
-    const int bins = 1 << bits;
-    const int64_t n_src = (PASS == 1) ? p.n : static_cast<int64_t>(p.counters[DDHF_CNT_N_IN]);
-    const int64_t tile_beg = static_cast<int64_t>(blockIdx.x) * kTile;
-    if (tile_beg >= n_src) return;
-    const int words = (PASS == 1) ? bins : (1 + kLoSpan) * bins;
-    for (int b = threadIdx.x; b < words; b += kTileThreads) s_hist[b] = 0;
-    if (threadIdx.x == 0) s_drop = 0;
+    return (it >> shift) & mask;
+}
+template <> __device__ __forceinline__ uint32_t digit_of<uint64_t>(uint64_t it, int shift, uint32_t mask)
+{
+    return (static_cast<uint32_t>(it >> 32) >> (shift - 32)) & mask;      // every digit sits in the high word
+}
+
+// Items it[0..K) of thread t are elements K t .. K t + K - 1 of the current order.  On return
+// buf[pad_pos(r)] holds the element of rank r of the order stably sorted by the digit
+// (it >> shift) & (2^width - 1), 1 <= width <= 5; the caller synchronises before reading buf.
+// cnt: kCntWords words; word (r, t) holds the counters of digits r (low half) and r + R (high half),
+// R = 2^(width-1): a packed add scans both halves at once (totals stay below 2^16).
+// WC = 5: the width is the compile-time constant 5 (the common case); WC = 0: `width` at run time.
+template <int K, typename T, int WC>
+__device__ __forceinline__ void sort_subpass(const T (&it)[K], uint32_t *cnt, T *buf, uint32_t *s_warp,
+                                             int shift, int width_rt)
+{
+    const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
+    const int width = WC ? WC : width_rt;
+    const uint32_t mask = (1u << width) - 1u;
+    const int R = 1 << (width - 1);
+    const uint32_t rmask = static_cast<uint32_t>(R - 1);
+    {
+        uint4 *c4 = reinterpret_cast<uint4 *>(cnt);
+        const int n4 = R * kCntStride / 4;
+        for (int w = t; w < n4; w += kNT) c4[w] = make_uint4(0u, 0u, 0u, 0u);
+    }
     __syncthreads();
-    if (PASS == 1) {
-        int32_t px[kTileEv];
+    // byte offset of the thread's column inside a counter row
+    const uint32_t tb4 = static_cast<uint32_t>(t + (t >> 5)) * 4u;
+    char *cb = reinterpret_cast<char *>(cnt);
 #pragma unroll
-        for (int u = 0; u < kTileEv; ++u) {
-            const int64_t i = tile_beg + u * kTileThreads + threadIdx.x;
-            px[u] = -2;
-            if (i < n_src) px[u] = decode_event(p.events, i, p.t0, p.t1, p.width, p.height).pix;
-        }
-        const uint32_t dmask = static_cast<uint32_t>(bins - 1);
-        int drop = 0;
+    for (int i = 0; i < K; ++i) {
+        const uint32_t d = digit_of<T>(it[i], shift, mask);
+        uint32_t *c = reinterpret_cast<uint32_t *>(cb + (d & rmask) * (kCntStride * 4u) + tb4);
+        *c += ((d >> (width - 1)) * 0xffffu) + 1u;     // +1 in the low or the high half; the thread's own
+    }                                                  // column: no other thread touches it
+    __syncthreads();
+    // exclusive scan of the matrix in (digit, thread) order: thread j rakes words [R j, R j + R)
+    {
+        const int w0 = R * t;
+        uint32_t *cp = cnt + w0 + (w0 >> 5);           // R <= 16: the R words share one pad offset
+        uint32_t run = 0;
 #pragma unroll
-        for (int u = 0; u < kTileEv; ++u) {
-            if (px[u] >= 0) atomicAdd(&s_hist[static_cast<uint32_t>(px[u]) & dmask], 1u);
-            drop += (px[u] == -1);
-        }
-        drop = __reduce_add_sync(kFullMask, drop);
-        if ((threadIdx.x & 31) == 0 && drop) atomicAdd(&s_drop, drop);
-    } else {
-        uint32_t *s_pix = s_hist + bins;            // [kLoSpan][bins]
-        const uint32_t lmask = (1u << p.bits1) - 1u;
-        const uint32_t lo_first = __ldg(reinterpret_cast<const uint32_t *>(p.pairs + tile_beg) + 1) & lmask;
-        uint32_t px[kTileEv];
+        for (int i = 0; i < 16; ++i)
+            if (i < R) run += cp[i];
+        uint32_t inc = run;
 #pragma unroll
-        for (int u = 0; u < kTileEv; ++u) {
-            const int64_t i = tile_beg + u * kTileThreads + threadIdx.x;
-            px[u] = 0xffffffffu;
-            if (i < n_src) px[u] = __ldg(reinterpret_cast<const uint32_t *>(p.pairs + i) + 1);
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t x = __shfl_up_sync(kFullMask, inc, o);
+            if (lane >= o) inc += x;
         }
-#pragma unroll
-        for (int u = 0; u < kTileEv; ++u) {
-            if (px[u] != 0xffffffffu) {
-                const uint32_t hi = px[u] >> p.bits1, dl = (px[u] & lmask) - lo_first;
-                if (dl < static_cast<uint32_t>(kLoSpan)) {
-                    atomicAdd(&s_pix[dl * bins + hi], 1u);
-                } else {
-                    atomicAdd(&s_hist[hi], 1u);
-                    atomicAdd(&p.cnt[px[u]], 1);
-                }
-            }
-        }
+        if (lane == 31) s_warp[wid] = inc;
         __syncthreads();
-        for (int b = threadIdx.x; b < bins; b += kTileThreads) {
-            uint32_t tot = 0;
+        uint32_t ws = (lane < kNT / 32) ? s_warp[lane] : 0u;
 #pragma unroll
-            for (int l = 0; l < kLoSpan; ++l) {
-                const uint32_t c = s_pix[l * bins + b];
-                if (c) atomicAdd(&p.cnt[(static_cast<uint32_t>(b) << p.bits1) | (lo_first + l)], static_cast<int>(c));
-                tot += c;
-            }
-            s_hist[b] += tot;                       // same thread reads it below
+        for (int o = 1; o < kNT / 32; o <<= 1) {
+            const uint32_t x = __shfl_up_sync(kFullMask, ws, o);
+            if (lane >= o) ws += x;
         }
+        const uint32_t grand = __shfl_sync(kFullMask, ws, kNT / 32 - 1);
+        uint32_t wex = __shfl_sync(kFullMask, ws, (wid + 31) & 31);
+        if (wid == 0) wex = 0u;
+        // every high-half digit ranks after all low-half digits
+        uint32_t ex = inc - run + wex + (grand << 16);
+#pragma unroll
+        for (int i = 0; i < 16; ++i)
+            if (i < R) { const uint32_t c = cp[i]; cp[i] = ex; ex += c; }
     }
     __syncthreads();
-    int32_t *row = p.tile_hist + static_cast<size_t>(blockIdx.x) * bins;
-    int32_t *chunk = ((PASS == 1) ? p.chunk1 : p.chunk2) + static_cast<size_t>(blockIdx.x / kChunkTiles) * bins;
-    for (int b = threadIdx.x; b < bins; b += kTileThreads) {
-        const int c = static_cast<int>(s_hist[b]);
-        row[b] = c;
-        if (c) atomicAdd(&chunk[b], c);
+#pragma unroll
+    for (int i = 0; i < K; ++i) {
+        const uint32_t d = digit_of<T>(it[i], shift, mask);
+        const uint32_t hi = d >> (width - 1);
+        uint32_t *c = reinterpret_cast<uint32_t *>(cb + (d & rmask) * (kCntStride * 4u) + tb4);
+        const uint32_t old = *c;
+        *c = old + (hi * 0xffffu) + 1u;
+        const int rank = static_cast<int>((old >> (hi * 16u)) & 0xffffu);
+        buf[pad_pos<T>(rank)] = it[i];
     }
-    if (PASS == 1 && threadIdx.x == 0 && s_drop) atomicAdd(&p.counters[DDHF_CNT_N_DROPPED], s_drop);
 }
 
-// ---- k_binscan: bin-major exclusive scan of the chunk totals ------------------------------
-// chunk[c][b] becomes the number of events of bin b in chunks before c; bin_base[b] the number
-// of events in bins before b.  One CTA per 32 bins; warp g of a CTA owns a contiguous range
-// of chunks, lane l the bin.  The last CTA to finish scans the bin totals.
-// Pass 1 also publishes the number of kept events.
-template <int PASS>
-__global__ void __launch_bounds__(1024) k_binscan(IngestParams p)
+// sub-passes of a `bits`-bit digit: 5 bits each, the remainder last
+__device__ __forceinline__ int subpass_count(int bits) { return (bits + 4) / 5; }
+
+// Sort the K x kNT items of buf (blocked, padded) by the `bits`-bit digit at `shift`; on return
+// it[] holds the thread's K items of the sorted order and buf the whole sorted order.
+template <int K, typename T>
+__device__ __forceinline__ void sort_items(T (&it)[K], uint32_t *cnt, T *buf, uint32_t *s_warp, int shift, int bits)
 {
-    __shared__ int s_grp[32][33];
-    __shared__ int s_w[33];
-    __shared__ bool s_last;
-    const int bits = (PASS == 1) ? p.bits1 : p.bits2;
-    const int bins = 1 << bits;
-    const int64_t n_src = (PASS == 1) ? p.n : static_cast<int64_t>(p.counters[DDHF_CNT_N_IN]);
-    const int n_tiles = static_cast<int>((n_src + kTile - 1) / kTile);
-    const int n_chunks = (n_tiles + kChunkTiles - 1) / kChunkTiles;
-    int32_t *chunk = (PASS == 1) ? p.chunk1 : p.chunk2;
-    int32_t *bin_base = (PASS == 1) ? p.bin_base1 : p.bin_base2;
-    int32_t *bin_tot = p.bin_tot;
-    const int lane = threadIdx.x & 31, g = threadIdx.x >> 5;
-    const int b = blockIdx.x * 32 + lane;
-    const bool live = b < bins;
-    const int per_g = (n_chunks + 31) / 32;
-    const int c_beg = min(g * per_g, n_chunks), c_end = min(c_beg + per_g, n_chunks);
-    int sum = 0;
-    if (live)
-        for (int c = c_beg; c < c_end; ++c) sum += chunk[static_cast<size_t>(c) * bins + b];
-    s_grp[g][lane] = sum;
-    __syncthreads();
-    int pre = 0, tot = 0;
-    for (int q = 0; q < 32; ++q) {
-        const int a = s_grp[q][lane];
-        if (q < g) pre += a;
-        tot += a;
+    const int t = threadIdx.x;
+    int sh = shift, left = bits;
+    while (left > 0) {
+        if (left >= 5) sort_subpass<K, T, 5>(it, cnt, buf, s_warp, sh, 5);
+        else sort_subpass<K, T, 0>(it, cnt, buf, s_warp, sh, left);
+        sh += 5;
+        left -= 5;
+        __syncthreads();
+#pragma unroll
+        for (int i = 0; i < K; ++i) it[i] = buf[pad_pos<T>(K * t + i)];
     }
-    if (live)
-        for (int c = c_beg; c < c_end; ++c) {
-            int32_t *q = chunk + static_cast<size_t>(c) * bins + b;
-            const int v = *q;
-            *q = pre;
-            pre += v;
+}
+
+// ---- block-wide helpers (kNT threads) --------------------------------------------------------------
+// exclusive prefix sum of one value per thread; `total` = sum over the block.  Two barriers.
+__device__ __forceinline__ int block_excl_sum(int v, int &total, uint32_t *s_warp)
+{
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    int inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int x = __shfl_up_sync(kFullMask, inc, o);
+        if (lane >= o) inc += x;
+    }
+    __syncthreads();                                   // earlier readers of s_warp are done
+    if (lane == 31) s_warp[wid] = static_cast<uint32_t>(inc);
+    __syncthreads();
+    int ws = (lane < kNT / 32) ? static_cast<int>(s_warp[lane]) : 0;
+#pragma unroll
+    for (int o = 1; o < kNT / 32; o <<= 1) {
+        const int x = __shfl_up_sync(kFullMask, ws, o);
+        if (lane >= o) ws += x;
+    }
+    total = __shfl_sync(kFullMask, ws, kNT / 32 - 1);
+    int wex = __shfl_sync(kFullMask, ws, (wid + 31) & 31);
+    if (wid == 0) wex = 0;
+    return inc - v + wex;
+}
+
+// r[0 .. n) holds the first position of every digit that occurs and 0xffffffff elsewhere; on return
+// r[d] = first position of the first digit >= d that occurs, `end` if there is none (the start of every
+// digit's run, empty runs included).  Thread t owns PER consecutive entries; n <= PER * kNT.
+template <int PER>
+__device__ __forceinline__ void fill_run_starts(uint32_t *r, int n, uint32_t end, uint32_t *s_warp)
+{
+    const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
+    uint32_t v[PER];
+    uint32_t m = 0xffffffffu;
+#pragma unroll
+    for (int k = 0; k < PER; ++k) {
+        const int i = t * PER + k;
+        v[k] = (i < n) ? r[i] : 0xffffffffu;
+        m = min(m, v[k]);
+    }
+    // suffix minimum over the threads after this one
+    uint32_t suf = m;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t x = __shfl_down_sync(kFullMask, suf, o);
+        if (lane + o < 32) suf = min(suf, x);
+    }
+    __syncthreads();
+    if (lane == 0) s_warp[wid] = suf;                  // minimum of the whole warp
+    __syncthreads();
+    uint32_t carry = end;
+    for (int w = wid + 1; w < kNT / 32; ++w) carry = min(carry, s_warp[w]);
+    const uint32_t nxt = __shfl_down_sync(kFullMask, suf, 1);
+    if (lane < 31) carry = min(carry, nxt);            // threads after this one in the warp
+#pragma unroll
+    for (int k = PER - 1; k >= 0; --k) {
+        const int i = t * PER + k;
+        carry = min(carry, v[k]);
+        if (i < n) r[i] = carry;
+    }
+    __syncthreads();
+}
+
+// ---- the last CTA of k_tile_sort: bucket bases, event counts, bucket order -----------------------------
+// order[] lists the buckets by descending size class (32 classes of the largest total), so that
+// k_bucket_sort, whose CTAs start in index order, takes the expensive buckets first.
+__device__ __forceinline__ void finish_buckets(const IngestParams &p, uint32_t *cnt, uint32_t *buf32, uint32_t *s_warp)
+{
+    const int t = threadIdx.x, lane = t & 31;
+    const uint32_t nb = static_cast<uint32_t>(p.nb);
+    const uint32_t b0 = 2u * t;                                    // nb + 1 <= 1024 = 2 kNT
+    const int v0 = (b0 < nb) ? __ldcg(p.bkt_total + b0) : 0;
+    const int v1 = (b0 + 1 < nb) ? __ldcg(p.bkt_total + b0 + 1) : 0;
+    int grand;
+    const int ex = block_excl_sum(v0 + v1, grand, s_warp);
+    if (b0 <= nb) p.bkt_base[b0] = ex;
+    if (b0 + 1 <= nb) p.bkt_base[b0 + 1] = ex + v0;
+    if (t == 0) {
+        p.counters[DDHF_CNT_N_IN] = grand;
+        p.counters[DDHF_CNT_N_DROPPED] = static_cast<int32_t>(p.n - grand);
+    }
+    int mx = __reduce_max_sync(kFullMask, max(v0, v1));
+    __syncthreads();
+    if (lane == 0) s_warp[t >> 5] = static_cast<uint32_t>(mx);
+    __syncthreads();
+    mx = 0;
+    for (int w = 0; w < kNT / 32; ++w) mx = max(mx, static_cast<int>(s_warp[w]));
+    const int shift = max(0, 27 - __clz(mx | 1));                 // mx >> shift < 32
+    uint32_t it[2];
+    it[0] = ((31u - (static_cast<uint32_t>(v0) >> shift)) << 16) | b0;
+    it[1] = ((31u - (static_cast<uint32_t>(v1) >> shift)) << 16) | (b0 + 1u);
+    __syncthreads();
+    sort_subpass<2, uint32_t, 5>(it, cnt, buf32, s_warp, 16, 5);
+    __syncthreads();
+    for (uint32_t r = t; r < nb; r += kNT) p.bkt_order[r] = static_cast<int32_t>(buf32[pad_pos<uint32_t>(static_cast<int>(r))] & 0xffffu);
+}
+
+// ---- k_tile_sort: decode + filter one tile, sort it by bucket, publish its runs -----------------
+// Item in shared memory: (bucket << 16 | low) << 32 | value; dropped events and the padding of the
+// last tile carry the sentinel bucket nb and sort to the end of the tile.  A tile goes back to HBM
+// with every bucket's run starting on a 16-byte boundary (k_bucket_sort gathers with 128-bit loads);
+// run table entry = first item of the run inside the tile's slot | length << 16.
+template <bool COMPACT> struct TileOut {
+    static constexpr int kAlign = COMPACT ? 4 : 2;                      // items per 16 bytes
+    static constexpr int kStride = kTile + (COMPACT ? 3 : 1) * 1024;     // items per tile slot (padding included)
+};
+
+template <bool FULL>
+__device__ __forceinline__ uint64_t load_item(const IngestParams &p, int64_t idx, uint32_t nb, uint32_t lmask, uint32_t window)
+{
+    uint64_t item = static_cast<uint64_t>(nb) << 48;
+    if (FULL || idx < p.n) {
+        const int4 w = __ldg(reinterpret_cast<const int4 *>(p.events) + idx);
+        const uint32_t x = static_cast<uint32_t>(w.x) & 0xffffu, y = static_cast<uint32_t>(w.x) >> 16;
+        const uint64_t t = (static_cast<uint64_t>(static_cast<uint32_t>(w.w)) << 32) | static_cast<uint32_t>(w.z);
+        const uint64_t dt = t - static_cast<uint64_t>(p.t0);              // window < 2^31: in range iff dt < window
+        const bool ok = (dt < window) && (x < static_cast<uint32_t>(p.width)) && (y < static_cast<uint32_t>(p.height));
+        const uint32_t px = y * static_cast<uint32_t>(p.width) + x;
+        const uint32_t pos = (((static_cast<uint32_t>(w.y) - 1u) & 0xffffu) < 0x7fffu) ? 1u : 0u;   // int16 p > 0
+        const uint32_t hi = ok ? (((px >> p.bl) << 16) | (px & lmask)) : (nb << 16);
+        item = (static_cast<uint64_t>(hi) << 32) | ((static_cast<uint32_t>(dt) << 1) | pos);
+    }
+    return item;
+}
+
+template <bool COMPACT>
+__global__ void __launch_bounds__(kNT, 2) k_tile_sort(IngestParams p)
+{
+    extern __shared__ __align__(16) uint32_t s_raw[];
+    __shared__ uint32_t s_warp[kNT / 32];
+    __shared__ bool s_last;
+    constexpr int K = kTile / kNT;
+    uint64_t *buf = reinterpret_cast<uint64_t *>(s_raw);                       // pad_pos(kTile) items
+    uint32_t *cnt = s_raw + 2 * (kTile + kTile / 16);
+    uint32_t *rstart = cnt + kCntWords;                                          // [1026]
+    const int t = threadIdx.x;
+    const int tile = blockIdx.x;
+    const int64_t tile_beg = static_cast<int64_t>(tile) * kTile;
+    const uint32_t nb = static_cast<uint32_t>(p.nb);
+    const uint32_t lmask = (1u << p.bl) - 1u;
+    const uint32_t window = static_cast<uint32_t>(p.t1 - p.t0);
+
+    // coalesced load, decode; staged in shared memory so that thread t then owns 16 consecutive events
+    if (tile_beg + kTile <= p.n) {
+#pragma unroll 8
+        for (int i = 0; i < K; ++i)
+            buf[pad_pos<uint64_t>(t + kNT * i)] = load_item<true>(p, tile_beg + t + kNT * i, nb, lmask, window);
+    } else {
+#pragma unroll 4
+        for (int i = 0; i < K; ++i)
+            buf[pad_pos<uint64_t>(t + kNT * i)] = load_item<false>(p, tile_beg + t + kNT * i, nb, lmask, window);
+    }
+    for (int b = t; b < 1026; b += kNT) rstart[b] = 0xffffffffu;
+    __syncthreads();
+    uint64_t it[K];
+#pragma unroll
+    for (int i = 0; i < K; ++i) it[i] = buf[pad_pos<uint64_t>(K * t + i)];
+    sort_items<K, uint64_t>(it, cnt, buf, s_warp, 48, p.hbits);
+
+    // start of every bucket's run inside the sorted tile
+    {
+        uint32_t prev = 0xffffffffu;
+        if (t > 0) prev = static_cast<uint32_t>(buf[pad_pos<uint64_t>(K * t - 1)] >> 48);
+#pragma unroll
+        for (int i = 0; i < K; ++i) {
+            const uint32_t d = static_cast<uint32_t>(it[i] >> 48);
+            if (d != prev) rstart[d] = static_cast<uint32_t>(K * t + i);
+            prev = d;
         }
-    if (g == 0 && live) bin_tot[b] = tot;
-    // last CTA: exclusive scan of the bin totals
+    }
+    __syncthreads();
+    fill_run_starts<2>(rstart, static_cast<int>(nb) + 1, kTile, s_warp);        // rstart[0 .. nb]; nb = the sentinel's run
+    // run lengths, aligned starts in the tile's output slot, bucket totals
+    uint32_t *delta = cnt;                                                       // [nb] output position - sorted position
+    {
+        const uint32_t b0 = 2u * t;
+        uint32_t len[2], alen[2];
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+            const uint32_t b = b0 + q;
+            len[q] = (b < nb) ? rstart[b + 1] - rstart[b] : 0u;
+            alen[q] = (len[q] + TileOut<COMPACT>::kAlign - 1) & ~static_cast<uint32_t>(TileOut<COMPACT>::kAlign - 1);
+        }
+        int tot;
+        uint32_t a = static_cast<uint32_t>(block_excl_sum(static_cast<int>(alen[0] + alen[1]), tot, s_warp));
+        uint32_t *row = p.run_tab + static_cast<size_t>(tile) * nb;
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+            const uint32_t b = b0 + q;
+            if (b < nb) {
+                row[b] = a | (len[q] << 16);
+                delta[b] = a - rstart[b];
+                if (len[q]) atomicAdd(&p.bkt_total[b], static_cast<int>(len[q]));
+                a += alen[q];
+            }
+        }
+    }
+    __syncthreads();
+    const int kept = static_cast<int>(rstart[nb]);
+    const size_t out0 = static_cast<size_t>(tile) * TileOut<COMPACT>::kStride;
+#pragma unroll 4
+    for (int i = 0; i < K; ++i) {
+        const int r = t + kNT * i;
+        if (r < kept) {
+            const uint64_t item = buf[pad_pos<uint64_t>(r)];
+            const uint32_t hi = static_cast<uint32_t>(item >> 32), val = static_cast<uint32_t>(item);
+            const size_t at = out0 + static_cast<uint32_t>(r) + delta[hi >> 16];
+            if (COMPACT)
+                reinterpret_cast<uint32_t *>(p.items)[at] = ((hi & 0xffffu) << p.vb) | val;
+            else
+                reinterpret_cast<uint64_t *>(p.items)[at] = (static_cast<uint64_t>(hi & 0xffffu) << 32) | val;
+        }
+    }
+    // the last CTA to finish turns the bucket totals into bases, publishes the event counts and
+    // orders the buckets by descending size class (k_bucket_sort takes them in that order)
     __threadfence();
     __syncthreads();
-    if (threadIdx.x == 0) s_last = (atomicAdd(p.scan_done + (PASS - 1), 1) == static_cast<int>(gridDim.x) - 1);
+    if (t == 0) s_last = (atomicAdd(p.sync + 0, 1) == static_cast<int>(gridDim.x) - 1);
     __syncthreads();
     if (!s_last) return;
     __threadfence();
-    // thread t owns bins 2t and 2t+1 (bins <= 2048)
-    const int b0 = 2 * threadIdx.x;
-    const int run0 = (b0 < bins) ? *reinterpret_cast<volatile int32_t *>(bin_tot + b0) : 0;
-    const int run1 = (b0 + 1 < bins) ? *reinterpret_cast<volatile int32_t *>(bin_tot + b0 + 1) : 0;
-    const int wid = g;
-    const int mine = run0 + run1;
-    int inc = mine;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const int t = __shfl_up_sync(kFullMask, inc, o);
-        if (lane >= o) inc += t;
-    }
-    if (lane == 31) s_w[wid] = inc;
-    __syncthreads();
-    if (wid == 0) {
-        const int w = s_w[lane];
-        int x = w;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int t = __shfl_up_sync(kFullMask, x, o);
-            if (lane >= o) x += t;
-        }
-        s_w[lane] = x - w;
-        if (lane == 31) s_w[32] = x;
-    }
-    __syncthreads();
-    const int excl = inc - mine + s_w[wid];
-    if (b0 < bins) bin_base[b0] = excl;
-    if (b0 + 1 < bins) bin_base[b0 + 1] = excl + run0;
-    if (PASS == 1 && threadIdx.x == 0) p.counters[DDHF_CNT_N_IN] = s_w[32];
+    finish_buckets(p, cnt, reinterpret_cast<uint32_t *>(buf), s_warp);
 }
 
-// ---- k_part: stable partition of one tile by the pass's digit ----------------------------
-// Warp w of the CTA owns the tile's events [512 w, 512 w + 512) and walks them in 16 steps of
-// 32 consecutive events.  Inside a step, lanes with the same digit find each other with
-// a ballot per digit bit; the lowest lane of a group advances the warp's counter of that digit, so an
-// event's rank inside (tile, digit) follows input order exactly.  The tile is then laid out in
-// shared memory in output order (bin-major) and written with consecutive threads on
-// consecutive elements, so that every run of a bin is a coalesced store.
-// Slow path of the ranking step (two lanes of the warp share a digit): lanes with the same digit
-// find each other by one ballot per digit bit (MATCH.ANY is far slower on sm_100); the lowest lane
-// of a group writes the group's count.  Kept out of line so that the common conflict-free step
-// does not pay for it.
-__device__ __noinline__ uint32_t rank_by_ballots(bool ok, uint32_t d, uint32_t c, int lane, unsigned short *my_cnt, int nbits)
-{
-    const uint32_t lt = (1u << lane) - 1u;
-    uint32_t peers = __ballot_sync(kFullMask, ok);
-#pragma unroll
-    for (int k = 0; k < 11; ++k) {
-        if (k < nbits) {                                   // warp-uniform: only the digit's own bits are voted on
-            int m;                                         // 0 or -1: bit k of the digit, sign-extended
-            asm("bfe.s32 %0, %1, %2, 1;" : "=r"(m) : "r"(d), "r"(k));
-            const uint32_t bal = __ballot_sync(kFullMask, m != 0);
-            peers &= ~(bal ^ static_cast<uint32_t>(m));    // lanes whose bit k equals mine
-        }
-    }
-    if (ok && (peers & lt) == 0u) my_cnt[d] = static_cast<unsigned short>(c + __popc(peers));
-    __syncwarp();
-    return c + __popc(peers & lt);
-}
+// ---- k_bucket_sort: gather one bucket from all tiles, sort it by the low digit, write the rows -------
+// Items: COMPACT  uint32  low << vb | value   (value < 2^vb, vb = 32 - bL)
+//        else     uint64  low << 32 | value
+// The padding of a partly filled chunk is all ones: it sorts behind every real item in every sub-pass
+// (it also comes last in input order), so positions [0, fill) of the sorted chunk are the real items.
+template <bool COMPACT> struct BucketItem { typedef uint32_t type; };
+template <> struct BucketItem<false> { typedef uint64_t type; };
 
-template <int PASS>
-struct PartSmem {
-    // words: base[bins] | binoff[bins] | wcnt[kTileWarps][bins] (u16) | stage
-    static constexpr int kStageWords = (PASS == 1) ? 2 * kTile : kTile + kTile / 2;
-    static size_t bytes(int bins) { return static_cast<size_t>(bins) * (8 + 2 * kTileWarps) + 4u * kStageWords; }
+template <bool COMPACT>
+struct BucketCfg {
+    typedef typename BucketItem<COMPACT>::type T;
+    static constexpr int kMaxK = COMPACT ? 32 : 16;
+    static constexpr int kCap = kMaxK * kNT;                       // items per chunk
+    static constexpr int kBufWords = COMPACT ? (kCap + kCap / 32) : 2 * (kCap + kCap / 16);
+    // words: buf | cnt | rstart [2^bL + 1] | pixtot [2^bL]
+    static size_t smem_bytes(int bl) { return 4u * (static_cast<size_t>(kBufWords) + kCntWords + 2u * (1u << bl) + 8u); }
+    __device__ static __forceinline__ uint32_t low_of(T it, int vb)
+    {
+        if (COMPACT) return static_cast<uint32_t>(it) >> vb;
+        return static_cast<uint32_t>(static_cast<uint64_t>(it) >> 32);
+    }
+    __device__ static __forceinline__ uint32_t val_of(T it, int vb)
+    {
+        if (COMPACT) return static_cast<uint32_t>(it) & ((1u << vb) - 1u);
+        return static_cast<uint32_t>(it);
+    }
 };
 
-#ifndef DDHF_PART_BLOCKS
-#define DDHF_PART_BLOCKS (kTileThreads >= 512 ? 2 : 4)
-#endif
-template <int PASS>
-__global__ void __launch_bounds__(kTileThreads, DDHF_PART_BLOCKS) k_part(IngestParams p)
+// Sort the first `fill` items of buf (input order, padded positions) by the low digit; returns with
+// rstart[l] = first sorted position of pixel l of the bucket (l = 0 .. 2^bL, rstart[2^bL] = fill) and
+// buf = the sorted chunk.
+template <int K, bool COMPACT>
+__device__ __noinline__ void sort_chunk(typename BucketItem<COMPACT>::type *buf, uint32_t *cnt, uint32_t *rstart,
+                                        uint32_t *s_warp, int fill, int bl, int vb)
 {
-    extern __shared__ uint32_t s_raw[];
-    __shared__ int s_ntile;
-    const int bits = (PASS == 1) ? p.bits1 : p.bits2;
-    const int bins = 1 << bits;
-    int32_t *s_base = reinterpret_cast<int32_t *>(s_raw);                              // [bins] global base - tile offset
-    uint32_t *s_binoff = s_raw + bins;                                                 // [bins] tile-local offset of the bin
-    unsigned short *s_wcnt = reinterpret_cast<unsigned short *>(s_raw + 2 * bins);     // [kTileWarps][bins]
-    uint32_t *s_stage = s_raw + 2 * bins + kTileWarps * bins / 2;
-    const int64_t n_src = (PASS == 1) ? p.n : static_cast<int64_t>(p.counters[DDHF_CNT_N_IN]);
-    const int tile = blockIdx.x;
-    const int64_t tile_beg = static_cast<int64_t>(tile) * kTile;
-    if (tile_beg >= n_src) return;
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-
-    for (int k = threadIdx.x; k < kTileWarps * bins / 2; k += kTileThreads)
-        reinterpret_cast<uint32_t *>(s_wcnt)[k] = 0u;
-    // global position of the first event of every bin of this tile
-    {
-        const int32_t *chunk = ((PASS == 1) ? p.chunk1 : p.chunk2) + static_cast<size_t>(tile / kChunkTiles) * bins;
-        const int32_t *bin_base = (PASS == 1) ? p.bin_base1 : p.bin_base2;
-        const int32_t *rows = p.tile_hist + static_cast<size_t>(tile / kChunkTiles) * kChunkTiles * bins;
-        const int n_before = tile % kChunkTiles;
-        for (int b = threadIdx.x; b < bins; b += kTileThreads) {
-            int acc = bin_base[b] + chunk[b];
+    typedef typename BucketItem<COMPACT>::type T;
+    const int t = threadIdx.x;
+    const int nl = 1 << bl;
+    for (int l = t; l <= nl; l += kNT) rstart[l] = 0xffffffffu;
+    T it[K];
 #pragma unroll
-            for (int t = 0; t < kChunkTiles - 1; ++t)
-                if (t < n_before) acc += rows[static_cast<size_t>(t) * bins + b];
-            s_base[b] = acc;
-        }
+    for (int i = 0; i < K; ++i) {
+        const int e = K * t + i;
+        it[i] = (e < fill) ? buf[pad_pos<T>(e)] : static_cast<T>(~static_cast<T>(0));
     }
-    uint32_t val[kTileEv], pix[kTileEv];
-    const int64_t warp_beg = tile_beg + wid * kWarpSpan + lane;
+    sort_items<K, T>(it, cnt, buf, s_warp, COMPACT ? vb : 32, bl);
+    uint32_t prev = 0xffffffffu;
+    if (t > 0) prev = BucketCfg<COMPACT>::low_of(buf[pad_pos<T>(K * t - 1)], vb);
 #pragma unroll
-    for (int s = 0; s < kTileEv; ++s) {
-        const int64_t i = warp_beg + s * 32;
-        pix[s] = 0xffffffffu;
-        val[s] = 0u;
-        if (i < n_src) {
-            if (PASS == 1) {
-                const Ev e = decode_event(p.events, i, p.t0, p.t1, p.width, p.height);
-                pix[s] = static_cast<uint32_t>(e.pix);          // -1 -> 0xffffffff
-                val[s] = e.val;
-            } else {
-                const uint2 q = __ldg(reinterpret_cast<const uint2 *>(p.pairs) + i);
-                val[s] = q.x;
-                pix[s] = q.y;
+    for (int i = 0; i < K; ++i) {
+        const uint32_t d = BucketCfg<COMPACT>::low_of(it[i], vb);
+        if (K * t + i < fill && d != prev) rstart[d] = static_cast<uint32_t>(K * t + i);
+        prev = d;
+    }
+    __syncthreads();
+    if (nl <= kNT) fill_run_starts<1>(rstart, nl, static_cast<uint32_t>(fill), s_warp);
+    else if (nl <= 2 * kNT) fill_run_starts<2>(rstart, nl, static_cast<uint32_t>(fill), s_warp);
+    else fill_run_starts<8>(rstart, nl, static_cast<uint32_t>(fill), s_warp);
+    if (t == 0) rstart[nl] = static_cast<uint32_t>(fill);
+    __syncthreads();
+}
+
+template <bool COMPACT>
+__device__ __forceinline__ void sort_chunk_any(typename BucketItem<COMPACT>::type *buf, uint32_t *cnt, uint32_t *rstart,
+                                               uint32_t *s_warp, int fill, int bl, int vb)
+{
+    if (fill <= 8 * kNT) sort_chunk<8, COMPACT>(buf, cnt, rstart, s_warp, fill, bl, vb);
+    else if (!COMPACT || fill <= 16 * kNT) sort_chunk<16, COMPACT>(buf, cnt, rstart, s_warp, fill, bl, vb);
+    else if (fill <= 24 * kNT) sort_chunk<COMPACT ? 24 : 16, COMPACT>(buf, cnt, rstart, s_warp, fill, bl, vb);
+    else sort_chunk<BucketCfg<COMPACT>::kMaxK, COMPACT>(buf, cnt, rstart, s_warp, fill, bl, vb);
+}
+
+// One row of the chunk table of a bucket that does not fit one chunk: header {previous row of the
+// bucket (-1: none), offset of the chunk inside the bucket, items, 0} followed by 2^bL per-pixel words
+// delta[l] = (events of pixel l in earlier chunks) - (first sorted position of pixel l in this chunk).
+constexpr int kRowHdr = 4;
+
+template <bool COMPACT>
+__global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
+{
+    typedef BucketCfg<COMPACT> C;
+    typedef typename C::T T;
+    extern __shared__ __align__(16) uint32_t s_raw[];
+    __shared__ uint32_t s_warp[kNT / 32];
+    __shared__ int s_cut, s_row;
+    T *buf = reinterpret_cast<T *>(s_raw);
+    uint32_t *cnt = s_raw + C::kBufWords;
+    uint32_t *rstart = cnt + kCntWords;                       // [nl + 1]
+    const int bl = p.bl, vb = p.vb, nl = 1 << bl;
+    uint32_t *pixtot = rstart + nl + 4;                        // [nl]
+    const int t = threadIdx.x;
+    const int b = p.bkt_order[blockIdx.x];                     // largest buckets first
+    const int m = p.bkt_total[b];
+    const int gbase = p.bkt_base[b];
+    const int pix0 = b << bl;
+    if (m == 0) {
+        for (int l = t; l < nl; l += kNT)
+            if (pix0 + l < p.np) p.cnt[pix0 + l] = 0;
+        return;
+    }
+    const bool single = m <= C::kCap;
+    if (!single)
+        for (int l = t; l < nl; l += kNT) pixtot[l] = 0u;
+    const int n_tiles = static_cast<int>((p.n + kTile - 1) / kTile);
+    const uint4 *items = reinterpret_cast<const uint4 *>(p.items);         // runs start on 16-byte boundaries
+    constexpr int kPer16 = TileOut<COMPACT>::kAlign;                        // items per 128-bit load
+    T *scratch = reinterpret_cast<T *>(p.scratch);
+    const int row_words = kRowHdr + nl;
+    int fill = 0;            // items gathered for the chunk being formed
+    int chunk_off = 0;       // offset of that chunk inside the bucket
+    int last_row = -1;
+
+    // Emit the chunk in buf[0, fill): the only chunk of the bucket -> csr_ev and counts; else loop 1.
+    auto flush = [&]() {
+        __syncthreads();
+        sort_chunk_any<COMPACT>(buf, cnt, rstart, s_warp, fill, bl, vb);
+        if (single) {
+            for (int l = t; l < nl; l += kNT)
+                if (pix0 + l < p.np) p.cnt[pix0 + l] = static_cast<int32_t>(rstart[l + 1] - rstart[l]);
+            for (int r = t; r < fill; r += kNT) p.csr_ev[gbase + r] = C::val_of(buf[pad_pos<T>(r)], vb);
+        } else {
+            if (t == 0) s_row = atomicAdd(p.sync + 1, 1);
+            __syncthreads();
+            const int row = s_row;
+            int32_t *rw = p.chunk_rows + static_cast<size_t>(row) * row_words;
+            if (t == 0) { rw[0] = last_row; rw[1] = chunk_off; rw[2] = fill; rw[3] = 0; }
+            for (int l = t; l < nl; l += kNT) {
+                const uint32_t before = pixtot[l];
+                rw[kRowHdr + l] = static_cast<int32_t>(before) - static_cast<int32_t>(rstart[l]);
+                pixtot[l] = before + (rstart[l + 1] - rstart[l]);
+            }
+            for (int r = t; r < fill; r += kNT) scratch[static_cast<size_t>(gbase) + chunk_off + r] = buf[pad_pos<T>(r)];
+            last_row = row;
+        }
+        __syncthreads();
+        chunk_off += fill;
+        fill = 0;
+    };
+
+    // runs of this bucket, 2 kNT tiles at a time, in tile order = input order
+    for (int tb = 0; tb < n_tiles; tb += 2 * kNT) {
+        int src[2], len[2];
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+            const int j = tb + 2 * t + q;
+            src[q] = 0; len[q] = 0;
+            if (j < n_tiles) {
+                const uint32_t e = __ldg(p.run_tab + static_cast<size_t>(j) * p.nb + b);
+                src[q] = static_cast<int>(e & 0xffffu); len[q] = static_cast<int>(e >> 16);
             }
         }
-    }
-    __syncthreads();
-
-    // rank inside (warp, digit) in input order
-    unsigned short *my_cnt = s_wcnt + wid * bins;
-    const uint32_t dmask = static_cast<uint32_t>(bins - 1);
-    const uint32_t lt = (1u << lane) - 1u;
-    uint32_t key[kTileEv];                    // digit | rank << 16
+        int total;
+        int off[2];
+        off[0] = block_excl_sum(len[0] + len[1], total, s_warp);
+        off[1] = off[0] + len[0];
+        int base_off = 0;                                  // runs before this offset are already emitted
+        while (true) {
+            // cut: the first run that does not fit the chunk any more
+            const int room = C::kCap - fill;
+            int cut = total;
+            if (total - base_off > room) {
+                __syncthreads();
+                if (t == 0) s_cut = total;
+                __syncthreads();
+                int cand = total;
 #pragma unroll
-    for (int s = 0; s < kTileEv; ++s) {
-        const bool ok = pix[s] != 0xffffffffu;
-        const uint32_t d = (PASS == 1) ? (pix[s] & dmask) : ((pix[s] >> p.bits1) & dmask);
-        // Optimistic step: every lane bumps its digit's counter and tags it with its lane id
-        // (counts are <= 512, the tag sits above bit 11).  If every lane reads its own tag back,
-        // no two lanes shared a digit and the ranks are simply the old counts.
-        const uint32_t c = ok ? (my_cnt[d] & 0x7ffu) : 0u;
-        __syncwarp();
-        if (ok) my_cnt[d] = static_cast<unsigned short>((c + 1u) | (static_cast<uint32_t>(lane) << 11));
-        __syncwarp();
-        const bool lost = ok && (static_cast<uint32_t>(my_cnt[d]) >> 11) != static_cast<uint32_t>(lane);
-        uint32_t rank = c;
-        if (__any_sync(kFullMask, lost)) rank = rank_by_ballots(ok, d, c, lane, my_cnt, bits);
-        key[s] = ok ? (d | (rank << 16)) : 0xffffffffu;
+                for (int q = 1; q >= 0; --q)
+                    if (len[q] > 0 && off[q] >= base_off && off[q] + len[q] - base_off > room) cand = off[q];
+                if (cand < total) atomicMin(&s_cut, cand);
+                __syncthreads();
+                cut = s_cut;
+            }
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+                if (len[q] > 0 && off[q] >= base_off && off[q] < cut) {
+                    const int j = tb + 2 * t + q;
+                    const uint4 *s = items + (static_cast<size_t>(j) * TileOut<COMPACT>::kStride + src[q]) / kPer16;
+                    const int dst = fill + off[q] - base_off;
+                    for (int i = 0; i < len[q]; i += 2 * kPer16) {     // two independent 128-bit loads per round
+                        const uint4 v0 = __ldg(s + i / kPer16);
+                        uint4 v1 = make_uint4(0u, 0u, 0u, 0u);
+                        if (i + kPer16 < len[q]) v1 = __ldg(s + i / kPer16 + 1);
+                        if (COMPACT) {
+                            const uint32_t w[8] = {v0.x, v0.y, v0.z, v0.w, v1.x, v1.y, v1.z, v1.w};
+#pragma unroll
+                            for (int u = 0; u < 8; ++u)
+                                if (i + u < len[q]) buf[pad_pos<T>(dst + i + u)] = static_cast<T>(w[u]);
+                        } else {
+                            const uint64_t w[4] = {(static_cast<uint64_t>(v0.y) << 32) | v0.x, (static_cast<uint64_t>(v0.w) << 32) | v0.z,
+                                                   (static_cast<uint64_t>(v1.y) << 32) | v1.x, (static_cast<uint64_t>(v1.w) << 32) | v1.z};
+#pragma unroll
+                            for (int u = 0; u < 4; ++u)
+                                if (i + u < len[q]) buf[pad_pos<T>(dst + i + u)] = static_cast<T>(w[u]);
+                        }
+                    }
+                }
+            }
+            fill += cut - base_off;
+            if (cut == total) break;
+            flush();
+            base_off = cut;
+        }
     }
-    __syncthreads();
-    // per bin: exclusive scan of the per-warp counters over the warps, then of the bin totals
-    // over the bins (thread t owns `per` consecutive bins)
+    flush();
+    if (single) return;
+
+    // loop 2: row starts of the bucket's pixels, then every chunk goes to its place
     {
-        __shared__ uint32_t s_ws[kTileWarps + 1];
-        const int per = (bins + kTileThreads - 1) / kTileThreads;
-        const int bb = threadIdx.x * per;
-        uint32_t tot[8];                                       // per <= 8 (bins <= 2048, >= 256 threads)
+        const int per = (nl + kNT - 1) / kNT;                // <= 8 (bL <= 12)
+        uint32_t v[8];
         uint32_t sum = 0;
 #pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            tot[j] = 0;
-            const int b = bb + j;
-            if (j < per && b < bins) {
-                uint32_t run = 0;
-#pragma unroll
-                for (int w = 0; w < kTileWarps; ++w) {
-                    const uint32_t t = s_wcnt[w * bins + b] & 0x7ffu;
-                    s_wcnt[w * bins + b] = static_cast<unsigned short>(run);
-                    run += t;
-                }
-                tot[j] = run;
-                sum += run;
-            }
+        for (int k = 0; k < 8; ++k) {
+            const int l = t * per + k;
+            v[k] = (k < per && l < nl) ? pixtot[l] : 0u;
+            sum += v[k];
         }
-        uint32_t inc = sum;
+        int tot;
+        uint32_t ex = static_cast<uint32_t>(block_excl_sum(static_cast<int>(sum), tot, s_warp));
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t t = __shfl_up_sync(kFullMask, inc, o);
-            if (lane >= o) inc += t;
-        }
-        if (lane == 31) s_ws[wid] = inc;
-        __syncthreads();
-        if (wid == 0) {
-            const uint32_t w = (lane < kTileWarps) ? s_ws[lane] : 0u;
-            uint32_t x = w;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const uint32_t t = __shfl_up_sync(kFullMask, x, o);
-                if (lane >= o) x += t;
+        for (int k = 0; k < 8; ++k) {
+            const int l = t * per + k;
+            if (k < per && l < nl) {
+                if (pix0 + l < p.np) p.cnt[pix0 + l] = static_cast<int32_t>(v[k]);
+                rstart[l] = ex;                              // row start of pixel l inside the bucket
+                ex += v[k];
             }
-            if (lane < kTileWarps) s_ws[lane] = x - w;
         }
         __syncthreads();
-        uint32_t off = inc - sum + s_ws[wid];
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {
-            const int b = bb + j;
-            if (j < per && b < bins) {
-                s_binoff[b] = off;
-                s_base[b] -= static_cast<int32_t>(off);
-                off += tot[j];
-            }
-        }
-        if (bb < bins && bb + per >= bins) s_ntile = static_cast<int>(off);
     }
-    __syncthreads();
-    // lay the tile out in output order
-    unsigned short *s_sbin = reinterpret_cast<unsigned short *>(s_stage + kTile);      // pass 2: bin of every staged element
-#pragma unroll
-    for (int s = 0; s < kTileEv; ++s) {
-        if (key[s] != 0xffffffffu) {
-            const uint32_t d = key[s] & 0xffffu;
-            const uint32_t at = s_binoff[d] + my_cnt[d] + (key[s] >> 16);
-            if (PASS == 1) {
-                reinterpret_cast<uint2 *>(s_stage)[at] = make_uint2(val[s], pix[s]);
-            } else {
-                s_stage[at] = val[s];
-                s_sbin[at] = static_cast<unsigned short>(d);
-            }
+    int32_t *delta = reinterpret_cast<int32_t *>(pixtot);    // the chunk's delta row, staged
+    for (int row = last_row; row >= 0;) {
+        const int32_t *rw = p.chunk_rows + static_cast<size_t>(row) * row_words;
+        const int prev_row = rw[0], coff = rw[1], cfill = rw[2];
+        __syncthreads();
+        for (int l = t; l < nl; l += kNT) delta[l] = rw[kRowHdr + l] + static_cast<int32_t>(rstart[l]);
+        __syncthreads();
+        for (int r = t; r < cfill; r += kNT) {
+            const T item = scratch[static_cast<size_t>(gbase) + coff + r];
+            const uint32_t l = C::low_of(item, vb);
+            p.csr_ev[gbase + delta[l] + r] = C::val_of(item, vb);
         }
-    }
-    __syncthreads();
-    const int n_tile = s_ntile;                                                          // kept events of this tile
-    for (int i = threadIdx.x; i < n_tile; i += kTileThreads) {
-        if (PASS == 1) {
-            const uint2 q = reinterpret_cast<const uint2 *>(s_stage)[i];
-            const uint32_t d = q.y & dmask;
-            p.pairs[s_base[d] + i] = (static_cast<uint64_t>(q.y) << 32) | q.x;
-        } else {
-            p.csr_ev[s_base[s_sbin[i]] + i] = s_stage[i];
-        }
+        row = prev_row;
     }
 }
 
@@ -611,36 +832,61 @@ __global__ void __launch_bounds__(1024) k_scan_apply(IngestParams p)
 }
 
 
+
 }  // namespace
+
+namespace {
+template <bool COMPACT>
+cudaError_t configure_sort_kernels()
+{
+    cudaError_t e = cudaFuncSetAttribute(k_tile_sort<COMPACT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         static_cast<int>(ingest_tile_smem(1023)));
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(k_bucket_sort<COMPACT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                static_cast<int>(BucketCfg<COMPACT>::smem_bytes(12)));
+}
+}  // namespace
+
+size_t ingest_tile_smem(int nb) { (void)nb; return 4u * (2u * (kTile + kTile / 16) + kCntWords + 1032u); }
 
 cudaError_t ingest_configure()
 {
-    // sized for the largest digit (2048 bins)
-    cudaError_t e = cudaFuncSetAttribute(k_part<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         static_cast<int>(PartSmem<1>::bytes(2048)));
+    const cudaError_t e = configure_sort_kernels<true>();
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(k_part<2>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                static_cast<int>(PartSmem<2>::bytes(2048)));
+    return configure_sort_kernels<false>();
 }
 
 int ingest_tile_events() { return kTile; }
-int ingest_chunk_tiles() { return kChunkTiles; }
+int ingest_tile_stride(bool compact) { return compact ? TileOut<true>::kStride : TileOut<false>::kStride; }
+
+void ingest_plan(int np, int *bl, int *nb, int *hbits)
+{
+    // pixel = bucket << bL | low with at most 1023 buckets (the sort digit of a tile also holds the
+    // sentinel bucket of dropped events); small sensors keep 32 pixels per bucket
+    int bits = 1;
+    while ((1ll << bits) < np) ++bits;
+    int l = bits > 15 ? bits - 10 : 5;
+    while (((np + (1 << l) - 1) >> l) > 1023) ++l;
+    *bl = l;
+    *nb = (np + (1 << l) - 1) >> l;
+    int hb = 1;
+    while ((1 << hb) < *nb + 1) ++hb;
+    *hbits = hb;
+}
 
 int launch_ingest(const IngestParams &p, cudaStream_t st)
 {
     const int n_tiles = (p.np + kScanTile - 1) / kScanTile;
     const int ev_tiles = static_cast<int>((p.n + kTile - 1) / kTile);
-    const int bins1 = 1 << p.bits1, bins2 = 1 << p.bits2;
-    const size_t part1_smem = PartSmem<1>::bytes(bins1), part2_smem = PartSmem<2>::bytes(bins2);
     int launches = 0;
-    k_init<<<(p.np + 255) / 256, 256, 0, st>>>(p); ++launches;
-    if (ev_tiles > 0) {
-        k_dhist<1><<<ev_tiles, kTileThreads, bins1 * 4, st>>>(p); ++launches;
-        k_binscan<1><<<(bins1 + 31) / 32, 1024, 0, st>>>(p); ++launches;
-        k_part<1><<<ev_tiles, kTileThreads, part1_smem, st>>>(p); ++launches;
-        k_dhist<2><<<ev_tiles, kTileThreads, (1 + kLoSpan) * bins2 * 4, st>>>(p); ++launches;
-        k_binscan<2><<<(bins2 + 31) / 32, 1024, 0, st>>>(p); ++launches;
-        k_part<2><<<ev_tiles, kTileThreads, part2_smem, st>>>(p); ++launches;
+    const int init_items = p.np > p.nb + 2 ? p.np : p.nb + 2;
+    k_init<<<(init_items + 255) / 256, 256, 0, st>>>(p); ++launches;
+    if (p.compact) {
+        if (ev_tiles > 0) { k_tile_sort<true><<<ev_tiles, kNT, ingest_tile_smem(p.nb), st>>>(p); ++launches; }
+        k_bucket_sort<true><<<p.nb, kNT, BucketCfg<true>::smem_bytes(p.bl), st>>>(p); ++launches;
+    } else {
+        if (ev_tiles > 0) { k_tile_sort<false><<<ev_tiles, kNT, ingest_tile_smem(p.nb), st>>>(p); ++launches; }
+        k_bucket_sort<false><<<p.nb, kNT, BucketCfg<false>::smem_bytes(p.bl), st>>>(p); ++launches;
     }
     k_scan_reduce<<<n_tiles, 1024, 0, st>>>(p); ++launches;
     k_scan_tiles<<<1, 1024, 0, st>>>(p, n_tiles); ++launches;
