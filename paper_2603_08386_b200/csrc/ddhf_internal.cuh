@@ -124,7 +124,7 @@ int launch_ingest(const IngestParams &p, cudaStream_t st);
 cudaError_t ingest_configure();              // opt in to large dynamic shared memory
 int ingest_tile_events();                    // events per sort tile
 int ingest_tile_stride(bool compact);        // items per tile slot of IngestParams::items (run padding included)
-size_t ingest_tile_smem(int nb);             // dynamic shared memory of k_tile_sort
+size_t ingest_tile_smem(bool compact);       // dynamic shared memory of k_tile_sort
 void ingest_plan(int np, int *bl, int *nb, int *hbits);   // digit split for a sensor of np pixels
 int launch_ndft(const NdftParams &p, int n_freq, int band_size, int grid_ndft, int grid_score, cudaStream_t st, cudaEvent_t between);
                                              // `between` (optional) is recorded after the NDFT kernel, before the scoring kernel

@@ -37,7 +37,8 @@ namespace {
 
 constexpr int kNT = 512;                       // threads per CTA of both sort kernels
 constexpr int kTile = 8192;                    // events per tile of k_tile_sort (16 per thread)
-constexpr int kCntStride = kNT + kNT / 32;     // words per counter row (one pad word per 32)
+constexpr int kCntStride = kNT + kNT / 32 + 16; // words per counter row: one pad word per 32, and a multiple of 32
+                                               // (the bank of a counter depends on the thread only, never on the digit)
 constexpr int kCntWords = 16 * kCntStride;     // 32 digits, two 16-bit counters per word
 constexpr unsigned kFullMask = 0xffffffffu;
 
@@ -134,17 +135,23 @@ __device__ __forceinline__ void sort_subpass(const T (&it)[K], uint32_t *cnt, T 
     // byte offset of the thread's column inside a counter row
     const uint32_t tb4 = static_cast<uint32_t>(t + (t >> 5)) * 4u;
     char *cb = reinterpret_cast<char *>(cnt);
+    // two items per round: both counters are read before either is written, so the two shared-memory
+    // round trips overlap; when both items hit the same counter the second sees the first's update
 #pragma unroll
-    for (int i = 0; i < K; ++i) {
-        const uint32_t d = digit_of<T>(it[i], shift, mask);
-        uint32_t *c = reinterpret_cast<uint32_t *>(cb + (d & rmask) * (kCntStride * 4u) + tb4);
-        *c += ((d >> (width - 1)) * 0xffffu) + 1u;     // +1 in the low or the high half; the thread's own
-    }                                                  // column: no other thread touches it
+    for (int i = 0; i < K; i += 2) {
+        const uint32_t d0 = digit_of<T>(it[i], shift, mask), d1 = digit_of<T>(it[i + 1], shift, mask);
+        uint32_t *c0 = reinterpret_cast<uint32_t *>(cb + (d0 & rmask) * (kCntStride * 4u) + tb4);
+        uint32_t *c1 = reinterpret_cast<uint32_t *>(cb + (d1 & rmask) * (kCntStride * 4u) + tb4);
+        const uint32_t v0 = *c0, v1 = *c1;
+        const uint32_t n0 = v0 + ((d0 >> (width - 1)) * 0xffffu) + 1u;     // +1 in the low or the high half
+        *c0 = n0;                                                          // the thread's own column: no other
+        *c1 = ((c0 == c1) ? n0 : v1) + ((d1 >> (width - 1)) * 0xffffu) + 1u;   // thread touches it
+    }
     __syncthreads();
     // exclusive scan of the matrix in (digit, thread) order: thread j rakes words [R j, R j + R)
     {
         const int w0 = R * t;
-        uint32_t *cp = cnt + w0 + (w0 >> 5);           // R <= 16: the R words share one pad offset
+        uint32_t *cp = cnt + w0 + (w0 >> 5) + 16 * (w0 >> 9);   // R <= 16: the R words share one pad offset
         uint32_t run = 0;
 #pragma unroll
         for (int i = 0; i < 16; ++i)
@@ -174,14 +181,18 @@ __device__ __forceinline__ void sort_subpass(const T (&it)[K], uint32_t *cnt, T 
     }
     __syncthreads();
 #pragma unroll
-    for (int i = 0; i < K; ++i) {
-        const uint32_t d = digit_of<T>(it[i], shift, mask);
-        const uint32_t hi = d >> (width - 1);
-        uint32_t *c = reinterpret_cast<uint32_t *>(cb + (d & rmask) * (kCntStride * 4u) + tb4);
-        const uint32_t old = *c;
-        *c = old + (hi * 0xffffu) + 1u;
-        const int rank = static_cast<int>((old >> (hi * 16u)) & 0xffffu);
-        buf[pad_pos<T>(rank)] = it[i];
+    for (int i = 0; i < K; i += 2) {
+        const uint32_t d0 = digit_of<T>(it[i], shift, mask), d1 = digit_of<T>(it[i + 1], shift, mask);
+        const uint32_t h0 = d0 >> (width - 1), h1 = d1 >> (width - 1);
+        uint32_t *c0 = reinterpret_cast<uint32_t *>(cb + (d0 & rmask) * (kCntStride * 4u) + tb4);
+        uint32_t *c1 = reinterpret_cast<uint32_t *>(cb + (d1 & rmask) * (kCntStride * 4u) + tb4);
+        const uint32_t v0 = *c0, v1 = *c1;
+        const uint32_t n0 = v0 + (h0 * 0xffffu) + 1u;
+        const uint32_t o1 = (c0 == c1) ? n0 : v1;
+        *c0 = n0;
+        *c1 = o1 + (h1 * 0xffffu) + 1u;
+        buf[pad_pos<T>(static_cast<int>((v0 >> (h0 * 16u)) & 0xffffu))] = it[i];
+        buf[pad_pos<T>(static_cast<int>((o1 >> (h1 * 16u)) & 0xffffu))] = it[i + 1];
     }
 }
 
@@ -305,19 +316,28 @@ __device__ __forceinline__ void finish_buckets(const IngestParams &p, uint32_t *
 }
 
 // ---- k_tile_sort: decode + filter one tile, sort it by bucket, publish its runs -----------------
-// Item in shared memory: (bucket << 16 | low) << 32 | value; dropped events and the padding of the
-// last tile carry the sentinel bucket nb and sort to the end of the tile.  A tile goes back to HBM
+// Only a 32-bit key (bucket << 13 | position in the tile) goes through the sort; dropped events and
+// the padding of the last tile carry the sentinel bucket nb and sort to the end of the tile.  The
+// payloads stay where the decode put them and are fetched by position at the end.  A tile goes back to HBM
 // with every bucket's run starting on a 16-byte boundary (k_bucket_sort gathers with 128-bit loads);
 // run table entry = first item of the run inside the tile's slot | length << 16.
+template <bool COMPACT> struct BucketItem { typedef uint32_t type; };
+template <> struct BucketItem<false> { typedef uint64_t type; };
+
 template <bool COMPACT> struct TileOut {
     static constexpr int kAlign = COMPACT ? 4 : 2;                      // items per 16 bytes
     static constexpr int kStride = kTile + (COMPACT ? 3 : 1) * 1024;     // items per tile slot (padding included)
 };
 
-template <bool FULL>
-__device__ __forceinline__ uint64_t load_item(const IngestParams &p, int64_t idx, uint32_t nb, uint32_t lmask, uint32_t window)
+// Decode one event: sort key = bucket << 13 | position in the tile (the sentinel bucket nb for dropped
+// events and for the padding of the last tile); payload = the item k_bucket_sort will read.
+template <bool FULL, bool COMPACT>
+__device__ __forceinline__ uint32_t load_event(const IngestParams &p, int64_t idx, uint32_t e, uint32_t nb, uint32_t lmask,
+                                               uint32_t window, typename BucketItem<COMPACT>::type &pay)
 {
-    uint64_t item = static_cast<uint64_t>(nb) << 48;
+    typedef typename BucketItem<COMPACT>::type TO;
+    uint32_t bucket = nb;
+    pay = 0;
     if (FULL || idx < p.n) {
         const int4 w = __ldg(reinterpret_cast<const int4 *>(p.events) + idx);
         const uint32_t x = static_cast<uint32_t>(w.x) & 0xffffu, y = static_cast<uint32_t>(w.x) >> 16;
@@ -325,23 +345,28 @@ __device__ __forceinline__ uint64_t load_item(const IngestParams &p, int64_t idx
         const uint64_t dt = t - static_cast<uint64_t>(p.t0);              // window < 2^31: in range iff dt < window
         const bool ok = (dt < window) && (x < static_cast<uint32_t>(p.width)) && (y < static_cast<uint32_t>(p.height));
         const uint32_t px = y * static_cast<uint32_t>(p.width) + x;
-        const uint32_t pos = (((static_cast<uint32_t>(w.y) - 1u) & 0xffffu) < 0x7fffu) ? 1u : 0u;   // int16 p > 0
-        const uint32_t hi = ok ? (((px >> p.bl) << 16) | (px & lmask)) : (nb << 16);
-        item = (static_cast<uint64_t>(hi) << 32) | ((static_cast<uint32_t>(dt) << 1) | pos);
+        const uint32_t pos = (static_cast<int32_t>(static_cast<uint32_t>(w.y) << 16) > 0) ? 1u : 0u;    // int16 p > 0
+        const uint32_t val = (static_cast<uint32_t>(dt) << 1) | pos;
+        if (ok) bucket = px >> p.bl;
+        if (COMPACT) pay = static_cast<TO>(((px & lmask) << p.vb) | val);
+        else pay = static_cast<TO>((static_cast<uint64_t>(px & lmask) << 32) | val);
     }
-    return item;
+    return (bucket << 13) | e;
 }
 
 template <bool COMPACT>
 __global__ void __launch_bounds__(kNT, 2) k_tile_sort(IngestParams p)
 {
+    typedef typename BucketItem<COMPACT>::type TO;
     extern __shared__ __align__(16) uint32_t s_raw[];
     __shared__ uint32_t s_warp[kNT / 32];
     __shared__ bool s_last;
     constexpr int K = kTile / kNT;
-    uint64_t *buf = reinterpret_cast<uint64_t *>(s_raw);                       // pad_pos(kTile) items
-    uint32_t *cnt = s_raw + 2 * (kTile + kTile / 16);
-    uint32_t *rstart = cnt + kCntWords;                                          // [1026]
+    // only the 32-bit keys go through the sort; the payloads stay where the decode put them
+    uint32_t *keys = s_raw;                                                      // pad_pos(kTile) keys
+    uint32_t *cnt = s_raw + (kTile + kTile / 32);
+    uint32_t *rstart = cnt + kCntWords;                                          // [1032]
+    TO *pay = reinterpret_cast<TO *>(rstart + 1032);                             // [kTile]
     const int t = threadIdx.x;
     const int tile = blockIdx.x;
     const int64_t tile_beg = static_cast<int64_t>(tile) * kTile;
@@ -349,30 +374,38 @@ __global__ void __launch_bounds__(kNT, 2) k_tile_sort(IngestParams p)
     const uint32_t lmask = (1u << p.bl) - 1u;
     const uint32_t window = static_cast<uint32_t>(p.t1 - p.t0);
 
-    // coalesced load, decode; staged in shared memory so that thread t then owns 16 consecutive events
+    // coalesced load and decode
     if (tile_beg + kTile <= p.n) {
 #pragma unroll 8
-        for (int i = 0; i < K; ++i)
-            buf[pad_pos<uint64_t>(t + kNT * i)] = load_item<true>(p, tile_beg + t + kNT * i, nb, lmask, window);
+        for (int i = 0; i < K; ++i) {
+            const uint32_t e = static_cast<uint32_t>(t + kNT * i);
+            TO py;
+            keys[pad_pos<uint32_t>(e)] = load_event<true, COMPACT>(p, tile_beg + e, e, nb, lmask, window, py);
+            pay[e] = py;
+        }
     } else {
 #pragma unroll 4
-        for (int i = 0; i < K; ++i)
-            buf[pad_pos<uint64_t>(t + kNT * i)] = load_item<false>(p, tile_beg + t + kNT * i, nb, lmask, window);
+        for (int i = 0; i < K; ++i) {
+            const uint32_t e = static_cast<uint32_t>(t + kNT * i);
+            TO py;
+            keys[pad_pos<uint32_t>(e)] = load_event<false, COMPACT>(p, tile_beg + e, e, nb, lmask, window, py);
+            pay[e] = py;
+        }
     }
     for (int b = t; b < 1026; b += kNT) rstart[b] = 0xffffffffu;
     __syncthreads();
-    uint64_t it[K];
+    uint32_t it[K];                                    // thread t owns 16 consecutive events
 #pragma unroll
-    for (int i = 0; i < K; ++i) it[i] = buf[pad_pos<uint64_t>(K * t + i)];
-    sort_items<K, uint64_t>(it, cnt, buf, s_warp, 48, p.hbits);
+    for (int i = 0; i < K; ++i) it[i] = keys[pad_pos<uint32_t>(K * t + i)];
+    sort_items<K, uint32_t>(it, cnt, keys, s_warp, 13, p.hbits);
 
     // start of every bucket's run inside the sorted tile
     {
         uint32_t prev = 0xffffffffu;
-        if (t > 0) prev = static_cast<uint32_t>(buf[pad_pos<uint64_t>(K * t - 1)] >> 48);
+        if (t > 0) prev = keys[pad_pos<uint32_t>(K * t - 1)] >> 13;
 #pragma unroll
         for (int i = 0; i < K; ++i) {
-            const uint32_t d = static_cast<uint32_t>(it[i] >> 48);
+            const uint32_t d = it[i] >> 13;
             if (d != prev) rstart[d] = static_cast<uint32_t>(K * t + i);
             prev = d;
         }
@@ -406,18 +439,15 @@ __global__ void __launch_bounds__(kNT, 2) k_tile_sort(IngestParams p)
     }
     __syncthreads();
     const int kept = static_cast<int>(rstart[nb]);
-    const size_t out0 = static_cast<size_t>(tile) * TileOut<COMPACT>::kStride;
-#pragma unroll 4
-    for (int i = 0; i < K; ++i) {
-        const int r = t + kNT * i;
-        if (r < kept) {
-            const uint64_t item = buf[pad_pos<uint64_t>(r)];
-            const uint32_t hi = static_cast<uint32_t>(item >> 32), val = static_cast<uint32_t>(item);
-            const size_t at = out0 + static_cast<uint32_t>(r) + delta[hi >> 16];
-            if (COMPACT)
-                reinterpret_cast<uint32_t *>(p.items)[at] = ((hi & 0xffffu) << p.vb) | val;
-            else
-                reinterpret_cast<uint64_t *>(p.items)[at] = (static_cast<uint64_t>(hi & 0xffffu) << 32) | val;
+    {
+        TO *out = reinterpret_cast<TO *>(p.items) + static_cast<size_t>(tile) * TileOut<COMPACT>::kStride;
+#pragma unroll
+        for (int i = 0; i < K; ++i) {
+            const int r = t + kNT * i;
+            if (r < kept) {
+                const uint32_t key = keys[pad_pos<uint32_t>(r)];
+                out[static_cast<uint32_t>(r) + delta[key >> 13]] = pay[key & 8191u];
+            }
         }
     }
     // the last CTA to finish turns the bucket totals into bases, publishes the event counts and
@@ -428,7 +458,7 @@ __global__ void __launch_bounds__(kNT, 2) k_tile_sort(IngestParams p)
     __syncthreads();
     if (!s_last) return;
     __threadfence();
-    finish_buckets(p, cnt, reinterpret_cast<uint32_t *>(buf), s_warp);
+    finish_buckets(p, cnt, keys, s_warp);
 }
 
 // ---- k_bucket_sort: gather one bucket from all tiles, sort it by the low digit, write the rows -------
@@ -436,8 +466,6 @@ __global__ void __launch_bounds__(kNT, 2) k_tile_sort(IngestParams p)
 //        else     uint64  low << 32 | value
 // The padding of a partly filled chunk is all ones: it sorts behind every real item in every sub-pass
 // (it also comes last in input order), so positions [0, fill) of the sorted chunk are the real items.
-template <bool COMPACT> struct BucketItem { typedef uint32_t type; };
-template <> struct BucketItem<false> { typedef uint64_t type; };
 
 template <bool COMPACT>
 struct BucketCfg {
@@ -840,14 +868,14 @@ template <bool COMPACT>
 cudaError_t configure_sort_kernels()
 {
     cudaError_t e = cudaFuncSetAttribute(k_tile_sort<COMPACT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         static_cast<int>(ingest_tile_smem(1023)));
+                                         static_cast<int>(ingest_tile_smem(COMPACT)));
     if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(k_bucket_sort<COMPACT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 static_cast<int>(BucketCfg<COMPACT>::smem_bytes(12)));
 }
 }  // namespace
 
-size_t ingest_tile_smem(int nb) { (void)nb; return 4u * (2u * (kTile + kTile / 16) + kCntWords + 1032u); }
+size_t ingest_tile_smem(bool compact) { return 4u * ((kTile + kTile / 32) + kCntWords + 1032u + (compact ? 1u : 2u) * kTile); }
 
 cudaError_t ingest_configure()
 {
@@ -882,10 +910,10 @@ int launch_ingest(const IngestParams &p, cudaStream_t st)
     const int init_items = p.np > p.nb + 2 ? p.np : p.nb + 2;
     k_init<<<(init_items + 255) / 256, 256, 0, st>>>(p); ++launches;
     if (p.compact) {
-        if (ev_tiles > 0) { k_tile_sort<true><<<ev_tiles, kNT, ingest_tile_smem(p.nb), st>>>(p); ++launches; }
+        if (ev_tiles > 0) { k_tile_sort<true><<<ev_tiles, kNT, ingest_tile_smem(true), st>>>(p); ++launches; }
         k_bucket_sort<true><<<p.nb, kNT, BucketCfg<true>::smem_bytes(p.bl), st>>>(p); ++launches;
     } else {
-        if (ev_tiles > 0) { k_tile_sort<false><<<ev_tiles, kNT, ingest_tile_smem(p.nb), st>>>(p); ++launches; }
+        if (ev_tiles > 0) { k_tile_sort<false><<<ev_tiles, kNT, ingest_tile_smem(false), st>>>(p); ++launches; }
         k_bucket_sort<false><<<p.nb, kNT, BucketCfg<false>::smem_bytes(p.bl), st>>>(p); ++launches;
     }
     k_scan_reduce<<<n_tiles, 1024, 0, st>>>(p); ++launches;
