@@ -31,7 +31,7 @@ struct ddhf_handle {
     int ndft_blocks_per_sm = 1, score_blocks_per_sm = 1;
     // workspace offsets (bytes)
     size_t off_cnt = 0, off_items = 0, off_scratch = 0, off_work = 0, off_tiles = 0, off_class = 0, off_cursor = 0, off_runs = 0, off_bkt = 0, off_rows = 0, off_spill = 0, off_spillrec = 0,
-           off_parent = 0, off_rec = 0, off_ctiles = 0, ws_bytes = 0;
+           off_parent = 0, off_rec = 0, off_ctiles = 0, off_split = 0, off_splitcnt = 0, off_partial = 0, ws_bytes = 0;
     cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     bool timed_once = false;
     // buffers of the host-buffer variant
@@ -241,7 +241,15 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
         h->off_items = o;  o = align_up(o + ev_tiles * (a > b ? a : b));
     }
     h->off_scratch = o;    o = align_up(o + sizeof(uint64_t) * static_cast<size_t>(c.max_events));
-    h->off_work = o;       o = align_up(o + sizeof(WorkItem) * static_cast<size_t>(h->np));
+    // work list: one item per active pixel, one more per extra segment of a split row (rows > kSplitMin
+    // events in segments of <= kSegEvents); partial sums and arrival counters of the segment trees
+    const size_t max_segs = static_cast<size_t>(c.max_events) / kSegEvents + static_cast<size_t>(c.max_events) / kSplitMin + 2;
+    const size_t max_rows = static_cast<size_t>(c.max_events) / kSplitMin + 1;          // rows that can be split
+    const size_t max_slots = max_segs * kSplitFan / (kSplitFan - 1) + 4 * max_rows + 64;   // leaves + inner nodes, rounding per level
+    h->off_work = o;       o = align_up(o + sizeof(WorkItem) * (static_cast<size_t>(h->np) + max_segs));
+    h->off_split = o;      o = align_up(o + sizeof(SplitRow) * max_rows);
+    h->off_splitcnt = o;   o = align_up(o + sizeof(int32_t) * (max_segs + 4 * max_rows + 64));
+    h->off_partial = o;    o = align_up(o + sizeof(float) * max_slots * 2 * ndft_padded_bins(c.n_freq));
     h->off_tiles = o;      o = align_up(o + sizeof(int32_t) * 4 * 1024);
     h->off_class = o;      o = align_up(o + sizeof(int32_t) * 2 * kNumClasses);
     h->off_cursor = o;     o = align_up(o + 256);
@@ -320,11 +328,15 @@ extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n
     ip.chunk_rows = reinterpret_cast<int32_t *>(ws + h->off_rows);
     ip.sync = reinterpret_cast<int32_t *>(ws + h->off_cursor + 16);       // [8]; the scoring queue counts are sync[2..3]
 
+    ip.split_tab = reinterpret_cast<SplitRow *>(ws + h->off_split);
+    ip.split_cnt = reinterpret_cast<int32_t *>(ws + h->off_splitcnt);
     ip.ccl_parent = cp_parent;
 
     NdftParams np{};
     np.work = ip.work; np.csr_ev = out->csr_ev; np.counters = out->counters;
     np.work_cursor = ip.work_cursor; np.max_active = c.max_active;
+    np.n_work = ip.sync + 4; np.split_tab = ip.split_tab; np.split_cnt = ip.split_cnt;
+    np.split_partial = reinterpret_cast<float *>(ws + h->off_partial);
     np.g_f0 = h->g_f0; np.g_d = h->g_d; np.g_h = h->g_h;
     np.power = out->power; np.sf = out->sf; np.score = out->score; np.f0_idx = out->f0_idx;
     np.mask = out->mask; np.comb_debug = out->comb_debug;

@@ -23,6 +23,23 @@ struct __align__(16) WorkItem {
     int32_t arow;        // row of the compact outputs (index into active_idx)
 };
 
+// Rows longer than kSplitMin events are split into segments of equal length (at most kSegEvents), one
+// work item each, and their partial sums are combined along a tree of fan-in kSplitFan; see k_ndft_score.
+// A segment's work item has pix = 0x80000000 | split row, arow = segment.
+constexpr int kSplitMin = 4096;
+constexpr int kSegEvents = 512;
+constexpr int kSplitFan = 8;
+struct __align__(16) SplitRow {
+    int32_t pix, arow;           // the row's identity (arow: row of the compact outputs)
+    int32_t n_seg;               // segments of the row = leaves of its tree
+    int32_t seg_base;            // first partial of the row in NdftParams::split_partial (leaves, then level 1, ...)
+    int32_t cnt_base;            // first arrival counter of the row in NdftParams::split_cnt (level 1, level 2, ...)
+    int32_t _pad[3];
+};
+// partial slots / arrival counters of a row of n_seg segments (the root has a counter but no slot)
+__host__ __device__ inline int split_slots(int n) { int s = 0; while (n > 1) { s += n; n = (n + kSplitFan - 1) / kSplitFan; } return s; }
+__host__ __device__ inline int split_nodes(int n) { int c = 0; while (n > 1) { n = (n + kSplitFan - 1) / kSplitFan; c += n; } return c; }
+
 // Constants of the SF / comb stages (a5-a7) and the per-candidate tables, built on the host at create
 // time (readings R7-R10).  Tables are padded to `cpad` candidates (a multiple of 32) so that a warp
 // reads them without range checks; layout [row][cpad], candidate fastest (coalesced per lane).
@@ -53,7 +70,11 @@ struct __align__(16) SpillRec {
 struct NdftParams {
     const WorkItem *work;        // DEVICE [n_active] ordered by descending size class
     const uint32_t *csr_ev;
-    const int32_t *counters;     // n_active is read from here (device side)
+    const int32_t *counters;
+    const int32_t *n_work;       // DEVICE: work items = active pixels + extra segments of split rows
+    const SplitRow *split_tab;   // rows longer than kSplitMin events
+    float *split_partial;        // [slots][2 * padded bins] partial (S1..S4) sums of the segments and tree nodes
+    int32_t *split_cnt;          // arrival counters of the tree nodes (zeroed when the row is split)
     unsigned long long *work_cursor;   // dynamic work queue: items taken from the head (hi 32) / tail (lo 32)
     int32_t max_active;
     uint64_t g_f0, g_d, g_h;     // 2^64 * f * 1e-6 for: centre base, df, 16*df
@@ -90,7 +111,10 @@ struct IngestParams {
     int32_t *bkt_order;          // [nb] buckets by descending size class
     int32_t *bkt_total, *bkt_base;   // [nb + 2] events per bucket; exclusive scan (bkt_base[nb] = n_in)
     int32_t *chunk_rows;         // [max_rows][4 + 2^bl] chunk table of the multi-chunk buckets
-    int32_t *sync;               // [8] 0: tiles finished, 1: chunk rows handed out, 2-3: scoring queue counts
+    int32_t *sync;               // [8] 0: tiles finished, 1: chunk rows handed out, 2-3: scoring queue counts,
+                                 //     4: work items, 5: split rows, 6: partials, 7: arrival counters handed out
+    SplitRow *split_tab;         // rows longer than kSplitMin (see NdftParams)
+    int32_t *split_cnt;
     int32_t *active_idx;
     WorkItem *work;
     int32_t *tile_sum, *tile_act;   // [n_tiles]

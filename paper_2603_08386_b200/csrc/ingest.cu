@@ -71,6 +71,14 @@ __device__ __forceinline__ int size_class(int n)
     return min(kNumClasses - 1, max(0, bl - 3));
 }
 
+// A row longer than kSplitMin becomes n_seg work items of seg_len <= kSegEvents events (the last one shorter).
+__device__ __forceinline__ int row_segments(int n, int &seg_len)
+{
+    const int n_seg = (n > kSplitMin) ? (n + kSegEvents - 1) / kSegEvents : 1;
+    seg_len = (n + n_seg - 1) / n_seg;
+    return n_seg;
+}
+
 // ---- k_init: per-pixel maps for inactive pixels, zeroed totals and counters ---------------
 __global__ void k_init(IngestParams p)
 {
@@ -769,7 +777,9 @@ __global__ void __launch_bounds__(1024) k_scan_reduce(IngestParams p)
         sum += v[j];
         if (v[j] >= nmin) {
             ++act;
-            atomicAdd(&s_cls[size_class(v[j])], 1);
+            int seg_len;
+            const int n_seg = row_segments(v[j], seg_len);
+            atomicAdd(&s_cls[size_class(seg_len)], n_seg);
         }
     }
     int ta, tb;
@@ -805,6 +815,7 @@ __global__ void __launch_bounds__(1024) k_scan_tiles(IngestParams p, int n_tiles
             p.class_cnt[c] = run;                         // becomes the class base
             run += n;
         }
+        p.sync[4] = run;                                  // work items (a split row counts once per segment)
     }
 }
 
@@ -827,7 +838,9 @@ __global__ void __launch_bounds__(1024) k_scan_apply(IngestParams p)
         lrank[j] = -1;
         if (v[j] >= nmin) {
             ++act;
-            lrank[j] = atomicAdd(&s_cls[size_class(v[j])], 1);
+            int seg_len;
+            const int n_seg = row_segments(v[j], seg_len);
+            lrank[j] = atomicAdd(&s_cls[size_class(seg_len)], n_seg);
         }
     }
     int ta, tb;
@@ -846,12 +859,35 @@ __global__ void __launch_bounds__(1024) k_scan_apply(IngestParams p)
             p.row_ptr[pix] = off;
             if (lrank[j] >= 0) {
                 if (aoff < p.max_active) p.active_idx[aoff] = pix;
+                int seg_len;
+                const int n_seg = row_segments(v[j], seg_len);
+                WorkItem *dst = p.work + s_base[size_class(seg_len)] + lrank[j];
                 WorkItem it;
-                it.row_begin = off;
-                it.n = v[j];
-                it.pix = pix;
-                it.arow = aoff;
-                p.work[s_base[size_class(v[j])] + lrank[j]] = it;
+                if (n_seg == 1) {
+                    it.row_begin = off;
+                    it.n = v[j];
+                    it.pix = pix;
+                    it.arow = aoff;
+                    *dst = it;
+                } else {
+                    // split row: one work item per segment, the row's identity in the split table
+                    const int sid = atomicAdd(p.sync + 5, 1);
+                    SplitRow sr;
+                    const int nodes = split_nodes(n_seg);
+                    sr.pix = pix; sr.arow = aoff; sr.n_seg = n_seg;
+                    sr.seg_base = atomicAdd(p.sync + 6, split_slots(n_seg));
+                    sr.cnt_base = atomicAdd(p.sync + 7, nodes);
+                    sr._pad[0] = 0; sr._pad[1] = 0; sr._pad[2] = 0;
+                    p.split_tab[sid] = sr;
+                    for (int q = 0; q < nodes; ++q) p.split_cnt[sr.cnt_base + q] = 0;
+                    for (int sg = 0; sg < n_seg; ++sg) {
+                        it.row_begin = off + sg * seg_len;
+                        it.n = min(seg_len, v[j] - sg * seg_len);
+                        it.pix = static_cast<int32_t>(0x80000000u | static_cast<uint32_t>(sid));
+                        it.arow = sg;
+                        dst[sg] = it;
+                    }
+                }
                 ++aoff;
             }
             off += v[j];

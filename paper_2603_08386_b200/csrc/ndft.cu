@@ -102,13 +102,20 @@ __device__ __forceinline__ void sincos_u32(uint32_t ph, float &s, float &c)
 #define DDHF_TAIL_BATCH 4
 #endif
 constexpr int kTailBatch = DDHF_TAIL_BATCH;
+constexpr unsigned kTailBatchMinLeft = 65536u;      // items left below which tail warps stop batching
 
-__device__ __forceinline__ int fetch_items(unsigned long long *cursor, bool head, int n_items, int &cnt)
+__device__ __forceinline__ int fetch_items(unsigned long long *cursor, bool head, int n_items, int &cnt, unsigned &seen_used)
 {
-    const unsigned b = head ? 1u : static_cast<unsigned>(kTailBatch);
+    // near the end of the list (or in a short list, where the tail holds long rows or segments of a split
+    // row) tail warps claim one item at a time, so that no warp sits on a batch of expensive items while
+    // others idle.  `seen_used` = items handed out as of this warp's previous claim: a hint, the atomic decides.
+    const unsigned n = static_cast<unsigned>(n_items);
+    const bool batch = !head && seen_used + kTailBatchMinLeft < n;
+    const unsigned b = batch ? static_cast<unsigned>(kTailBatch) : 1u;
     const unsigned long long old = atomicAdd(cursor, head ? (1ull << 32) : static_cast<unsigned long long>(b));
     const unsigned h = static_cast<unsigned>(old >> 32), t = static_cast<unsigned>(old);
-    const unsigned used = h + t, n = static_cast<unsigned>(n_items);
+    const unsigned used = h + t;
+    seen_used = used;
     cnt = (used >= n) ? 0 : static_cast<int>(min(b, n - used));
     return head ? static_cast<int>(h) : n_items - 1 - static_cast<int>(t);
 }
@@ -151,7 +158,7 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
     float2 *btab = reinterpret_cast<float2 *>(scr);                 // [kEC][TN]
     uint4 *phs = reinterpret_cast<uint4 *>(scr + kEC * TN * 2);     // [kEC]
 
-    const int n_items = p.counters[DDHF_CNT_N_ACTIVE];
+    const int n_items = *p.n_work;                     // active pixels + the extra segments of split rows
     const ScoreParams &sp = p.sp;
     constexpr int EPP = 32 / TN;       // events per table pass
     constexpr bool full_grid = FULL;
@@ -165,7 +172,8 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
     const bool head = (wid % 3) < DDHF_NDFT_HEAD_WARPS;
     int claim_left = 0;                                             // items of the current claim not yet started
     int idx = 0;
-    if (lane == 0) idx = fetch_items(p.work_cursor, head, n_items, claim_left);
+    unsigned seen_used = 0u;
+    if (lane == 0) idx = fetch_items(p.work_cursor, head, n_items, claim_left, seen_used);
     idx = __shfl_sync(kFull, idx, 0);
     claim_left = __shfl_sync(kFull, claim_left, 0);
     if (claim_left == 0) idx = n_items;
@@ -179,8 +187,11 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
     while (idx < n_items) {
         const WorkItem it = it_next;
         // next item: the following one of the claim (tail warps walk down the list), or a new claim
+        // (claimed before the row is processed, except by the segments of a split row: a warp that starts a
+        // segment must not sit on a second one that an idle warp could take)
         int next_idx = idx - 1, next_cnt = claim_left;
-        if (claim_left <= 0 && lane == 0) next_idx = fetch_items(p.work_cursor, head, n_items, next_cnt);
+        const bool claim_early = it.pix >= 0;
+        if (claim_left <= 0 && claim_early && lane == 0) next_idx = fetch_items(p.work_cursor, head, n_items, next_cnt, seen_used);
 
         float2 acc1[TM][TN], acc2[TM][TN];     // (S1, S4) and (S3, S2)
 #pragma unroll
@@ -278,6 +289,7 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
 
         // the next pixel's work item and first events are fetched under the epilogue
         if (claim_left <= 0) {
+            if (!claim_early && lane == 0) next_idx = fetch_items(p.work_cursor, head, n_items, next_cnt, seen_used);
             idx = __shfl_sync(kFull, next_idx, 0);
             claim_left = __shfl_sync(kFull, next_cnt, 0);
             if (claim_left == 0) idx = n_items;
@@ -286,6 +298,76 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
         }
         --claim_left;
         if (idx < n_items) it_next = p.work[idx];
+
+        // ---- split rows: a row longer than kSplitMin events is accumulated by several warps, one segment
+        // of <= kSegEvents events each (S1..S4 are linear in the events).  The partial sums are combined
+        // along a fixed tree of fan-in kSplitFan: the warp that arrives last at a node adds the node's
+        // children in index order, whoever that warp is, so the result does not depend on the schedule;
+        // the warp that completes the root runs the row's epilogue.
+        int out_pix = it.pix, out_arow = it.arow;
+        if (__builtin_expect(it.pix < 0, 0)) {
+            const SplitRow *sr = p.split_tab + (it.pix & 0x7fffffff);
+            constexpr int PW = 2 * NBL * 32;                       // floats per partial
+            int n_l = sr->n_seg, idx_l = it.arow;                  // nodes of the current level, this warp's node
+            int slot0 = sr->seg_base, cnt0 = sr->cnt_base;         // first partial / first counter of the level
+            bool last = true;
+            while (n_l > 1) {
+                float *mine = p.split_partial + static_cast<size_t>(slot0 + idx_l) * PW + lane;
+#pragma unroll
+                for (int g = 0; g < TM; ++g)
+#pragma unroll
+                    for (int m = 0; m < TN; ++m) {
+                        const int k = (g * TN + m) * 4;
+                        __stcg(mine + (k + 0) * 32, acc1[g][m].x);
+                        __stcg(mine + (k + 1) * 32, acc1[g][m].y);
+                        __stcg(mine + (k + 2) * 32, acc2[g][m].x);
+                        __stcg(mine + (k + 3) * 32, acc2[g][m].y);
+                    }
+                __threadfence();
+                __syncwarp();
+                const int parent = idx_l / kSplitFan;
+                const int c_beg = parent * kSplitFan, c_end = min(n_l, c_beg + kSplitFan);
+                int done = 0;
+                if (lane == 0) done = atomicAdd(p.split_cnt + cnt0 + parent, 1);
+                done = __shfl_sync(kFull, done, 0);
+                if (done != c_end - c_beg - 1) { last = false; break; }
+                __threadfence();
+#pragma unroll
+                for (int g = 0; g < TM; ++g)
+#pragma unroll
+                    for (int m = 0; m < TN; ++m) {
+                        acc1[g][m] = make_float2(0.f, 0.f);
+                        acc2[g][m] = make_float2(0.f, 0.f);
+                    }
+#pragma unroll 1
+                for (int c = c_beg; c < c_end; ++c) {
+                    const float *ps = p.split_partial + static_cast<size_t>(slot0 + c) * PW + lane;
+#pragma unroll
+                    for (int g = 0; g < TM; ++g)
+#pragma unroll
+                        for (int m = 0; m < TN; ++m) {
+                            const int k = (g * TN + m) * 4;
+                            acc1[g][m].x += __ldcg(ps + (k + 0) * 32);
+                            acc1[g][m].y += __ldcg(ps + (k + 1) * 32);
+                            acc2[g][m].x += __ldcg(ps + (k + 2) * 32);
+                            acc2[g][m].y += __ldcg(ps + (k + 3) * 32);
+                        }
+                }
+                slot0 += n_l;
+                n_l = (n_l + kSplitFan - 1) / kSplitFan;
+                cnt0 += n_l;
+                idx_l = parent;
+            }
+            if (!last) {
+                // another warp finishes the row: no epilogue; the next pixel's first events are staged here
+                if (idx < n_items && lane < it_next.n)
+                    stage_event(ev_s + evb * kEC + lane, p.csr_ev + it_next.row_begin + lane);
+                __syncwarp();
+                continue;
+            }
+            out_pix = sr->pix;
+            out_arow = sr->arow;
+        }
 
         // ---- epilogue: powers, optional spectrum store, spectral flatness -------------------
         float preg[NBL];
@@ -299,9 +381,9 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
                 preg[g * 2 * TN + TN + m] = rp * rp + ip * ip;
                 preg[g * 2 * TN + TN - 1 - m] = rm * rm + im * im;
             }
-        const bool has_row = it.arow < p.max_active;
+        const bool has_row = out_arow < p.max_active;
         if (store_power && has_row) {
-            float *dst = p.power + static_cast<size_t>(it.arow) * sp.n_freq + lane;
+            float *dst = p.power + static_cast<size_t>(out_arow) * sp.n_freq + lane;
 #pragma unroll
             for (int i = 0; i < NBL; ++i)
                 if (full_grid || i * 32 + lane < sp.n_freq) __stcs(dst + i * 32, preg[i]);
@@ -372,7 +454,7 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
                 for (int i = 0; i < NBL; ++i) dst[i * 32] = preg[i];
                 if (lane == 0) {
                     SpillRec r;
-                    r.pix = it.pix; r.arow = has_row ? it.arow : -1; r.mean_p = mean_p; r._pad = 0;
+                    r.pix = out_pix; r.arow = has_row ? out_arow : -1; r.mean_p = mean_p; r._pad = 0;
                     p.spill_rec[slot] = r;
                 }
             } else if (L::INPLACE) {
@@ -388,7 +470,7 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
                 }
                 __syncwarp();
                 float *dbg = (p.comb_debug != nullptr && has_row)
-                                 ? p.comb_debug + static_cast<size_t>(it.arow) * sp.n_f0 * 3 : nullptr;
+                                 ? p.comb_debug + static_cast<size_t>(out_arow) * sp.n_f0 * 3 : nullptr;
                 const float2 r = comb_score_from_smem<NBL, L::INPLACE ? BS : 256>(scr, sp, mean_p, lane, dbg);
                 score = r.x;
                 f0 = __float_as_int(r.y);
@@ -396,11 +478,11 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
             }
         }
         if (lane == 0) {
-            p.sf[it.pix] = sfv;
+            p.sf[out_pix] = sfv;
             if (!deferred) {
-                p.score[it.pix] = score;
-                p.f0_idx[it.pix] = f0;
-                p.mask[it.pix] = (sf_ok && f0 >= 0 && score >= sp.tau_comb) ? 1 : 0;   // eq. 11
+                p.score[out_pix] = score;
+                p.f0_idx[out_pix] = f0;
+                p.mask[out_pix] = (sf_ok && f0 >= 0 && score >= sp.tau_comb) ? 1 : 0;   // eq. 11
             }
         }
         __syncwarp();

@@ -332,3 +332,77 @@ def test_box_merge_disabled_leaves_output_alone(oracle):
     prm = dict(w.params, merge_alpha=0.0)
     gpu = gu.run_gpu(prm, w.events, 0, w.window_us)
     assert "merged_boxes" not in gpu and int(gpu["counters"][8]) == 0
+
+
+@pytest.mark.parametrize("n_hot", [4096, 4097, 8200, 30_000])
+def test_split_row_segments(oracle, n_hot):
+    """A row longer than 4096 events is split into segments of <= 1024 events whose partial sums are
+    combined along a fixed tree (ndft.cu): 4096 stays whole, 4097 gives 5 segments (one tree level),
+    8200 gives 9 (two levels), 30 000 gives 30.  Everything is compared with the oracle."""
+    rng = np.random.default_rng(n_hot)
+    bg = wl.random_window(21, 48, 40, 6000, 20_000, hot_fraction=0.2)
+    hot = np.zeros(n_hot, dtype=wl.EVENT_DTYPE)
+    hot["x"], hot["y"] = 17, 23
+    hot["t"] = rng.integers(0, 20_000, size=n_hot)
+    # a rotor at 300 Hz, duty 0.3: ON at the start of the pulse, OFF at its end, plus noise
+    k = np.arange(n_hot)
+    hot["t"][::2] = ((k[::2] // 2 % 6) * 3333 + rng.integers(0, 40, size=len(k[::2]))) % 20_000
+    hot["p"] = np.where(k % 2 == 0, 1, -1)
+    ev = np.concatenate([bg, hot])
+    ev = ev[np.argsort(ev["t"], kind="stable")]
+    prm = dict(SMALL, n_min=3)
+    orc = oracle.window(prm, ev, 0, 20_000, score_all=True)
+    gpu = gu.run_gpu(prm, ev, 0, 20_000, score_all=True)
+    gu.check_csr(gpu, orc)
+    assert np.diff(orc["row_ptr"]).max() >= n_hot
+    assert gu.power_error(gpu["power"], orc["power"]) <= gu.POWER_TOL
+    gu.check_maps(gpu, orc, prm, score_all=True, oracle_mod=oracle, orc_power=orc["power"])
+    # the split is deterministic: a second run gives the same bits
+    gpu2 = gu.run_gpu(prm, ev, 0, 20_000, score_all=True)
+    assert np.array_equal(gpu["power"], gpu2["power"]) and np.array_equal(gpu["score"], gpu2["score"], equal_nan=True)
+
+
+@pytest.mark.slow
+def test_stuck_pixel_million_events_on_config2(oracle):
+    """One pixel firing 10^6 events in the window on top of the config-2 scene (PAPER.md L141 assumes
+    "tens of events per pixel"): its spectrum matches the oracle, every other pixel is what it is
+    without the stuck pixel, and the NDFT stage stays within 2x of (terms / the config-4 rate)."""
+    w = wl.make(2)
+    prm = dict(w.params, n_min=6)
+    n_hot = 1_000_000
+    rng = np.random.default_rng(99)
+    hot = np.zeros(n_hot, dtype=wl.EVENT_DTYPE)
+    hot["x"], hot["y"] = 301, 17
+    hot["t"] = np.sort(rng.integers(0, w.window_us, size=n_hot)) + w.t0_us
+    hot["p"] = rng.integers(0, 2, size=n_hot) * 2 - 1
+    ev = np.concatenate([w.events, hot])
+    ev = ev[np.argsort(ev["t"], kind="stable")]
+    base = gu.run_gpu(prm, w.events, w.t0_us, w.window_us)
+    gpu = gu.run_gpu(prm, ev, w.t0_us, w.window_us, timing=True)
+    pix = 17 * w.width + 301
+    # the stuck pixel against the oracle's direct sum on its row (one pixel: seconds on one core)
+    row_ptr, csr, _ = oracle.bucket(ev, w.width, w.height, w.t0_us, w.window_us)
+    assert np.array_equal(gpu["row_ptr"], row_ptr) and np.array_equal(gpu["csr_ev"], csr)
+    row = csr[row_ptr[pix]:row_ptr[pix + 1]]
+    assert len(row) >= n_hot
+    p_orc = oracle.ndft_power(row >> 1, np.where(row & 1, 1.0, -1.0), prm["f_min_hz"], prm["df_hz"], prm["n_freq"])
+    r = int(np.flatnonzero(gpu["active_idx"] == pix)[0])
+    err = np.abs(gpu["power"][r] - p_orc).max() / p_orc.max()
+    print(f"stuck pixel: {len(row)} events, power err / peak {err:.2e}, stage ms {gpu['stage_ms']}")
+    assert err <= gu.POWER_TOL
+    sf_o = oracle.spectral_flatness(p_orc, prm["k_lo"], prm["sf_eps"])
+    assert abs(gpu["sf"].ravel()[pix] - sf_o) <= 1e-3 * sf_o
+    # every other pixel: exactly the maps of the scene without the stuck pixel
+    other = np.ones(w.width * w.height, dtype=bool)
+    other[pix] = False
+    for k in ("sf", "score", "f0_idx"):
+        assert np.array_equal(gpu[k].ravel()[other], base[k].ravel()[other], equal_nan=True), k
+    m_g, m_b = gpu["mask"].ravel().copy(), base["mask"].ravel().copy()
+    assert np.array_equal(m_g[other], m_b[other])
+    if m_g[pix] == m_b[pix]:
+        assert np.array_equal(gpu["boxes"], base["boxes"])
+    # time: terms of the window / 10 Tterms/s (the NDFT kernel's rate on config 4), within 2x
+    cnt = np.diff(row_ptr)
+    terms = prm["n_freq"] * float(cnt[cnt >= prm["n_min"]].sum())
+    budget_ms = 2.0 * terms / 10.0e12 * 1e3
+    assert gpu["stage_ms"][1] <= budget_ms, (gpu["stage_ms"], budget_ms)
