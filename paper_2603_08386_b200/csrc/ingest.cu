@@ -543,6 +543,7 @@ __device__ __forceinline__ void sort_chunk_any(typename BucketItem<COMPACT>::typ
 // bucket (-1: none), offset of the chunk inside the bucket, items, 0} followed by 2^bL per-pixel words
 // delta[l] = (events of pixel l in earlier chunks) - (first sorted position of pixel l in this chunk).
 constexpr int kRowHdr = 4;
+constexpr int kLongRun = 256;      // runs longer than this are gathered by the whole CTA
 
 template <bool COMPACT>
 __global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
@@ -639,12 +640,26 @@ __global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
                 __syncthreads();
                 cut = s_cut;
             }
+            // short runs: one thread each; long runs (a hot pixel fills most of a tile) are queued in the
+            // counter array, idle during the gather, and copied by the whole CTA
+            uint32_t *lq = cnt;                                   // [0] = queued runs, then {src / 16 B, dst, len}
+            if (t == 0) lq[0] = 0u;
+            __syncthreads();
 #pragma unroll
             for (int q = 0; q < 2; ++q) {
                 if (len[q] > 0 && off[q] >= base_off && off[q] < cut) {
                     const int j = tb + 2 * t + q;
-                    const uint4 *s = items + (static_cast<size_t>(j) * TileOut<COMPACT>::kStride + src[q]) / kPer16;
+                    const size_t s16 = (static_cast<size_t>(j) * TileOut<COMPACT>::kStride + src[q]) / kPer16;
                     const int dst = fill + off[q] - base_off;
+                    if (len[q] > kLongRun) {
+                        const uint32_t e = atomicAdd(&lq[0], 1u);
+                        lq[1 + 4 * e] = static_cast<uint32_t>(s16);
+                        lq[2 + 4 * e] = static_cast<uint32_t>(s16 >> 32);
+                        lq[3 + 4 * e] = static_cast<uint32_t>(dst);
+                        lq[4 + 4 * e] = static_cast<uint32_t>(len[q]);
+                        continue;
+                    }
+                    const uint4 *s = items + s16;
                     for (int i = 0; i < len[q]; i += 2 * kPer16) {     // two independent 128-bit loads per round
                         const uint4 v0 = __ldg(s + i / kPer16);
                         uint4 v1 = make_uint4(0u, 0u, 0u, 0u);
@@ -662,6 +677,17 @@ __global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
                                 if (i + u < len[q]) buf[pad_pos<T>(dst + i + u)] = static_cast<T>(w[u]);
                         }
                     }
+                }
+            }
+            __syncthreads();
+            {
+                const int n_long = static_cast<int>(lq[0]);
+                const T *items_t = reinterpret_cast<const T *>(p.items);
+                for (int e = 0; e < n_long; ++e) {
+                    const size_t s16 = (static_cast<size_t>(lq[2 + 4 * e]) << 32) | lq[1 + 4 * e];
+                    const int dst = static_cast<int>(lq[3 + 4 * e]), ln = static_cast<int>(lq[4 + 4 * e]);
+                    const T *s = items_t + s16 * kPer16;
+                    for (int i = t; i < ln; i += kNT) buf[pad_pos<T>(dst + i)] = __ldg(s + i);
                 }
             }
             fill += cut - base_off;
