@@ -1,13 +1,19 @@
 #!/usr/bin/env python
 """bench.py -- DDHF hot path on B200: NDFT Gterms/s and ms per 1280x720 window.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4|cfg5] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4|cfg5|cfg3|paper] [--impl reference]
+                  [--no-sub] [--no-cpu-baseline] [--score-all] [--spectra]
 
 A *step* is one pass of the whole hot path (a0-a8: ingest, NDFT power, spectral flatness, comb
 score, mask, CCL/boxes) over one synthetic window.  Default workload: BASELINE.json config 4
 (1280x720, 100 ms, ~10 M events, 5 % of the pixels hold 60 % of the events) -- the heaviest
 single 1280x720 window; `--workload cfg5` runs the streaming config (sliding 50 ms windows,
 10 ms hop, 50 Mev/s) with one step per window.
+
+The default run (config 4, one GPU) also measures, each with its own clocks record, the variants
+SURVEY.md section 8(d) lists: config 4 with the comb score on every active pixel, with Table 2's
+thresholds, with the compact spectra written to HBM, config 5 (100 sliding windows, p50 / p99) and
+the paper's own operating point -- the `sub` object of the line (`--no-sub` skips them).
 
 Prints ONE JSON line (rank 0).  `value` = (pixel x frequency x event) terms of the active
 pixels per step / device time per step, inputs resident in HBM.  `e2e` = the same through
@@ -36,7 +42,24 @@ sys.path.insert(0, ROOT)
 
 NOMINAL_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # 74.45: SMs x FP32 lanes x 2 flop x max SM clock
 FLOP_PER_TERM = 4.0                                        # one complex phasor accumulate = 2 FMA
-NDFT_DRAM_BYTES_NCU = 84.0e6                               # profiles/r1c_summary.md (config 4, no spectra output)
+TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r2_traffic.csv")   # dram__bytes per launch from committed ncu captures
+
+
+def traffic_of(kernel_prefixes, workload: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the kernels whose names start with
+    one of `kernel_prefixes`, from the committed ncu summary of this build (profiles/r2_traffic.csv,
+    written from `ncu --set full` / `--metrics dram__bytes_*` captures; profiles/r2_traffic.md names the
+    commands).  None when the table has no row for the workload: nothing is guessed."""
+    try:
+        tot, hit = 0.0, False
+        for line in open(TRAFFIC_CSV):
+            f = [x.strip() for x in line.split(",")]
+            if len(f) >= 4 and f[0] == workload and any(f[1].startswith(k) for k in kernel_prefixes):
+                tot += float(f[2]) + float(f[3])
+                hit = True
+        return tot if hit else None
+    except OSError:
+        return None
 
 
 class ClockSampler(threading.Thread):
@@ -157,6 +180,111 @@ def aggregate_over_ranks(time_ms: float, units: float, world: int, device="cpu")
     return float(t.item()), float(u.item())
 
 
+def measure(w, *, steps, warmup, dev, world=1, local_rank=0, score_all=False, spectra=False, params=None, name=""):
+    """Device-resident timing of `steps` windows of workload `w` (after `warmup`): whole-window CUDA-event
+    time, per-stage times, clocks sampled during the timed region.  Returns (record, detector state)."""
+    import torch
+    import torch.distributed as dist
+    from paper_2603_08386_b200 import binding
+    prm = dict(params or w.params)
+    # the stream stays resident; max_events = the largest window handed to ddhf_window
+    max_ev = len(w.events) if w.n_windows == 1 else max(w.window_slice(k)[1] for k in range(w.n_windows))
+    det = binding.Detector(prm, max_events=max_ev, score_all=score_all, timing=True, want_power=spectra, want_labels=False,
+                           device=f"cuda:{local_rank}",
+                           max_active=(prm["width"] * prm["height"]) if spectra else 1)
+    d_ev = det.upload(w.events)
+    wins = window_list(w, warmup + steps)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    # one untimed pass to count the terms of every distinct window (device counters only tell
+    # events and pixels; the term count needs the row lengths)
+    terms_by_win = {}
+    for lo, n, t0 in dict.fromkeys(wins):
+        det.window(d_ev, n, t0, w.window_us, offset_events=lo)
+        res = det.results()
+        terms_by_win[(lo, n, t0)] = (terms_of(res, prm["n_freq"], prm["n_min"]), res)
+    launches_per_window = binding.ddhf_launches_per_window(det.h)
+
+    for lo, n, t0 in wins[:warmup]:
+        det.window(d_ev, n, t0, w.window_us, offset_events=lo)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    per_step_ms, stage = [], []
+    # L2 hygiene: a step touches the events (16 B), the bucket-sorted items (4 B, written and read), csr_ev
+    # (4 B) and the per-pixel maps.  When that is below twice the 126 MB L2, a 256 MB buffer is written
+    # between steps (outside the timed intervals: one CUDA-event pair per step, their sum is the time).
+    n_ev_step = max(n for _, n, _ in wins[warmup:])
+    footprint = 28.0 * n_ev_step + 40.0 * prm["width"] * prm["height"]
+    flush = footprint < 2 * 126e6
+    scratch = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if flush else None
+    if flush:
+        pairs_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in wins[warmup:]]
+        for (e0, e1), (lo, n, t0) in zip(pairs_ev, wins[warmup:]):
+            scratch.fill_(1)
+            e0.record()
+            det.window(d_ev, n, t0, w.window_us, offset_events=lo)
+            e1.record()
+        barrier()
+        total_ms = float(sum(e0.elapsed_time(e1) for e0, e1 in pairs_ev))
+    else:
+        ev0 = torch.cuda.Event(enable_timing=True)
+        ev1 = torch.cuda.Event(enable_timing=True)
+        ev0.record()
+        for lo, n, t0 in wins[warmup:]:
+            det.window(d_ev, n, t0, w.window_us, offset_events=lo)
+        ev1.record()
+        barrier()
+        total_ms = ev0.elapsed_time(ev1)
+    # per-step latency and per-stage split: a second timed pass with a sync per window
+    for lo, n, t0 in wins[warmup:]:
+        if flush:
+            scratch.fill_(1)
+        det.window(d_ev, n, t0, w.window_us, offset_events=lo)
+        ms = det.stage_ms()
+        stage.append(ms)
+        per_step_ms.append(ms[4])
+    sampler.stop_flag.set()
+    sampler.join()
+    stage = np.array(stage)
+    terms_total = sum(terms_by_win[k][0] for k in wins[warmup:])
+    total_ms, terms_all = aggregate_over_ranks(total_ms, terms_total, world, dev)
+    res0 = terms_by_win[wins[warmup]][1]
+    ndft_ms = float(stage[:, 1].mean())
+    terms_per_step = terms_total / len(wins[warmup:])
+    rec = {
+        "name": name, "value": terms_all / (total_ms * 1e-3) / 1e9, "unit": "Gterms/s", "steps": steps, "warmup": warmup,
+        "ms_per_step": total_ms / steps,
+        "config": {"workload": f"{name}: {prm['width']}x{prm['height']} sensor, "
+                               f"{w.window_us / 1e3:.1f} ms window, {res0['n_in']} events, "
+                               f"{prm['n_freq']} bins, {prm['n_f0']} f0 candidates, H={prm['n_harm']}, "
+                               f"n_min={prm['n_min']}, tau_sf={prm['tau_sf']}, tau_comb={prm['tau_comb']}",
+                   "events_per_step": res0["n_in"], "active_pixels": res0["n_active"],
+                   "scored_pixels": res0["n_scored"], "terms_per_step": terms_per_step,
+                   "mask_pixels": int(res0["mask"].sum()), "boxes": res0["n_boxes"],
+                   "score_all": bool(score_all), "spectra_to_hbm": bool(spectra),
+                   "scoring_note": "the comb score is evaluated where SF <= tau_sf (PAPER.md L139 order) unless score_all: "
+                                   "thresholds change the work done, not only the mask",
+                   "l2": ("L2 flushed between steps (256 MB write, outside the timed intervals); step footprint %.0f MB"
+                          if flush else "step footprint %.0f MB (events + bucket-sorted items + csr + maps) exceeds the 126 MB L2")
+                         % (footprint / 1e6),
+                   "replicas": world},
+        "latency_ms": {"p50": float(np.percentile(per_step_ms, 50)), "p99": float(np.percentile(per_step_ms, 99)),
+                       "ingest": float(stage[:, 0].mean()), "ndft": ndft_ms, "comb_score": float(stage[:, 2].mean()),
+                       "ccl": float(stage[:, 3].mean())},
+        "ndft_frac_of_fp32_peak": terms_per_step * FLOP_PER_TERM / (ndft_ms * 1e-3) / 1e12 / NOMINAL_FP32_TFLOPS,
+        "clocks": sampler.summary(), "gpu_launches": launches_per_window * steps,
+    }
+    state = dict(det=det, d_ev=d_ev, wins=wins, terms_by_win=terms_by_win, stage=stage, terms_total=terms_total,
+                 barrier=barrier, prm=prm, launches_per_window=launches_per_window)
+    return rec, state
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -165,6 +293,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg4")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sub", action="store_true", help="skip the variant measurements (the `sub` object)")
     ap.add_argument("--score-all", action="store_true", help="comb score on every active pixel (R14)")
     ap.add_argument("--spectra", action="store_true", help="also write the compact power spectra to HBM")
     args = ap.parse_args()
@@ -205,74 +334,10 @@ def main():
         dist.init_process_group("nccl", device_id=dev)
 
     w = load_workload(args.workload)
-    prm = w.params
-    det = binding.Detector(prm, max_events=len(w.events), score_all=args.score_all, timing=True,
-                           want_power=args.spectra, want_labels=False, device=f"cuda:{local_rank}",
-                           max_active=(prm["width"] * prm["height"]) if args.spectra else 1)
-    d_ev = det.upload(w.events)
-    wins = window_list(w, warmup + steps)
-
-    def barrier():
-        torch.cuda.synchronize(dev)
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize(dev)
-
-    # one untimed pass to count the terms of every distinct window (device counters only tell
-    # events and pixels; the term count needs the row lengths)
-    terms_by_win = {}
-    for lo, n, t0 in dict.fromkeys(wins):
-        det.window(d_ev, n, t0, w.window_us, offset_events=lo)
-        res = det.results()
-        terms_by_win[(lo, n, t0)] = (terms_of(res, prm["n_freq"], prm["n_min"]), res)
-    launches_per_window = binding.ddhf_launches_per_window(det.h)
-
-    # ---- device-resident timing ---------------------------------------------------------------
-    for lo, n, t0 in wins[:warmup]:
-        det.window(d_ev, n, t0, w.window_us, offset_events=lo)
-    barrier()
-    sampler = ClockSampler(local_rank)
-    sampler.start()
-    per_step_ms, stage = [], []
-    # L2 hygiene: a step touches the events (16 B), the partition pairs (8 B, written and read), csr_ev
-    # (4 B) and the per-pixel maps.  When that is below twice the 126 MB L2, a 256 MB buffer is written
-    # between steps (outside the timed intervals: one CUDA-event pair per step, their sum is the time).
-    n_ev_step = max(n for _, n, _ in wins[warmup:])
-    footprint = 36.0 * n_ev_step + 40.0 * prm["width"] * prm["height"]
-    flush = footprint < 2 * 126e6
-    if flush:
-        scratch = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-        pairs_ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in wins[warmup:]]
-        for (e0, e1), (lo, n, t0) in zip(pairs_ev, wins[warmup:]):
-            scratch.fill_(1)
-            e0.record()
-            det.window(d_ev, n, t0, w.window_us, offset_events=lo)
-            e1.record()
-        barrier()
-        total_ms = float(sum(e0.elapsed_time(e1) for e0, e1 in pairs_ev))
-    else:
-        ev0 = torch.cuda.Event(enable_timing=True)
-        ev1 = torch.cuda.Event(enable_timing=True)
-        ev0.record()
-        for lo, n, t0 in wins[warmup:]:
-            det.window(d_ev, n, t0, w.window_us, offset_events=lo)
-        ev1.record()
-        barrier()
-        total_ms = ev0.elapsed_time(ev1)
-    # per-step latency and per-stage split: a second timed pass with a sync per window
-    for lo, n, t0 in wins[warmup:]:
-        if flush:
-            scratch.fill_(1)
-        det.window(d_ev, n, t0, w.window_us, offset_events=lo)
-        ms = det.stage_ms()
-        stage.append(ms)
-        per_step_ms.append(ms[4])
-    sampler.stop_flag.set()
-    sampler.join()
-    stage = np.array(stage)
-    terms_total = sum(terms_by_win[k][0] for k in wins[warmup:])
-    total_ms, terms_all = aggregate_over_ranks(total_ms, terms_total, world, dev)
-    value = terms_all / (total_ms * 1e-3) / 1e9
+    rec, st = measure(w, steps=steps, warmup=warmup, dev=dev, world=world, local_rank=local_rank,
+                      score_all=args.score_all, spectra=args.spectra, name=args.workload)
+    det, wins, terms_by_win, stage, prm = st["det"], st["wins"], st["terms_by_win"], st["stage"], st["prm"]
+    barrier = st["barrier"]
 
     # ---- end to end through the host-buffer entry points -------------------------------------------
     # e2e: ddhf_host_submit / ddhf_host_wait (two windows in flight: the 16 B/event host->device copy
@@ -290,20 +355,20 @@ def main():
         o.mask, o.boxes, o.counters = t[0].data_ptr(), t[1].data_ptr(), t[2].data_ptr()
         hbufs.append(t)
         houts.append(o)
-    st = torch.cuda.current_stream(dev).cuda_stream
+    cst = torch.cuda.current_stream(dev).cuda_stream
     e2e_steps = min(steps, 10)
     e2e_wins = wins[warmup:warmup + e2e_steps]
 
     def run_pipelined(ws):
         for i, (lo, n, t0) in enumerate(ws):
-            binding.ddhf_host_submit(det.h, h_ev.data_ptr() + 16 * lo, n, t0, w.window_us, houts[i & 1], st)
+            binding.ddhf_host_submit(det.h, h_ev.data_ptr() + 16 * lo, n, t0, w.window_us, houts[i & 1], cst)
             if i >= 1:
                 binding.ddhf_host_wait(det.h)
         binding.ddhf_host_wait(det.h)
 
     def run_serial(ws):
         for lo, n, t0 in ws:
-            binding.ddhf_window_host(det.h, h_ev.data_ptr() + 16 * lo, n, t0, w.window_us, houts[0], st)
+            binding.ddhf_window_host(det.h, h_ev.data_ptr() + 16 * lo, n, t0, w.window_us, houts[0], cst)
 
     e2e_terms = sum(terms_by_win[k][0] for k in e2e_wins)
     h2d = sum(16 * n for _, n, _ in e2e_wins)
@@ -337,57 +402,73 @@ def main():
     ing_ms = float(stage[:, 0].mean())
     ing_bytes = 20.0 * n_ev + 8.0 * prm["width"] * prm["height"]          # 16 B read + 4 B written per event, 8 B per pixel
     roofline_stages = {
-        "ingest": {"bound": "hbm", "kernels": "k_dhist/k_binscan/k_part x2 + k_scan_*", "achieved": ing_bytes / (ing_ms * 1e-3) / 1e9,
+        "ingest": {"bound": "hbm", "kernels": "k_init, k_tile_sort, k_bucket_sort, k_scan_reduce/tiles/apply",
+                   "achieved": ing_bytes / (ing_ms * 1e-3) / 1e9,
                    "peak": hbm_peak, "unit": "GB/s", "frac": ing_bytes / (ing_ms * 1e-3) / 1e9 / hbm_peak,
                    "algorithmic_bytes": ing_bytes, "ms": ing_ms, "peak_kind": hbm_kind,
-                   "note": "a two-pass stable partition moves 60 B per event; the ranking step is instruction-bound"},
+                   "traffic": traffic_of(("k_init", "k_tile_sort", "k_bucket_sort", "k_scan_"), args.workload),
+                   "traffic_source": "sum of dram__bytes_read.sum + dram__bytes_write.sum of the ingest kernels, one launch each "
+                                     "(profiles/r2_traffic.csv)",
+                   "note": "events are read once (16 B), bucket-sorted 4-byte items written and read once, csr_ev written; "
+                           "both sort kernels are bound by shared-memory bandwidth and latency, not by HBM"},
     }
 
     # ---- roofline of the dominant kernel (k_ndft_score), measured live ----------------------------
     ndft_ms = float(stage[:, 1].mean())
-    terms_per_step = terms_total / len(wins[warmup:])
+    terms_per_step = st["terms_total"] / len(wins[warmup:])
     achieved = terms_per_step * FLOP_PER_TERM / (ndft_ms * 1e-3) / 1e12
     probe = binding.ddhf_fma_peak_probe(20.0)
     roofline = {"bound": "alu", "kernel": "k_ndft_score", "achieved": achieved, "peak": NOMINAL_FP32_TFLOPS,
                 "unit": "TFLOP/s", "frac": achieved / NOMINAL_FP32_TFLOPS,
-                "traffic": NDFT_DRAM_BYTES_NCU if args.workload == "cfg4" and not args.spectra else None,
-                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture "
-                                  "(profiles/), config 4, per launch",
+                "traffic": traffic_of(("k_ndft_score",), args.workload) if not args.spectra else None,
+                "traffic_source": "dram__bytes_read.sum + dram__bytes_write.sum of one ncu --set full capture of this build "
+                                  "(profiles/r2_traffic.csv), per launch",
                 "peak_kind": "nominal FP32 FMA: 148 SM x 128 lanes x 2 flop x 1.965 GHz (DESIGN.md section 5)",
                 "flop_per_term": FLOP_PER_TERM, "kernel_ms": ndft_ms,
                 "gterms_per_s_kernel": terms_per_step / (ndft_ms * 1e-3) / 1e9,
                 "measured_fma_peak_tflops": {"ffma": probe[0], "ffma2": probe[1]},
                 "frac_of_measured_fma_peak": achieved / max(probe)}
-    res0 = terms_by_win[wins[warmup]][1]
     line = {
-        "metric": "ndft_gterms_per_s", "value": value, "unit": "Gterms/s", "n_gpus": world,
-        "steps": steps, "warmup": warmup, "ms_per_step": total_ms / steps, "higher_is_better": True,
+        "metric": "ndft_gterms_per_s", "value": rec["value"], "unit": "Gterms/s", "n_gpus": world,
+        "steps": steps, "warmup": warmup, "ms_per_step": rec["ms_per_step"], "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"{args.workload}: {prm['width']}x{prm['height']} sensor, "
-                               f"{w.window_us / 1e3:.0f} ms window, {res0['n_in']} events, "
-                               f"{prm['n_freq']} bins, {prm['n_f0']} f0 candidates, H={prm['n_harm']}, "
-                               f"n_min={prm['n_min']}",
-                   "events_per_step": res0["n_in"], "active_pixels": res0["n_active"],
-                   "scored_pixels": res0["n_scored"], "terms_per_step": terms_per_step,
-                   "mask_pixels": int(res0["mask"].sum()), "boxes": res0["n_boxes"],
-                   "score_all": bool(args.score_all), "spectra_to_hbm": bool(args.spectra),
-                   "l2": ("L2 flushed between steps (256 MB write, outside the timed intervals); step footprint %.0f MB"
-                          if flush else "step footprint %.0f MB (events + partition pairs + csr + maps) exceeds the 126 MB L2")
-                         % (footprint / 1e6),
-                   "replicas": world},
-        "latency_ms": {"p50": float(np.percentile(per_step_ms, 50)), "p99": float(np.percentile(per_step_ms, 99)),
-                       "ingest": float(stage[:, 0].mean()), "ndft": ndft_ms, "comb_score": float(stage[:, 2].mean()),
-                       "ccl": float(stage[:, 3].mean())},
-        "clocks": sampler.summary(), "e2e": e2e, "e2e_serial": e2e_serial, "gpu_launches": launches_per_window * steps,
+        "config": rec["config"], "latency_ms": rec["latency_ms"],
+        "clocks": rec["clocks"], "e2e": e2e, "e2e_serial": e2e_serial, "gpu_launches": rec["gpu_launches"],
         "roofline": roofline, "roofline_stages": roofline_stages,
         "paper_context": "DDHF 2.39 ms/frame, YOLOv11-n 12.40 ms/frame on an NVIDIA L40-8Q, 33.3 ms windows (PAPER.md L154-156)",
     }
+    det.close()
+    del h_ev, hbufs, st
+    torch.cuda.empty_cache()
+
+    # ---- the variants of SURVEY.md section 8(d), each with its own clocks ------------------------------
+    if world == 1 and not args.no_sub and args.workload == "cfg4":
+        from paper_2603_08386_b200 import workloads
+        sub = {}
+        sub_steps = min(steps, 10)
+
+        def run_sub(key, wl_, **kw):
+            r, s_ = measure(wl_, steps=kw.pop("steps", sub_steps), warmup=3, dev=dev, local_rank=local_rank, name=key, **kw)
+            s_["det"].close()
+            del s_
+            torch.cuda.empty_cache()
+            sub[key] = r
+
+        run_sub("cfg4_score_all", w, score_all=True)
+        run_sub("cfg4_table2_thresholds", w, params=dict(w.params, tau_sf=0.89, tau_comb=1.5))
+        run_sub("cfg4_spectra_to_hbm", w, spectra=True)
+        run_sub("paper_point", workloads.paper_native())
+        run_sub("cfg3", workloads.make(3))
+        w5 = workloads.make(5, n_windows=100)
+        run_sub("cfg5_stream_100_windows", w5, steps=100)
+        line["sub"] = sub
+
     if not args.no_cpu_baseline:
-        r = time_oracle(w, 2, 0, crop=(640, 360))      # ~10 s of CPU work
+        full = args.workload in ("cfg4", "cfg3", "paper")
+        r = time_oracle(w, 1, 0, crop=(w.width, w.height) if full else (640, 360))      # cfg4: ~27 s on 16 cores
         line["cpu_baseline"] = {"value": r["value"], "unit": "Gterms/s", "cores": r["cores"], "kind": "oracle",
                                 "sample": r["sample"], "ms": r["ms_per_step"]}
     print(json.dumps(line))
-    det.close()
     if world > 1:
         dist.destroy_process_group()
 

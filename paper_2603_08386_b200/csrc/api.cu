@@ -31,7 +31,7 @@ struct ddhf_handle {
     int ndft_blocks_per_sm = 1, score_blocks_per_sm = 1;
     // workspace offsets (bytes)
     size_t off_cnt = 0, off_items = 0, off_scratch = 0, off_work = 0, off_tiles = 0, off_class = 0, off_cursor = 0, off_runs = 0, off_bkt = 0, off_rows = 0, off_spill = 0, off_spillrec = 0,
-           off_parent = 0, off_rec = 0, off_ctiles = 0, off_split = 0, off_splitcnt = 0, off_partial = 0, ws_bytes = 0;
+           off_parent = 0, off_rec = 0, off_ctiles = 0, off_merge = 0, off_split = 0, off_splitcnt = 0, off_partial = 0, ws_bytes = 0;
     cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     bool timed_once = false;
     // buffers of the host-buffer variant
@@ -100,8 +100,6 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
         return fail(nullptr, DDHF_E_INVAL, "ddhf_create: k_lo / sf_eps out of range");
     if (c.max_events < 1 || c.max_events >= (1ll << 31) || c.max_active < 1 || c.max_boxes < 1)
         return fail(nullptr, DDHF_E_INVAL, "ddhf_create: capacities out of range");
-    if (c.merge_alpha > 0.f && c.max_boxes > 8192)
-        return fail(nullptr, DDHF_E_INVAL, "ddhf_create: box merge (merge_alpha > 0) supports max_boxes <= 8192");
 
     ddhf_handle *h = new (std::nothrow) ddhf_handle();
     if (!h) return fail(nullptr, DDHF_E_NOMEM, "ddhf_create: out of host memory");
@@ -211,7 +209,7 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
         h->sp.meta = reinterpret_cast<const uint4 *>(h->d_tables + off_meta);
     }
     h->band_size = band_size;
-    if (ingest_configure() != cudaSuccess || (c.merge_alpha > 0.f && ccl_configure(c.max_boxes) != cudaSuccess) ||
+    if (ingest_configure() != cudaSuccess ||
         ndft_configure(c.n_freq, band_size, cpad, &h->ndft_blocks_per_sm, &h->score_blocks_per_sm) != cudaSuccess) {
         const std::string msg = std::string("ddhf_create: ") + cudaGetErrorString(cudaGetLastError());
         cudaFree(h->d_tables);
@@ -272,6 +270,7 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
     h->off_parent = o;     o = align_up(o + sizeof(int32_t) * h->np);
     h->off_rec = o;        o = align_up(o + sizeof(int32_t) * 5 * static_cast<size_t>(h->np));
     h->off_ctiles = o;     o = align_up(o + sizeof(int32_t) * 1024);
+    h->off_merge = o;      o = align_up(o + sizeof(int32_t) * 6 * static_cast<size_t>(c.max_boxes));
     h->ws_bytes = o;
 
     if (c.flags & DDHF_FLAG_TIMING)
@@ -326,7 +325,7 @@ extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n
     ip.bkt_base = ip.bkt_total + h->nb + 2;
     ip.bkt_order = ip.bkt_base + h->nb + 2;
     ip.chunk_rows = reinterpret_cast<int32_t *>(ws + h->off_rows);
-    ip.sync = reinterpret_cast<int32_t *>(ws + h->off_cursor + 16);       // [8]; the scoring queue counts are sync[2..3]
+    ip.sync = reinterpret_cast<int32_t *>(ws + h->off_cursor + 16);       // [16]; the scoring queue counts are sync[2..3]
 
     ip.split_tab = reinterpret_cast<SplitRow *>(ws + h->off_split);
     ip.split_cnt = reinterpret_cast<int32_t *>(ws + h->off_splitcnt);
@@ -356,6 +355,9 @@ extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n
     cp.boxes = out->boxes; cp.counters = out->counters;
     cp.merged = (c.merge_alpha > 0.f) ? out->merged_boxes : nullptr;
     cp.merge_alpha = c.merge_alpha;
+    cp.merge_parent = cp.merged ? reinterpret_cast<int32_t *>(ws + h->off_merge) : nullptr;
+    cp.merge_rec = cp.merge_parent ? cp.merge_parent + c.max_boxes : nullptr;
+    cp.merge_sync = ip.sync + 8;
 
     int launches = 0;
     if (timing) cudaEventRecord(h->ev[0], st);

@@ -15,7 +15,7 @@
 //   k_ccl_label     parent[i] = root (labels; -1 off the mask); box record of the root updated
 //   k_ccl_count     per tile of 4096 pixels: roots, and roots whose box passes A_min
 //   k_ccl_emit      ordered compaction of the passing roots into boxes[] (ascending label)
-//   k_box_merge     (optional) eq. 12: boxes with close centres merged into the final detections
+//   k_box_merge_pairs   (optional) eq. 12: boxes with close centres merged into the final detections
 #include "ddhf_internal.cuh"
 
 namespace ddhf {
@@ -198,6 +198,7 @@ __global__ void __launch_bounds__(1024) k_ccl_emit(CclParams p, int n_tiles)
             b.x0 = c[0]; b.y0 = c[1]; b.x1 = c[2]; b.y1 = c[3]; b.n_pix = c[4];
             b.label = i;
             p.boxes[pos] = b;
+            if (p.merge_parent) p.merge_parent[pos] = pos;       // every box starts as its own detection (eq. 12 merge)
         }
         ++pos;
     }
@@ -205,11 +206,15 @@ __global__ void __launch_bounds__(1024) k_ccl_emit(CclParams p, int n_tiles)
 
 // ---- a9: box merge, eq. 12 ---------------------------------------------------
 // "two boxes ... are merged if dist(c1, c2) < alpha max(w1, h1, w2, h2)".  Readings R27-R29: box
-// centres, the rule evaluated on the boxes that entered the step, merging transitive.  A handful of
-// boxes: one CTA, union-find over box indices in shared memory (root = smallest index = smallest
-// label, since boxes[] is ascending by label), all pairs tested in double precision with the same
-// expression as the oracle.
+// centres, the rule evaluated on the boxes that entered the step, merging transitive.  Every pair is
+// tested in double precision with the same expression as the oracle; the pair matrix is cut into
+// 64 x 64 tiles spread over the grid (4096 boxes = 8.4 M pairs: one CTA needed 52 ms), pairs that pass
+// are united in a union-find over box indices in the workspace (root = smallest index = smallest label,
+// since boxes[] is ascending by label), and one CTA emits the roots in order.
 constexpr int kMergeThreads = 256;
+constexpr int kMergeTile = 64;
+
+constexpr int kMergeSmall = 128;      // up to this many boxes one CTA does the whole step in shared memory
 
 __device__ __forceinline__ int mg_find(volatile int *par, int x)
 {
@@ -218,31 +223,24 @@ __device__ __forceinline__ int mg_find(volatile int *par, int x)
     return x;
 }
 
-__global__ void __launch_bounds__(kMergeThreads) k_box_merge(CclParams p)
+// The usual case, a handful of boxes: all pairs, union-find, records and ordered emit by one CTA in
+// shared memory (a few microseconds; the general path below costs three times that in global atomics).
+__device__ __forceinline__ void merge_small(const CclParams &p, int n)
 {
-    extern __shared__ int s_par[];                       // [n] parents, then [n][5] merged records
-    __shared__ int s_out;
-    const int n = min(p.counters[DDHF_CNT_N_BOXES], p.max_boxes);
-    int *s_rec = s_par + n;
-    for (int i = threadIdx.x; i < n; i += kMergeThreads) s_par[i] = i;
-    if (threadIdx.x == 0) s_out = 0;
+    __shared__ int s_par[kMergeSmall], s_rec[kMergeSmall][5];
+    for (int i = threadIdx.x; i < n; i += kMergeThreads) {
+        s_par[i] = i;
+        s_rec[i][0] = 0x7fffffff; s_rec[i][1] = 0x7fffffff; s_rec[i][2] = -1; s_rec[i][3] = -1; s_rec[i][4] = 0;
+    }
     __syncthreads();
     const double alpha = static_cast<double>(p.merge_alpha);
-    const long long n_pairs = static_cast<long long>(n) * (n - 1) / 2;
-    for (long long q = threadIdx.x; q < n_pairs; q += kMergeThreads) {
-        // pair (i, j), i < j, from the linear index q = j (j - 1) / 2 + i
-        int j = static_cast<int>((1.0 + sqrt(1.0 + 8.0 * static_cast<double>(q))) * 0.5);
-        while (static_cast<long long>(j) * (j - 1) / 2 > q) --j;
-        while (static_cast<long long>(j + 1) * j / 2 <= q) ++j;
-        const int i = static_cast<int>(q - static_cast<long long>(j) * (j - 1) / 2);
+    for (int q = threadIdx.x; q < n * n; q += kMergeThreads) {
+        const int i = q / n, j = q % n;
+        if (i >= j) continue;
         const ddhf_box a = p.boxes[i], b = p.boxes[j];
-        const double cxa = 0.5 * (a.x0 + a.x1), cya = 0.5 * (a.y0 + a.y1);
-        const double cxb = 0.5 * (b.x0 + b.x1), cyb = 0.5 * (b.y0 + b.y1);
-        const double dist = sqrt((cxa - cxb) * (cxa - cxb) + (cya - cyb) * (cya - cyb));
-        double m = a.x1 - a.x0 + 1;
-        if (a.y1 - a.y0 + 1 > m) m = a.y1 - a.y0 + 1;
-        if (b.x1 - b.x0 + 1 > m) m = b.x1 - b.x0 + 1;
-        if (b.y1 - b.y0 + 1 > m) m = b.y1 - b.y0 + 1;
+        const double dx = 0.5 * (a.x0 + a.x1) - 0.5 * (b.x0 + b.x1), dy = 0.5 * (a.y0 + a.y1) - 0.5 * (b.y0 + b.y1);
+        const double dist = sqrt(dx * dx + dy * dy);
+        const double m = static_cast<double>(max(max(a.x1 - a.x0 + 1, a.y1 - a.y0 + 1), max(b.x1 - b.x0 + 1, b.y1 - b.y0 + 1)));
         if (dist < alpha * m) {
             int x = i, y = j;
             while (true) {                               // unite: larger root under the smaller
@@ -258,29 +256,21 @@ __global__ void __launch_bounds__(kMergeThreads) k_box_merge(CclParams p)
     }
     __syncthreads();
     for (int i = threadIdx.x; i < n; i += kMergeThreads) {
-        int *c = s_rec + 5 * i;
-        c[0] = 0x7fffffff; c[1] = 0x7fffffff; c[2] = -1; c[3] = -1; c[4] = 0;
-    }
-    __syncthreads();
-    for (int i = threadIdx.x; i < n; i += kMergeThreads) {
         const int r = mg_find(s_par, i);
         const ddhf_box b = p.boxes[i];
-        int *c = s_rec + 5 * r;
-        atomicMin(c + 0, b.x0);
-        atomicMin(c + 1, b.y0);
-        atomicMax(c + 2, b.x1);
-        atomicMax(c + 3, b.y1);
-        atomicAdd(c + 4, b.n_pix);
+        atomicMin(&s_rec[r][0], b.x0);
+        atomicMin(&s_rec[r][1], b.y0);
+        atomicMax(&s_rec[r][2], b.x1);
+        atomicMax(&s_rec[r][3], b.y1);
+        atomicAdd(&s_rec[r][4], b.n_pix);
     }
     __syncthreads();
-    // ordered emit: roots in ascending index (= ascending label); one thread walks them (n is small)
-    if (threadIdx.x == 0) {
+    if (threadIdx.x == 0) {                              // roots in ascending index = ascending label
         int k = 0;
         for (int i = 0; i < n; ++i) {
             if (s_par[i] != i) continue;
-            const int *c = s_rec + 5 * i;
             ddhf_box b;
-            b.x0 = c[0]; b.y0 = c[1]; b.x1 = c[2]; b.y1 = c[3]; b.n_pix = c[4];
+            b.x0 = s_rec[i][0]; b.y0 = s_rec[i][1]; b.x1 = s_rec[i][2]; b.y1 = s_rec[i][3]; b.n_pix = s_rec[i][4];
             b.label = p.boxes[i].label;
             p.merged[k++] = b;
         }
@@ -288,13 +278,114 @@ __global__ void __launch_bounds__(kMergeThreads) k_box_merge(CclParams p)
     }
 }
 
+__global__ void __launch_bounds__(kMergeThreads) k_box_merge_pairs(CclParams p)
+{
+    __shared__ double s_cx[2][kMergeTile], s_cy[2][kMergeTile], s_m[2][kMergeTile];
+    const int n = min(p.counters[DDHF_CNT_N_BOXES], p.max_boxes);
+    if (n <= kMergeSmall) {
+        if (blockIdx.x == 0) merge_small(p, n);
+        return;
+    }
+    const int nt = (n + kMergeTile - 1) / kMergeTile;
+    const int n_tiles = nt * (nt + 1) / 2;
+    const double alpha = static_cast<double>(p.merge_alpha);
+    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        // tile (ti, tj), ti <= tj, from the linear index tile = tj (tj + 1) / 2 + ti
+        int tj = static_cast<int>((sqrt(8.0 * tile + 1.0) - 1.0) * 0.5);
+        while (tj * (tj + 1) / 2 > tile) --tj;
+        while ((tj + 1) * (tj + 2) / 2 <= tile) ++tj;
+        const int ti = tile - tj * (tj + 1) / 2;
+        __syncthreads();
+        if (threadIdx.x < 2 * kMergeTile) {
+            const int side = threadIdx.x / kMergeTile, k = threadIdx.x % kMergeTile;
+            const int idx = (side ? tj : ti) * kMergeTile + k;
+            if (idx < n) {
+                const ddhf_box b = p.boxes[idx];
+                s_cx[side][k] = 0.5 * (b.x0 + b.x1);
+                s_cy[side][k] = 0.5 * (b.y0 + b.y1);
+                s_m[side][k] = static_cast<double>(max(b.x1 - b.x0 + 1, b.y1 - b.y0 + 1));
+            }
+        }
+        __syncthreads();
+        for (int q = threadIdx.x; q < kMergeTile * kMergeTile; q += kMergeThreads) {
+            const int a = q / kMergeTile, b = q % kMergeTile;
+            const int i = ti * kMergeTile + a, j = tj * kMergeTile + b;
+            if (i >= j || j >= n) continue;
+            const double dx = s_cx[0][a] - s_cx[1][b], dy = s_cy[0][a] - s_cy[1][b];
+            const double dist = sqrt(dx * dx + dy * dy);
+            const double m = s_m[0][a] > s_m[1][b] ? s_m[0][a] : s_m[1][b];
+            if (dist < alpha * m && uf_find(p.merge_parent, i) != uf_find(p.merge_parent, j))
+                uf_union(p.merge_parent, i, j);
+        }
+    }
+    // the last CTA to finish emits the roots in ascending index (= ascending label) with the union of
+    // their members' boxes
+    __shared__ int s_w[33];
+    __shared__ bool s_last;
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = (atomicAdd(p.merge_sync, 1) == static_cast<int>(gridDim.x) - 1);
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    constexpr int NT = kMergeThreads;
+    int *rec = p.merge_rec;
+    for (int i = threadIdx.x; i < n; i += NT) {
+        int *c = rec + 5 * i;
+        c[0] = 0x7fffffff; c[1] = 0x7fffffff; c[2] = -1; c[3] = -1; c[4] = 0;
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < n; i += NT) {
+        const int r = uf_find(p.merge_parent, i);
+        const ddhf_box b = p.boxes[i];
+        int *c = rec + 5 * r;
+        atomicMin(c + 0, b.x0);
+        atomicMin(c + 1, b.y0);
+        atomicMax(c + 2, b.x1);
+        atomicMax(c + 3, b.y1);
+        atomicAdd(c + 4, b.n_pix);
+    }
+    __syncthreads();
+    // ordered emit: thread t owns a contiguous range of box indices; exclusive scan of the root counts
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int per = (n + NT - 1) / NT;
+    const int beg = min(threadIdx.x * per, n), end = min(beg + per, n);
+    int cnt = 0;
+    for (int i = beg; i < end; ++i) cnt += (__ldcg(p.merge_parent + i) >= i);
+    int inc = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int v = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += v;
+    }
+    if (lane == 31) s_w[wid] = inc;
+    __syncthreads();
+    if (wid == 0) {
+        const int w = (lane < NT / 32) ? s_w[lane] : 0;
+        int x = w;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int v = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += v;
+        }
+        s_w[lane] = x - w;
+        if (lane == 31) s_w[32] = x;
+    }
+    __syncthreads();
+    int k = inc - cnt + s_w[wid];
+    for (int i = beg; i < end; ++i) {
+        if (__ldcg(p.merge_parent + i) < i) continue;
+        const int *c = rec + 5 * i;
+        ddhf_box b;
+        b.x0 = c[0]; b.y0 = c[1]; b.x1 = c[2]; b.y1 = c[3]; b.n_pix = c[4];
+        b.label = p.boxes[i].label;
+        p.merged[k++] = b;
+    }
+    if (threadIdx.x == 0) p.counters[DDHF_CNT_N_MERGED] = s_w[32];
+}
+
 }  // namespace
 
-cudaError_t ccl_configure(int max_boxes)
-{
-    return cudaFuncSetAttribute(k_box_merge, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                static_cast<int>(static_cast<size_t>(max_boxes) * 6 * sizeof(int)));
-}
 
 int launch_ccl(const CclParams &p, cudaStream_t st)
 {
@@ -306,7 +397,9 @@ int launch_ccl(const CclParams &p, cudaStream_t st)
     k_ccl_count<<<n_tiles, 1024, 0, st>>>(p); ++launches;
     k_ccl_emit<<<n_tiles, 1024, 0, st>>>(p, n_tiles); ++launches;
     if (p.merged != nullptr) {
-        k_box_merge<<<1, kMergeThreads, static_cast<size_t>(p.max_boxes) * 6 * sizeof(int), st>>>(p); ++launches;
+        const int nt = (p.max_boxes + kMergeTile - 1) / kMergeTile;
+        const int pair_tiles = nt * (nt + 1) / 2;
+        k_box_merge_pairs<<<pair_tiles < 296 ? pair_tiles : 296, kMergeThreads, 0, st>>>(p); ++launches;
     }
     return launches;
 }

@@ -111,8 +111,8 @@ struct IngestParams {
     int32_t *bkt_order;          // [nb] buckets by descending size class
     int32_t *bkt_total, *bkt_base;   // [nb + 2] events per bucket; exclusive scan (bkt_base[nb] = n_in)
     int32_t *chunk_rows;         // [max_rows][4 + 2^bl] chunk table of the multi-chunk buckets
-    int32_t *sync;               // [8] 0: tiles finished, 1: chunk rows handed out, 2-3: scoring queue counts,
-                                 //     4: work items, 5: split rows, 6: partials, 7: arrival counters handed out
+    int32_t *sync;               // [16] 0: tiles finished, 1: chunk rows handed out, 2-3: scoring queue counts,
+                                 //     4: work items, 5: split rows, 6: partials, 7: arrival counters handed out, 8: box-merge CTAs finished
     SplitRow *split_tab;         // rows longer than kSplitMin (see NdftParams)
     int32_t *split_cnt;
     int32_t *active_idx;
@@ -139,6 +139,9 @@ struct CclParams {
     ddhf_box *boxes;
     int32_t *counters;
     ddhf_box *merged;            // optional: eq. 12 detections
+    int32_t *merge_parent;       // [max_boxes] union-find over box indices (eq. 12), set by k_ccl_emit
+    int32_t *merge_rec;          // [max_boxes][5] merged box records
+    int32_t *merge_sync;         // CTAs of k_box_merge_pairs that have finished (zeroed by the ingest stage)
     float merge_alpha;
 };
 
@@ -153,7 +156,6 @@ void ingest_plan(int np, int *bl, int *nb, int *hbits);   // digit split for a s
 int launch_ndft(const NdftParams &p, int n_freq, int band_size, int grid_ndft, int grid_score, cudaStream_t st, cudaEvent_t between);
                                              // `between` (optional) is recorded after the NDFT kernel, before the scoring kernel
 int launch_ccl(const CclParams &p, cudaStream_t st);
-cudaError_t ccl_configure(int max_boxes);    // shared memory of the box-merge kernel
 int ndft_bins_per_lane(int n_freq);          // 8, 16, 32 or 64
 int ndft_tn(int n_freq);                     // offset pairs per centre for that kernel
 int ndft_padded_bins(int n_freq);            // row length of the deferred-scoring queue

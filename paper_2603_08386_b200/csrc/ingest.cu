@@ -97,7 +97,7 @@ __global__ void k_init(IngestParams p)
             p.class_cnt[threadIdx.x] = 0;
             p.class_cur[threadIdx.x] = 0;
         }
-        if (threadIdx.x < 8) p.sync[threadIdx.x] = 0;
+        if (threadIdx.x < 16) p.sync[threadIdx.x] = 0;
         if (threadIdx.x == 0) *p.work_cursor = 0ull;
     }
 }
