@@ -180,7 +180,8 @@ def aggregate_over_ranks(time_ms: float, units: float, world: int, device="cpu")
     return float(t.item()), float(u.item())
 
 
-def measure(w, *, steps, warmup, dev, world=1, local_rank=0, score_all=False, spectra=False, params=None, name=""):
+def measure(w, *, steps, warmup, dev, world=1, local_rank=0, score_all=False, spectra=False, params=None, name="",
+            slide=False):
     """Device-resident timing of `steps` windows of workload `w` (after `warmup`): whole-window CUDA-event
     time, per-stage times, clocks sampled during the timed region.  Returns (record, detector state)."""
     import torch
@@ -210,8 +211,23 @@ def measure(w, *, steps, warmup, dev, world=1, local_rank=0, score_all=False, sp
         terms_by_win[(lo, n, t0)] = (terms_of(res, prm["n_freq"], prm["n_min"]), res)
     launches_per_window = binding.ddhf_launches_per_window(det.h)
 
+    prev = {"hi": None, "t0": None}
+
+    def run_window(lo, n, t0):
+        """One step: ddhf_window on the slice, or (slide) ddhf_window_slide on the events that follow the
+        previous step's slice; a step whose t0 does not continue the sequence restarts it from scratch."""
+        if not slide:
+            det.window(d_ev, n, t0, w.window_us, offset_events=lo)
+            return
+        hi = lo + n
+        if prev["hi"] is not None and 0 <= t0 - prev["t0"] < w.window_us:
+            det.slide(d_ev, hi - prev["hi"], t0, w.window_us, offset_events=prev["hi"])
+        else:
+            det.slide(d_ev, n, t0, w.window_us, offset_events=lo)
+        prev["hi"], prev["t0"] = hi, t0
+
     for lo, n, t0 in wins[:warmup]:
-        det.window(d_ev, n, t0, w.window_us, offset_events=lo)
+        run_window(lo, n, t0)
     barrier()
     sampler = ClockSampler(local_rank)
     sampler.start()
@@ -228,7 +244,7 @@ def measure(w, *, steps, warmup, dev, world=1, local_rank=0, score_all=False, sp
         for (e0, e1), (lo, n, t0) in zip(pairs_ev, wins[warmup:]):
             scratch.fill_(1)
             e0.record()
-            det.window(d_ev, n, t0, w.window_us, offset_events=lo)
+            run_window(lo, n, t0)
             e1.record()
         barrier()
         total_ms = float(sum(e0.elapsed_time(e1) for e0, e1 in pairs_ev))
@@ -237,7 +253,7 @@ def measure(w, *, steps, warmup, dev, world=1, local_rank=0, score_all=False, sp
         ev1 = torch.cuda.Event(enable_timing=True)
         ev0.record()
         for lo, n, t0 in wins[warmup:]:
-            det.window(d_ev, n, t0, w.window_us, offset_events=lo)
+            run_window(lo, n, t0)
         ev1.record()
         barrier()
         total_ms = ev0.elapsed_time(ev1)
@@ -245,7 +261,7 @@ def measure(w, *, steps, warmup, dev, world=1, local_rank=0, score_all=False, sp
     for lo, n, t0 in wins[warmup:]:
         if flush:
             scratch.fill_(1)
-        det.window(d_ev, n, t0, w.window_us, offset_events=lo)
+        run_window(lo, n, t0)
         ms = det.stage_ms()
         stage.append(ms)
         per_step_ms.append(ms[4])
@@ -268,6 +284,9 @@ def measure(w, *, steps, warmup, dev, world=1, local_rank=0, score_all=False, sp
                    "scored_pixels": res0["n_scored"], "terms_per_step": terms_per_step,
                    "mask_pixels": int(res0["mask"].sum()), "boxes": res0["n_boxes"],
                    "score_all": bool(score_all), "spectra_to_hbm": bool(spectra),
+                   "ingest_mode": ("ddhf_window_slide: only the events that follow the previous window are sorted; the "
+                                   "sequence restarts from scratch when the window list wraps around") if slide
+                                  else "ddhf_window: every window bucketed from scratch",
                    "scoring_note": "the comb score is evaluated where SF <= tau_sf (PAPER.md L139 order) unless score_all: "
                                    "thresholds change the work done, not only the mask",
                    "l2": ("L2 flushed between steps (256 MB write, outside the timed intervals); step footprint %.0f MB"
@@ -296,6 +315,7 @@ def main():
     ap.add_argument("--no-sub", action="store_true", help="skip the variant measurements (the `sub` object)")
     ap.add_argument("--score-all", action="store_true", help="comb score on every active pixel (R14)")
     ap.add_argument("--spectra", action="store_true", help="also write the compact power spectra to HBM")
+    ap.add_argument("--slide", action="store_true", help="streaming workloads: ddhf_window_slide (incremental CSR)")
     args = ap.parse_args()
     steps, warmup = max(args.steps, 1), max(args.warmup, 3 if args.impl == "ours" else 0)
 
@@ -335,7 +355,7 @@ def main():
 
     w = load_workload(args.workload)
     rec, st = measure(w, steps=steps, warmup=warmup, dev=dev, world=world, local_rank=local_rank,
-                      score_all=args.score_all, spectra=args.spectra, name=args.workload)
+                      score_all=args.score_all, spectra=args.spectra, name=args.workload, slide=args.slide)
     det, wins, terms_by_win, stage, prm = st["det"], st["wins"], st["terms_by_win"], st["stage"], st["prm"]
     barrier = st["barrier"]
 
@@ -461,6 +481,7 @@ def main():
         run_sub("cfg3", workloads.make(3))
         w5 = workloads.make(5, n_windows=100)
         run_sub("cfg5_stream_100_windows", w5, steps=100)
+        run_sub("cfg5_stream_100_windows_slide", w5, steps=100, slide=True)
         line["sub"] = sub
 
     if not args.no_cpu_baseline:

@@ -58,7 +58,8 @@ extern "C" {
 #define DDHF_CNT_N_ACTIVE      2  /* pixels with >= n_min events (before truncation)       */
 #define DDHF_CNT_N_BOXES       3  /* boxes written (<= max_boxes)                          */
 #define DDHF_CNT_N_BOXES_TOTAL 4  /* components that passed A_min                          */
-#define DDHF_CNT_OVERFLOW      5  /* bit 0: n_active > max_active, bit 1: boxes > max_boxes */
+#define DDHF_CNT_OVERFLOW      5  /* bit 0: n_active > max_active, bit 1: boxes > max_boxes,
+                                     bit 2: sliding window > max_events                   */
 #define DDHF_CNT_N_SCORED      6  /* active pixels on which the comb score was evaluated   */
 #define DDHF_CNT_N_COMPONENTS  7  /* connected components before the A_min filter          */
 #define DDHF_CNT_N_MERGED      8  /* detections written to merged_boxes (eq. 12)           */
@@ -161,6 +162,22 @@ size_t ddhf_workspace_bytes(const ddhf_handle *h);
 int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n, int64_t t0_us,
                 int64_t window_us, void *d_workspace, const ddhf_outputs *out,
                 void *cuda_stream);
+
+/* Sliding windows ("Events are streamed in temporal windows"): advance the
+ * window kept in the workspace to [t0, t0+window).  d_new_events: DEVICE, the n_new events that follow,
+ * in the stream, the events handed over by the previous call.  The row of a pixel becomes the previous
+ * row's events that are still inside the window (re-based to the new t0) followed by its new events: the
+ * input order of the window's slice of the stream, so row_ptr / csr_ev are bit-identical to ddhf_window()
+ * on that slice (R20), and so is everything downstream; only the new slab is sorted.  The first call (and
+ * any call with another workspace, another window length, or t0 moved backwards or by a whole window or
+ * more) starts a sequence: its events are the whole first window.  counters[n_dropped] counts the new
+ * events outside the window or the sensor.  If the window outgrows max_events it is truncated and bit 2 of
+ * counters[overflow] is set.  The workspace must not be used by other calls in between (ddhf_window()
+ * on the same workspace keeps the state intact; ddhf_slide_reset() forgets it).  Otherwise as ddhf_window(). */
+int ddhf_window_slide(ddhf_handle *h, const ddhf_event *d_new_events, int64_t n_new, int64_t t0_us,
+                      int64_t window_us, void *d_workspace, const ddhf_outputs *out,
+                      void *cuda_stream);
+int ddhf_slide_reset(ddhf_handle *h);
 
 /* End-to-end variant: h_events is HOST memory (pinned for full PCIe speed).  Copies the
  * events to the device, runs ddhf_window() on buffers owned by the handle (allocated on

@@ -22,7 +22,8 @@ DDHF_FLAG_SCORE_ALL, DDHF_FLAG_TIMING = 1, 2
 N_COUNTERS = 16
 
 #: every symbol include/ddhf.h declares
-EXPORTS = ["ddhf_create", "ddhf_workspace_bytes", "ddhf_window", "ddhf_window_host",
+EXPORTS = ["ddhf_create", "ddhf_workspace_bytes", "ddhf_window", "ddhf_window_slide", "ddhf_slide_reset",
+           "ddhf_window_host",
            "ddhf_host_submit", "ddhf_host_wait",
            "ddhf_stage_ms", "ddhf_launches_per_window", "ddhf_fma_peak_probe", "ddhf_destroy",
            "ddhf_last_error", "ddhf_version"]
@@ -78,6 +79,11 @@ def lib() -> C.CDLL:
         L.ddhf_window.restype = C.c_int
         L.ddhf_window.argtypes = [vp, vp, C.c_int64, C.c_int64, C.c_int64, vp,
                                   C.POINTER(DdhfOutputs), vp]
+        L.ddhf_window_slide.restype = C.c_int
+        L.ddhf_window_slide.argtypes = [vp, vp, C.c_int64, C.c_int64, C.c_int64, vp,
+                                        C.POINTER(DdhfOutputs), vp]
+        L.ddhf_slide_reset.restype = C.c_int
+        L.ddhf_slide_reset.argtypes = [vp]
         L.ddhf_window_host.restype = C.c_int
         L.ddhf_window_host.argtypes = [vp, vp, C.c_int64, C.c_int64, C.c_int64,
                                        C.POINTER(DdhfHostOutputs), vp]
@@ -145,6 +151,18 @@ def ddhf_window(h, d_events_ptr: int, n: int, t0_us: int, window_us: int, d_work
                            stream_ptr)
     if rc != DDHF_OK:
         raise DdhfError(rc, (lib().ddhf_last_error(h) or b"").decode())
+
+
+def ddhf_window_slide(h, d_new_events_ptr: int, n_new: int, t0_us: int, window_us: int, d_workspace_ptr: int,
+                      out: DdhfOutputs, stream_ptr: int = 0) -> None:
+    rc = lib().ddhf_window_slide(h, d_new_events_ptr, n_new, t0_us, window_us, d_workspace_ptr, C.byref(out),
+                                 stream_ptr)
+    if rc != DDHF_OK:
+        raise DdhfError(rc, (lib().ddhf_last_error(h) or b"").decode())
+
+
+def ddhf_slide_reset(h) -> None:
+    lib().ddhf_slide_reset(h)
 
 
 def ddhf_window_host(h, h_events_ptr: int, n: int, t0_us: int, window_us: int,
@@ -255,6 +273,16 @@ class Detector:
         ptr = d_events.data_ptr() + 16 * offset_events if n > 0 else 0
         ddhf_window(self.h, ptr, n, t0_us, window_us, self.workspace.data_ptr(), self.out,
                     st.cuda_stream)
+
+    def slide(self, d_events, n_new: int, t0_us: int, window_us: int, *, offset_events: int = 0,
+              stream=None) -> None:
+        """Advance the sliding window kept in the workspace (ddhf_window_slide): ``n_new`` events starting
+        at record ``offset_events`` of ``d_events`` are the events that follow those of the previous call."""
+        torch = self.torch
+        st = stream if stream is not None else torch.cuda.current_stream(self.device)
+        ptr = d_events.data_ptr() + 16 * offset_events if n_new > 0 else 0
+        ddhf_window_slide(self.h, ptr, n_new, t0_us, window_us, self.workspace.data_ptr(), self.out,
+                          st.cuda_stream)
 
     def stage_ms(self) -> list[float]:
         return ddhf_stage_ms(self.h)

@@ -31,7 +31,7 @@ struct ddhf_handle {
     int ndft_blocks_per_sm = 1, score_blocks_per_sm = 1;
     // workspace offsets (bytes)
     size_t off_cnt = 0, off_items = 0, off_scratch = 0, off_work = 0, off_tiles = 0, off_class = 0, off_cursor = 0, off_runs = 0, off_bkt = 0, off_rows = 0, off_spill = 0, off_spillrec = 0,
-           off_parent = 0, off_rec = 0, off_ctiles = 0, off_merge = 0, off_split = 0, off_splitcnt = 0, off_partial = 0, ws_bytes = 0;
+           off_parent = 0, off_rec = 0, off_ctiles = 0, off_merge = 0, off_slide = 0, off_split = 0, off_splitcnt = 0, off_partial = 0, ws_bytes = 0;
     cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     bool timed_once = false;
     // buffers of the host-buffer variant
@@ -49,6 +49,11 @@ struct ddhf_handle {
     cudaStream_t copy_stream = nullptr;
     bool pipe_ready = false;
     long long pipe_head = 0, pipe_tail = 0;      // windows submitted / waited for
+    // sliding-window state (ddhf_window_slide): the previous window's CSR lives in the workspace
+    bool slide_valid = false;
+    int64_t slide_t0 = 0, slide_window = 0;
+    void *slide_ws = nullptr;
+    int slide_parity = 0;
     std::string err;
 };
 
@@ -270,6 +275,9 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
     h->off_parent = o;     o = align_up(o + sizeof(int32_t) * h->np);
     h->off_rec = o;        o = align_up(o + sizeof(int32_t) * 5 * static_cast<size_t>(h->np));
     h->off_ctiles = o;     o = align_up(o + sizeof(int32_t) * 1024);
+    // sliding windows: two copies of (row_ptr, csr_ev) used alternately, the new slab's own CSR
+    h->off_slide = o;      o = align_up(o + 2 * (sizeof(int32_t) * (static_cast<size_t>(h->np) + 2) + sizeof(uint32_t) * static_cast<size_t>(c.max_events))
+                                         + sizeof(int32_t) * static_cast<size_t>(h->np) + sizeof(uint32_t) * static_cast<size_t>(c.max_events) + 1024);
     h->off_merge = o;      o = align_up(o + sizeof(int32_t) * 6 * static_cast<size_t>(c.max_boxes));
     h->ws_bytes = o;
 
@@ -283,9 +291,11 @@ extern "C" size_t ddhf_workspace_bytes(const ddhf_handle *h) { return h ? h->ws_
 
 extern "C" int ddhf_launches_per_window(const ddhf_handle *h) { return h ? h->launches : 0; }
 
-extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n, int64_t t0_us,
-                           int64_t window_us, void *d_workspace, const ddhf_outputs *out,
-                           void *cuda_stream)
+// mode 0: one window from scratch; 1: first window of a sliding sequence (from scratch, CSR saved in the
+// workspace); 2: slide (d_events = the new slab, shift = t0 - previous t0)
+static int run_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n, int64_t t0_us,
+                      int64_t window_us, void *d_workspace, const ddhf_outputs *out,
+                      void *cuda_stream, int mode, int64_t shift_us)
 {
     if (!h) return DDHF_E_INVAL;
     if (!out || !d_workspace || (n > 0 && !d_events))
@@ -327,6 +337,22 @@ extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n
     ip.chunk_rows = reinterpret_cast<int32_t *>(ws + h->off_rows);
     ip.sync = reinterpret_cast<int32_t *>(ws + h->off_cursor + 16);       // [16]; the scoring queue counts are sync[2..3]
 
+    if (mode != 0) {
+        // state buffers: {row_ptr [np + 2], csr [max_events]} x 2, then the slab's {row starts [np], csr [max_events]}
+        const size_t rp_bytes = sizeof(int32_t) * (static_cast<size_t>(h->np) + 2), cs_bytes = sizeof(uint32_t) * static_cast<size_t>(c.max_events);
+        char *s0 = ws + h->off_slide, *s1 = s0 + rp_bytes + cs_bytes, *s2 = s1 + rp_bytes + cs_bytes;
+        char *prev = h->slide_parity ? s1 : s0, *next = h->slide_parity ? s0 : s1;
+        ip.next_row_ptr = reinterpret_cast<int32_t *>(next);
+        ip.next_csr = reinterpret_cast<uint32_t *>(next + rp_bytes);
+        if (mode == 2) {
+            ip.prev_row_ptr = reinterpret_cast<const int32_t *>(prev);
+            ip.prev_csr = reinterpret_cast<const uint32_t *>(prev + rp_bytes);
+            ip.slab_row_ptr = reinterpret_cast<int32_t *>(s2);
+            ip.slab_csr = reinterpret_cast<uint32_t *>(s2 + sizeof(int32_t) * static_cast<size_t>(h->np));
+            ip.shift2 = static_cast<uint32_t>(2 * shift_us);
+        }
+        ip.csr_cap = static_cast<int32_t>(c.max_events);
+    }
     ip.split_tab = reinterpret_cast<SplitRow *>(ws + h->off_split);
     ip.split_cnt = reinterpret_cast<int32_t *>(ws + h->off_splitcnt);
     ip.ccl_parent = cp_parent;
@@ -361,7 +387,7 @@ extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n
 
     int launches = 0;
     if (timing) cudaEventRecord(h->ev[0], st);
-    launches += launch_ingest(ip, st);
+    launches += (mode == 2) ? launch_ingest_slide(ip, st) : launch_ingest(ip, st);
     if (timing) cudaEventRecord(h->ev[1], st);
     launches += launch_ndft(np, c.n_freq, h->band_size, h->sm_count * h->ndft_blocks_per_sm,
                             h->sm_count * h->score_blocks_per_sm, st, timing ? h->ev[2] : nullptr);
@@ -371,6 +397,40 @@ extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n
     h->launches = launches;
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return fail(h, DDHF_E_CUDA, std::string("ddhf_window: ") + cudaGetErrorString(e));
+    return DDHF_OK;
+}
+
+extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n, int64_t t0_us,
+                           int64_t window_us, void *d_workspace, const ddhf_outputs *out,
+                           void *cuda_stream)
+{
+    return run_window(h, d_events, n, t0_us, window_us, d_workspace, out, cuda_stream, 0, 0);
+}
+
+extern "C" int ddhf_window_slide(ddhf_handle *h, const ddhf_event *d_new_events, int64_t n_new, int64_t t0_us,
+                                 int64_t window_us, void *d_workspace, const ddhf_outputs *out,
+                                 void *cuda_stream)
+{
+    if (!h) return DDHF_E_INVAL;
+    // a continuation needs the state of the previous call: same workspace, same window length, t0 not
+    // moved backwards and by less than a window; anything else starts a new sequence from scratch
+    const bool cont = h->slide_valid && h->slide_ws == d_workspace && h->slide_window == window_us &&
+                      t0_us >= h->slide_t0 && t0_us - h->slide_t0 < window_us;
+    const int rc = run_window(h, d_new_events, n_new, t0_us, window_us, d_workspace, out, cuda_stream,
+                              cont ? 2 : 1, cont ? t0_us - h->slide_t0 : 0);
+    if (rc != DDHF_OK) { h->slide_valid = false; return rc; }
+    h->slide_valid = true;
+    h->slide_t0 = t0_us;
+    h->slide_window = window_us;
+    h->slide_ws = d_workspace;
+    h->slide_parity ^= 1;
+    return DDHF_OK;
+}
+
+extern "C" int ddhf_slide_reset(ddhf_handle *h)
+{
+    if (!h) return DDHF_E_INVAL;
+    h->slide_valid = false;
     return DDHF_OK;
 }
 

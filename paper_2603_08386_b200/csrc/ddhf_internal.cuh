@@ -115,6 +115,15 @@ struct IngestParams {
                                  //     4: work items, 5: split rows, 6: partials, 7: arrival counters handed out, 8: box-merge CTAs finished
     SplitRow *split_tab;         // rows longer than kSplitMin (see NdftParams)
     int32_t *split_cnt;
+    // sliding windows (ddhf_window_slide): NULL otherwise
+    const int32_t *prev_row_ptr; // [np + 1] CSR of the previous window (workspace copy)
+    const uint32_t *prev_csr;
+    int32_t *next_row_ptr;       // [np + 1] copy of this window's CSR for the next call
+    uint32_t *next_csr;
+    int32_t *slab_row_ptr;       // [np] row starts of the new slab's own CSR
+    uint32_t *slab_csr;          // [max_events]
+    uint32_t shift2;             // 2 (t0 - previous t0): values below it have left the window
+    int32_t csr_cap;             // max_events: a sliding window that outgrows it is truncated and flagged
     int32_t *active_idx;
     WorkItem *work;
     int32_t *tile_sum, *tile_act;   // [n_tiles]
@@ -148,6 +157,7 @@ struct CclParams {
 // kernel-set entry points (host functions that enqueue on `st`); each returns the number
 // of kernels it launched
 int launch_ingest(const IngestParams &p, cudaStream_t st);
+int launch_ingest_slide(const IngestParams &p, cudaStream_t st);   // p.events = the new slab; previous CSR in p.prev_*
 cudaError_t ingest_configure();              // opt in to large dynamic shared memory
 int ingest_tile_events();                    // events per sort tile
 int ingest_tile_stride(bool compact);        // items per tile slot of IngestParams::items (run padding included)

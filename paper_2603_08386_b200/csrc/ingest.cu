@@ -565,7 +565,10 @@ __global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
     const int pix0 = b << bl;
     if (m == 0) {
         for (int l = t; l < nl; l += kNT)
-            if (pix0 + l < p.np) p.cnt[pix0 + l] = 0;
+            if (pix0 + l < p.np) {
+                p.cnt[pix0 + l] = 0;
+                if (p.slab_row_ptr) p.slab_row_ptr[pix0 + l] = gbase;
+            }
         return;
     }
     const bool single = m <= C::kCap;
@@ -586,7 +589,10 @@ __global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
         sort_chunk_any<COMPACT>(buf, cnt, rstart, s_warp, fill, bl, vb);
         if (single) {
             for (int l = t; l < nl; l += kNT)
-                if (pix0 + l < p.np) p.cnt[pix0 + l] = static_cast<int32_t>(rstart[l + 1] - rstart[l]);
+                if (pix0 + l < p.np) {
+                    p.cnt[pix0 + l] = static_cast<int32_t>(rstart[l + 1] - rstart[l]);
+                    if (p.slab_row_ptr) p.slab_row_ptr[pix0 + l] = gbase + static_cast<int32_t>(rstart[l]);
+                }
             for (int r = t; r < fill; r += kNT) p.csr_ev[gbase + r] = C::val_of(buf[pad_pos<T>(r)], vb);
         } else {
             if (t == 0) s_row = atomicAdd(p.sync + 1, 1);
@@ -716,7 +722,10 @@ __global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
         for (int k = 0; k < 8; ++k) {
             const int l = t * per + k;
             if (k < per && l < nl) {
-                if (pix0 + l < p.np) p.cnt[pix0 + l] = static_cast<int32_t>(v[k]);
+                if (pix0 + l < p.np) {
+                    p.cnt[pix0 + l] = static_cast<int32_t>(v[k]);
+                    if (p.slab_row_ptr) p.slab_row_ptr[pix0 + l] = gbase + static_cast<int32_t>(ex);
+                }
                 rstart[l] = ex;                              // row start of pixel l inside the bucket
                 ex += v[k];
             }
@@ -835,6 +844,7 @@ __global__ void __launch_bounds__(1024) k_scan_tiles(IngestParams p, int n_tiles
         p.counters[DDHF_CNT_N_IN] = ta;
         p.counters[DDHF_CNT_N_ACTIVE] = tb;
         if (tb > p.max_active) atomicOr(&p.counters[DDHF_CNT_OVERFLOW], 1);
+        if (p.prev_csr && ta > p.csr_cap) atomicOr(&p.counters[DDHF_CNT_OVERFLOW], 4);   // sliding window outgrew max_events
         int run = 0;
         for (int c = kNumClasses - 1; c >= 0; --c) {     // descending cost
             const int n = p.class_cnt[c];
@@ -923,6 +933,62 @@ __global__ void __launch_bounds__(1024) k_scan_apply(IngestParams p)
 
 
 
+
+// ---- sliding windows: the previous window's CSR advanced by one hop --------------------
+// Row of a pixel in the new window = the previous row's events that are still inside it (value >= 2 shift,
+// shift = t0 - previous t0; re-based to the new t0) followed by the pixel's events of the new slab, which
+// has just been bucketed on its own (k_tile_sort / k_bucket_sort: cnt = slab counts, slab_row_ptr, slab_csr).
+// That is the input order of the window's slice of the stream, so row_ptr / csr_ev equal a bucketing from
+// scratch bit for bit (R20).  One thread per pixel: rows hold a few events.
+__global__ void k_slide_count(IngestParams p)
+{
+    const int pix = blockIdx.x * blockDim.x + threadIdx.x;
+    if (pix >= p.np) return;
+    const int r0 = p.prev_row_ptr[pix], r1 = p.prev_row_ptr[pix + 1];
+    int kept = 0;
+    for (int k = r0; k < r1; ++k) kept += (p.prev_csr[k] >= p.shift2) ? 1 : 0;
+    p.cnt[pix] += kept;
+}
+
+__global__ void k_slide_merge(IngestParams p)
+{
+    const int pix = blockIdx.x * blockDim.x + threadIdx.x;
+    if (pix > p.np) return;
+    const int dst0 = p.row_ptr[pix];
+    p.next_row_ptr[pix] = dst0;                           // the state of the next call
+    if (pix == p.np) return;
+    const int total = p.row_ptr[pix + 1] - dst0;
+    const int r0 = p.prev_row_ptr[pix], r1 = p.prev_row_ptr[pix + 1];
+    int k = 0;
+    for (int q = r0; q < r1; ++q) {
+        const uint32_t v = p.prev_csr[q];
+        if (v >= p.shift2) {
+            const uint32_t w = v - p.shift2;
+            if (dst0 + k < p.csr_cap) {
+                p.csr_ev[dst0 + k] = w;
+                p.next_csr[dst0 + k] = w;
+            }
+            ++k;
+        }
+    }
+    const uint32_t *src = p.slab_csr + p.slab_row_ptr[pix];
+    for (int q = 0; k < total; ++q, ++k) {
+        const uint32_t w = src[q];
+        if (dst0 + k < p.csr_cap) {
+            p.csr_ev[dst0 + k] = w;
+            p.next_csr[dst0 + k] = w;
+        }
+    }
+}
+
+// first call of a sliding sequence: the window was bucketed from scratch; keep a copy as the state
+__global__ void k_slide_save(IngestParams p)
+{
+    const int n_in = p.row_ptr[p.np];
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n_in; i += gridDim.x * blockDim.x) p.next_csr[i] = p.csr_ev[i];
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i <= p.np; i += gridDim.x * blockDim.x) p.next_row_ptr[i] = p.row_ptr[i];
+}
+
 }  // namespace
 
 namespace {
@@ -964,13 +1030,11 @@ void ingest_plan(int np, int *bl, int *nb, int *hbits)
     *hbits = hb;
 }
 
-int launch_ingest(const IngestParams &p, cudaStream_t st)
+namespace {
+int launch_sort(const IngestParams &p, cudaStream_t st)
 {
-    const int n_tiles = (p.np + kScanTile - 1) / kScanTile;
     const int ev_tiles = static_cast<int>((p.n + kTile - 1) / kTile);
     int launches = 0;
-    const int init_items = p.np > p.nb + 2 ? p.np : p.nb + 2;
-    k_init<<<(init_items + 255) / 256, 256, 0, st>>>(p); ++launches;
     if (p.compact) {
         if (ev_tiles > 0) { k_tile_sort<true><<<ev_tiles, kNT, ingest_tile_smem(true), st>>>(p); ++launches; }
         k_bucket_sort<true><<<p.nb, kNT, BucketCfg<true>::smem_bytes(p.bl), st>>>(p); ++launches;
@@ -978,9 +1042,42 @@ int launch_ingest(const IngestParams &p, cudaStream_t st)
         if (ev_tiles > 0) { k_tile_sort<false><<<ev_tiles, kNT, ingest_tile_smem(false), st>>>(p); ++launches; }
         k_bucket_sort<false><<<p.nb, kNT, BucketCfg<false>::smem_bytes(p.bl), st>>>(p); ++launches;
     }
-    k_scan_reduce<<<n_tiles, 1024, 0, st>>>(p); ++launches;
-    k_scan_tiles<<<1, 1024, 0, st>>>(p, n_tiles); ++launches;
-    k_scan_apply<<<n_tiles, 1024, 0, st>>>(p); ++launches;
+    return launches;
+}
+
+int launch_scans(const IngestParams &p, cudaStream_t st)
+{
+    const int n_tiles = (p.np + kScanTile - 1) / kScanTile;
+    k_scan_reduce<<<n_tiles, 1024, 0, st>>>(p);
+    k_scan_tiles<<<1, 1024, 0, st>>>(p, n_tiles);
+    k_scan_apply<<<n_tiles, 1024, 0, st>>>(p);
+    return 3;
+}
+}  // namespace
+
+int launch_ingest(const IngestParams &p, cudaStream_t st)
+{
+    int launches = 0;
+    const int init_items = p.np > p.nb + 2 ? p.np : p.nb + 2;
+    k_init<<<(init_items + 255) / 256, 256, 0, st>>>(p); ++launches;
+    launches += launch_sort(p, st);
+    launches += launch_scans(p, st);
+    if (p.next_csr) { k_slide_save<<<592, 256, 0, st>>>(p); ++launches; }      // first window of a sliding sequence
+    return launches;
+}
+
+// p.events / p.n: the new slab only; the previous window is in prev_row_ptr / prev_csr
+int launch_ingest_slide(const IngestParams &p, cudaStream_t st)
+{
+    int launches = 0;
+    const int init_items = p.np > p.nb + 2 ? p.np : p.nb + 2;
+    k_init<<<(init_items + 255) / 256, 256, 0, st>>>(p); ++launches;
+    IngestParams q = p;                      // the slab is bucketed into its own CSR
+    q.csr_ev = p.slab_csr;
+    launches += launch_sort(q, st);
+    k_slide_count<<<(p.np + 255) / 256, 256, 0, st>>>(p); ++launches;
+    launches += launch_scans(p, st);
+    k_slide_merge<<<(p.np + 256) / 256, 256, 0, st>>>(p); ++launches;
     return launches;
 }
 

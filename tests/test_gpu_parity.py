@@ -303,3 +303,65 @@ def test_config5_whole_window(oracle):
 def test_paper_point_whole_window(oracle):
     w = wl.paper_native()
     _whole_window_compare(oracle, w, w.params, w.events, 0, score_all=False, name="paper point whole window")
+
+
+@pytest.mark.slow
+def test_sliding_windows_incremental_csr(oracle):
+    """SURVEY 8(f)-3 / PAPER.md L137: config 5's stream (half scale) through ddhf_window_slide(), 100 windows
+    of 50 ms with a 10 ms hop -- only the new 10 ms slab is sorted.  row_ptr and csr_ev of EVERY window are
+    bit-identical to the oracle's bucketing of that window's slice, and the detections of sampled windows
+    equal ddhf_window() on the same slice."""
+    from paper_2603_08386_b200 import binding
+    w = wl.make(5, n_windows=100, scale=0.5)
+    prm = w.params
+    slices = [w.window_slice(k) for k in range(w.n_windows)]
+    max_ev = max(n for _, n, _ in slices)
+    det = binding.Detector(prm, max_events=max_ev, want_power=False)
+    ref = binding.Detector(prm, max_events=max_ev, want_power=False)
+    d_ev = det.upload(w.events)
+    prev_hi = None
+    for k, (lo, n, t0) in enumerate(slices):
+        hi = lo + n
+        if prev_hi is None:
+            det.slide(d_ev, n, t0, w.window_us, offset_events=lo)              # the whole first window
+        else:
+            det.slide(d_ev, hi - prev_hi, t0, w.window_us, offset_events=prev_hi)   # the new slab only
+        prev_hi = hi
+        g = det.results()
+        row_ptr, csr, dropped = oracle.bucket(w.events[lo:hi], w.width, w.height, t0, w.window_us)
+        assert g["n_in"] == row_ptr[-1] and g["overflow"] == 0, k
+        assert np.array_equal(g["row_ptr"], row_ptr), f"row_ptr differs in window {k}"
+        assert np.array_equal(g["csr_ev"], csr), f"csr_ev differs in window {k}"
+        if k % 17 == 0 or k == w.n_windows - 1:
+            ref.window(d_ev, n, t0, w.window_us, offset_events=lo)
+            r = ref.results()
+            for key in ("active_idx", "sf", "score", "f0_idx", "mask", "boxes"):
+                assert np.array_equal(g[key], r[key], equal_nan=True) if g[key].dtype.kind == "f" else np.array_equal(g[key], r[key]), (k, key)
+    det.close()
+    ref.close()
+
+
+def test_sliding_window_restarts_and_empty_slabs(oracle):
+    """ddhf_window_slide(): an empty slab, a hop of a whole window (restart from scratch), t0 moved backwards."""
+    from paper_2603_08386_b200 import binding
+    W, H, T = 48, 40, 20_000
+    ev = wl.random_window(31, W, H, 30_000, 100_000, hot_fraction=0.3, out_of_range=0.05)
+    prm = dict(wl.preset(1), width=W, height=H, n_min=2)
+    det = binding.Detector(prm, max_events=len(ev), want_power=False)
+    d_ev = det.upload(ev)
+    t = ev["t"]
+    def sl(t0):
+        return int(np.searchsorted(t, t0, "left")), int(np.searchsorted(t, t0 + T, "left"))
+    prev_hi = None
+    for t0 in (0, 5_000, 5_000, 12_000, 40_000, 45_000, 20_000, 21_000):
+        lo, hi = sl(t0)
+        cont = prev_hi is not None and 0 <= t0 - prev_t0 < T
+        if cont:
+            det.slide(d_ev, hi - prev_hi, t0, T, offset_events=prev_hi)
+        else:
+            det.slide(d_ev, hi - lo, t0, T, offset_events=lo)
+        prev_hi, prev_t0 = hi, t0
+        g = det.results()
+        row_ptr, csr, _ = oracle.bucket(ev[lo:hi], W, H, t0, T)
+        assert np.array_equal(g["row_ptr"], row_ptr) and np.array_equal(g["csr_ev"], csr), t0
+    det.close()
