@@ -262,7 +262,7 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
         ingest_plan(h->np, &h->bl, &h->nb, &h->hbits);
         const size_t ev_tiles = (static_cast<size_t>(c.max_events) + ingest_tile_events() - 1) / ingest_tile_events();
         h->off_runs = o;    o = align_up(o + sizeof(uint32_t) * ev_tiles * static_cast<size_t>(h->nb));
-        h->off_bkt = o;     o = align_up(o + sizeof(int32_t) * 3 * (static_cast<size_t>(h->nb) + 2));
+        h->off_bkt = o;     o = align_up(o + sizeof(int32_t) * 4 * (static_cast<size_t>(h->nb) + 2));
         h->off_rows = o;    o = align_up(o + sizeof(int32_t) * (2 * ev_tiles + h->nb + 2) * (4 + (static_cast<size_t>(1) << h->bl)));
     }
     // deferred-scoring queue: spectra of the pixels that pass the SF filter (32 Ki rows at most;
@@ -334,6 +334,7 @@ static int run_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n, int
     ip.bkt_total = reinterpret_cast<int32_t *>(ws + h->off_bkt);
     ip.bkt_base = ip.bkt_total + h->nb + 2;
     ip.bkt_order = ip.bkt_base + h->nb + 2;
+    ip.bkt_act = ip.bkt_order + h->nb + 2;
     ip.chunk_rows = reinterpret_cast<int32_t *>(ws + h->off_rows);
     ip.sync = reinterpret_cast<int32_t *>(ws + h->off_cursor + 16);       // [16]; the scoring queue counts are sync[2..3]
 

@@ -109,6 +109,7 @@ struct IngestParams {
     void *scratch;               // [max_events] sorted chunks of the buckets that need more than one
     uint32_t *run_tab;           // [ev_tiles][nb] run of every bucket inside its tile: first item | length << 16
     int32_t *bkt_order;          // [nb] buckets by descending size class
+    int32_t *bkt_act;            // [nb] active pixels (count >= n_min) of every bucket
     int32_t *bkt_total, *bkt_base;   // [nb + 2] events per bucket; exclusive scan (bkt_base[nb] = n_in)
     int32_t *chunk_rows;         // [max_rows][4 + 2^bl] chunk table of the multi-chunk buckets
     int32_t *sync;               // [16] 0: tiles finished, 1: chunk rows handed out, 2-3: scoring queue counts,

@@ -563,6 +563,9 @@ __global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
     const int m = p.bkt_total[b];
     const int gbase = p.bkt_base[b];
     const int pix0 = b << bl;
+    __shared__ int s_act, s_class[kNumClasses];           // active pixels / work items per class of this bucket
+    if (t == 0) { s_act = 0; p.bkt_act[b] = 0; }
+    if (t < kNumClasses) s_class[t] = 0;
     if (m == 0) {
         for (int l = t; l < nl; l += kNT)
             if (pix0 + l < p.np) {
@@ -571,6 +574,22 @@ __global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
             }
         return;
     }
+    // (not on the sliding-window path: its counts are completed later and go through the scan kernels)
+    const int nmin = p.prev_csr ? 0x7fffffff : max(p.n_min, 1);
+    // a pixel's row length is known: count it for the active list and the work-list classes (k_worklist)
+    auto tally = [&](int n) {
+        if (n >= nmin) {
+            int seg_len;
+            const int n_seg = row_segments(n, seg_len);
+            atomicAdd(&s_act, 1);
+            atomicAdd(&s_class[size_class(seg_len)], n_seg);
+        }
+    };
+    auto publish_tally = [&]() {
+        __syncthreads();
+        if (t == 0) p.bkt_act[b] = s_act;
+        if (t < kNumClasses && s_class[t]) atomicAdd(&p.class_cnt[t], s_class[t]);
+    };
     const bool single = m <= C::kCap;
     if (!single)
         for (int l = t; l < nl; l += kNT) pixtot[l] = 0u;
@@ -592,6 +611,7 @@ __global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
                 if (pix0 + l < p.np) {
                     p.cnt[pix0 + l] = static_cast<int32_t>(rstart[l + 1] - rstart[l]);
                     if (p.slab_row_ptr) p.slab_row_ptr[pix0 + l] = gbase + static_cast<int32_t>(rstart[l]);
+                    tally(static_cast<int>(rstart[l + 1] - rstart[l]));
                 }
             for (int r = t; r < fill; r += kNT) p.csr_ev[gbase + r] = C::val_of(buf[pad_pos<T>(r)], vb);
         } else {
@@ -703,7 +723,7 @@ __global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
         }
     }
     flush();
-    if (single) return;
+    if (single) { publish_tally(); return; }
 
     // loop 2: row starts of the bucket's pixels, then every chunk goes to its place
     {
@@ -725,6 +745,7 @@ __global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
                 if (pix0 + l < p.np) {
                     p.cnt[pix0 + l] = static_cast<int32_t>(v[k]);
                     if (p.slab_row_ptr) p.slab_row_ptr[pix0 + l] = gbase + static_cast<int32_t>(ex);
+                    tally(static_cast<int>(v[k]));
                 }
                 rstart[l] = ex;                              // row start of pixel l inside the bucket
                 ex += v[k];
@@ -746,6 +767,7 @@ __global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
         }
         row = prev_row;
     }
+    publish_tally();
 }
 
 // ---- block-wide exclusive scan of two ints (1024 threads) -----------------------------
@@ -792,6 +814,38 @@ __device__ __forceinline__ void load4(const int32_t *src, int base, int np, int 
     } else {
 #pragma unroll
         for (int j = 0; j < 4; ++j) v[j] = (base + j < np) ? src[base + j] : 0;
+    }
+}
+
+// Work item(s) of one active row: the row itself, or one item per segment of a split row (ndft.cu)
+__device__ __forceinline__ void emit_work(const IngestParams &p, WorkItem *dst, int pix, int off, int n, int aoff,
+                                          int n_seg, int seg_len)
+{
+    WorkItem it;
+    if (n_seg == 1) {
+        it.row_begin = off;
+        it.n = n;
+        it.pix = pix;
+        it.arow = aoff;
+        *dst = it;
+        return;
+    }
+    // split row: the row's identity goes to the split table
+    const int sid = atomicAdd(p.sync + 5, 1);
+    SplitRow sr;
+    const int nodes = split_nodes(n_seg);
+    sr.pix = pix; sr.arow = aoff; sr.n_seg = n_seg;
+    sr.seg_base = atomicAdd(p.sync + 6, split_slots(n_seg));
+    sr.cnt_base = atomicAdd(p.sync + 7, nodes);
+    sr._pad[0] = 0; sr._pad[1] = 0; sr._pad[2] = 0;
+    p.split_tab[sid] = sr;
+    for (int q = 0; q < nodes; ++q) p.split_cnt[sr.cnt_base + q] = 0;
+    for (int sg = 0; sg < n_seg; ++sg) {
+        it.row_begin = off + sg * seg_len;
+        it.n = min(seg_len, n - sg * seg_len);
+        it.pix = static_cast<int32_t>(0x80000000u | static_cast<uint32_t>(sid));
+        it.arow = sg;
+        dst[sg] = it;
     }
 }
 
@@ -898,32 +952,7 @@ __global__ void __launch_bounds__(1024) k_scan_apply(IngestParams p)
                 int seg_len;
                 const int n_seg = row_segments(v[j], seg_len);
                 WorkItem *dst = p.work + s_base[size_class(seg_len)] + lrank[j];
-                WorkItem it;
-                if (n_seg == 1) {
-                    it.row_begin = off;
-                    it.n = v[j];
-                    it.pix = pix;
-                    it.arow = aoff;
-                    *dst = it;
-                } else {
-                    // split row: one work item per segment, the row's identity in the split table
-                    const int sid = atomicAdd(p.sync + 5, 1);
-                    SplitRow sr;
-                    const int nodes = split_nodes(n_seg);
-                    sr.pix = pix; sr.arow = aoff; sr.n_seg = n_seg;
-                    sr.seg_base = atomicAdd(p.sync + 6, split_slots(n_seg));
-                    sr.cnt_base = atomicAdd(p.sync + 7, nodes);
-                    sr._pad[0] = 0; sr._pad[1] = 0; sr._pad[2] = 0;
-                    p.split_tab[sid] = sr;
-                    for (int q = 0; q < nodes; ++q) p.split_cnt[sr.cnt_base + q] = 0;
-                    for (int sg = 0; sg < n_seg; ++sg) {
-                        it.row_begin = off + sg * seg_len;
-                        it.n = min(seg_len, v[j] - sg * seg_len);
-                        it.pix = static_cast<int32_t>(0x80000000u | static_cast<uint32_t>(sid));
-                        it.arow = sg;
-                        dst[sg] = it;
-                    }
-                }
+                emit_work(p, dst, pix, off, v[j], aoff, n_seg, seg_len);
                 ++aoff;
             }
             off += v[j];
@@ -933,6 +962,72 @@ __global__ void __launch_bounds__(1024) k_scan_apply(IngestParams p)
 
 
 
+
+// ---- k_worklist: active list and size-classed work list, one CTA per bucket ---------------------------
+// The from-scratch path: k_bucket_sort has written cnt and row_ptr of every pixel, the active pixels of
+// every bucket (bkt_act) and the class totals (class_cnt), so the three scan kernels above (still used by
+// the sliding-window path, where the counts come from two sources) collapse into this one.
+__global__ void __launch_bounds__(1024) k_worklist(IngestParams p)
+{
+    __shared__ int s_a[33], s_b[33];
+    __shared__ int s_cls[kNumClasses], s_base[kNumClasses], s_tot[kNumClasses];
+    const int t = threadIdx.x;
+    if (t < kNumClasses) { s_cls[t] = 0; s_tot[t] = p.class_cnt[t]; }
+    // a tile of kScanTile pixels holds whole buckets (2^bL divides it): active pixels in the buckets before it
+    const int nl = 1 << p.bl;
+    const int first_bucket = (blockIdx.x * kScanTile) >> p.bl;
+    int a = (t < p.nb) ? p.bkt_act[t] : 0;                // nb <= 1023: one value per thread
+    int before = (t < first_bucket) ? a : 0;
+    int ta, tb;
+    block_scan2(a, before, ta, tb, s_a, s_b);             // ta = all active pixels, tb = those before this tile
+    const int n_active = ta, aoff0 = tb;
+    if (t == 0) {
+        // class bases: descending cost (every CTA derives the same values from the totals)
+        int run = 0;
+        for (int c = kNumClasses - 1; c >= 0; --c) { s_base[c] = run; run += s_tot[c]; }
+        if (blockIdx.x == 0) {
+            p.row_ptr[p.np] = p.bkt_base[p.nb];
+            p.counters[DDHF_CNT_N_ACTIVE] = n_active;
+            if (n_active > p.max_active) atomicOr(&p.counters[DDHF_CNT_OVERFLOW], 1);
+            p.sync[4] = run;                              // work items (a split row counts once per segment)
+        }
+    }
+    __syncthreads();
+    (void)nl;
+    const int base = blockIdx.x * kScanTile + t * 4;
+    const int nmin = max(p.n_min, 1);
+    int v[4], lrank[4], act = 0, dummy = 0;
+    load4(p.cnt, base, p.np, v);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        lrank[j] = -1;
+        if (v[j] >= nmin) {
+            ++act;
+            int seg_len;
+            const int n_seg = row_segments(v[j], seg_len);
+            lrank[j] = atomicAdd(&s_cls[size_class(seg_len)], n_seg);
+        }
+    }
+    int t1, t2;
+    block_scan2(act, dummy, t1, t2, s_a, s_b);            // contains __syncthreads: s_cls is final
+    if (t < kNumClasses) {
+        const int n = s_cls[t];
+        s_base[t] += (n ? atomicAdd(&p.class_cur[t], n) : 0);
+    }
+    __syncthreads();
+    int aoff = aoff0 + act;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        if (lrank[j] >= 0) {
+            const int pix = base + j;
+            if (aoff < p.max_active) p.active_idx[aoff] = pix;
+            int seg_len;
+            const int n_seg = row_segments(v[j], seg_len);
+            emit_work(p, p.work + s_base[size_class(seg_len)] + lrank[j], pix, p.row_ptr[pix], v[j], aoff, n_seg, seg_len);
+            ++aoff;
+        }
+    }
+}
 
 // ---- sliding windows: the previous window's CSR advanced by one hop --------------------
 // Row of a pixel in the new window = the previous row's events that are still inside it (value >= 2 shift,
@@ -1060,8 +1155,10 @@ int launch_ingest(const IngestParams &p, cudaStream_t st)
     int launches = 0;
     const int init_items = p.np > p.nb + 2 ? p.np : p.nb + 2;
     k_init<<<(init_items + 255) / 256, 256, 0, st>>>(p); ++launches;
-    launches += launch_sort(p, st);
-    launches += launch_scans(p, st);
+    IngestParams q = p;                      // k_bucket_sort writes row_ptr itself
+    q.slab_row_ptr = p.row_ptr;
+    launches += launch_sort(q, st);
+    k_worklist<<<(p.np + kScanTile - 1) / kScanTile, 1024, 0, st>>>(p); ++launches;
     if (p.next_csr) { k_slide_save<<<592, 256, 0, st>>>(p); ++launches; }      // first window of a sliding sequence
     return launches;
 }
