@@ -422,11 +422,11 @@ def main():
     ing_ms = float(stage[:, 0].mean())
     ing_bytes = 20.0 * n_ev + 8.0 * prm["width"] * prm["height"]          # 16 B read + 4 B written per event, 8 B per pixel
     roofline_stages = {
-        "ingest": {"bound": "hbm", "kernels": "k_init, k_tile_sort, k_bucket_sort, k_scan_reduce/tiles/apply",
+        "ingest": {"bound": "hbm", "kernels": "k_init, k_tile_sort, k_bucket_sort, k_worklist",
                    "achieved": ing_bytes / (ing_ms * 1e-3) / 1e9,
                    "peak": hbm_peak, "unit": "GB/s", "frac": ing_bytes / (ing_ms * 1e-3) / 1e9 / hbm_peak,
                    "algorithmic_bytes": ing_bytes, "ms": ing_ms, "peak_kind": hbm_kind,
-                   "traffic": traffic_of(("k_init", "k_tile_sort", "k_bucket_sort", "k_scan_"), args.workload),
+                   "traffic": traffic_of(("k_init", "k_tile_sort", "k_bucket_sort", "k_worklist"), args.workload),
                    "traffic_source": "sum of dram__bytes_read.sum + dram__bytes_write.sum of the ingest kernels, one launch each "
                                      "(profiles/r2_traffic.csv)",
                    "note": "events are read once (16 B), bucket-sorted 4-byte items written and read once, csr_ev written; "
