@@ -101,7 +101,9 @@ typedef struct {
     int32_t max_active;             /* capacity: rows of the compact power output         */
     int32_t max_boxes;              /* capacity: boxes                                    */
     int32_t max_scored;             /* capacity (rows of n_freq floats) of the deferred comb-
-                                       scoring queue in the workspace; 0 = min(NP, 32768).
+                                       scoring queue in the workspace; 0 = one row per pixel
+                                       if that is below 1/16 of the device memory (the NDFT
+                                       kernel then runs its lean variant), else min(NP, 32768).
                                        Pixels beyond it are scored in place: same results   */
     uint32_t flags;                 /* DDHF_FLAG_*                                        */
 } ddhf_config;

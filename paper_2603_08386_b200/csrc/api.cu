@@ -24,6 +24,7 @@ struct ddhf_handle {
     int launches = 0;
     int bl = 5, nb = 1, hbits = 1;          // ingest digit split (ingest_plan)
     int spill_cap = 0;
+    bool fallback = true;                  // the NDFT kernel variant with in-place scoring (queue smaller than the sensor)
     ScoreParams sp{};
     uint64_t g_f0 = 0, g_d = 0, g_h = 0;
     unsigned char *d_tables = nullptr;      // comb tables (num_tab | piece_tab | meta)
@@ -214,8 +215,21 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
         h->sp.meta = reinterpret_cast<const uint4 *>(h->d_tables + off_meta);
     }
     h->band_size = band_size;
+    {
+        // deferred-scoring queue: one row (the padded spectrum) per pixel to score.  Default: a row for every
+        // pixel when that stays below 1/16 of the device's memory (1280x720 at 2048 bins: 7.5 GB of the
+        // workspace on a 180 GB part) -- the NDFT kernel then never scores in place and runs its lean variant;
+        // else 32 Ki rows with the in-place fallback.  max_scored > 0 sets the row count explicitly.
+        const size_t row_bytes = sizeof(float) * static_cast<size_t>(ndft_padded_bins(c.n_freq));
+        size_t mem_free = 0, mem_total = 0;
+        cudaMemGetInfo(&mem_free, &mem_total);
+        h->spill_cap = (row_bytes * static_cast<size_t>(h->np) <= mem_total / 16) ? h->np : (h->np < 32768 ? h->np : 32768);
+        if (c.max_scored > 0) h->spill_cap = c.max_scored < h->np ? c.max_scored : h->np;
+        if (!ndft_scores_in_place(c.n_freq, band_size)) h->spill_cap = h->np;      // every pixel must fit in the queue
+        h->fallback = h->spill_cap < h->np;
+    }
     if (ingest_configure() != cudaSuccess ||
-        ndft_configure(c.n_freq, band_size, cpad, &h->ndft_blocks_per_sm, &h->score_blocks_per_sm) != cudaSuccess) {
+        ndft_configure(c.n_freq, band_size, cpad, h->fallback, &h->ndft_blocks_per_sm, &h->score_blocks_per_sm) != cudaSuccess) {
         const std::string msg = std::string("ddhf_create: ") + cudaGetErrorString(cudaGetLastError());
         cudaFree(h->d_tables);
         delete h;
@@ -265,11 +279,7 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
         h->off_bkt = o;     o = align_up(o + sizeof(int32_t) * 4 * (static_cast<size_t>(h->nb) + 2));
         h->off_rows = o;    o = align_up(o + sizeof(int32_t) * (2 * ev_tiles + h->nb + 2) * (4 + (static_cast<size_t>(1) << h->bl)));
     }
-    // deferred-scoring queue: spectra of the pixels that pass the SF filter (32 Ki rows at most;
-    // pixels beyond the capacity are scored in place by the NDFT kernel)
-    h->spill_cap = h->np < 32768 ? h->np : 32768;
-    if (c.max_scored > 0) h->spill_cap = c.max_scored < h->np ? c.max_scored : h->np;
-    if (!ndft_scores_in_place(c.n_freq, band_size)) h->spill_cap = h->np;      // every pixel must fit in the queue
+    // deferred-scoring queue (row count decided above)
     h->off_spill = o;      o = align_up(o + sizeof(float) * static_cast<size_t>(h->spill_cap) * ndft_padded_bins(c.n_freq));
     h->off_spillrec = o;   o = align_up(o + sizeof(SpillRec) * static_cast<size_t>(h->spill_cap));
     h->off_parent = o;     o = align_up(o + sizeof(int32_t) * h->np);
@@ -390,7 +400,7 @@ static int run_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n, int
     if (timing) cudaEventRecord(h->ev[0], st);
     launches += (mode == 2) ? launch_ingest_slide(ip, st) : launch_ingest(ip, st);
     if (timing) cudaEventRecord(h->ev[1], st);
-    launches += launch_ndft(np, c.n_freq, h->band_size, h->sm_count * h->ndft_blocks_per_sm,
+    launches += launch_ndft(np, c.n_freq, h->band_size, h->fallback, h->sm_count * h->ndft_blocks_per_sm,
                             h->sm_count * h->score_blocks_per_sm, st, timing ? h->ev[2] : nullptr);
     if (timing) cudaEventRecord(h->ev[3], st);
     launches += launch_ccl(cp, st);

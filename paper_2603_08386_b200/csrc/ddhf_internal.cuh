@@ -164,14 +164,15 @@ int ingest_tile_events();                    // events per sort tile
 int ingest_tile_stride(bool compact);        // items per tile slot of IngestParams::items (run padding included)
 size_t ingest_tile_smem(bool compact);       // dynamic shared memory of k_tile_sort
 void ingest_plan(int np, int *bl, int *nb, int *hbits);   // digit split for a sensor of np pixels
-int launch_ndft(const NdftParams &p, int n_freq, int band_size, int grid_ndft, int grid_score, cudaStream_t st, cudaEvent_t between);
+int launch_ndft(const NdftParams &p, int n_freq, int band_size, bool fallback, int grid_ndft, int grid_score, cudaStream_t st, cudaEvent_t between);
+                                             // fallback: the kernel variant that can score a pixel itself (queue smaller than the sensor)
                                              // `between` (optional) is recorded after the NDFT kernel, before the scoring kernel
 int launch_ccl(const CclParams &p, cudaStream_t st);
 int ndft_bins_per_lane(int n_freq);          // 8, 16, 32 or 64
 int ndft_tn(int n_freq);                     // offset pairs per centre for that kernel
 int ndft_padded_bins(int n_freq);            // row length of the deferred-scoring queue
 int ndft_band_size(int n_freq, int r0, int r1);   // sort capacity needed, 0 if unsupported
-cudaError_t ndft_configure(int n_freq, int band_size, int cpad, int *blocks_per_sm, int *score_blocks_per_sm);
+cudaError_t ndft_configure(int n_freq, int band_size, int cpad, bool fallback, int *blocks_per_sm, int *score_blocks_per_sm);
                                              // opt in to the kernels' dynamic shared memory on the current device
 bool ndft_scores_in_place(int n_freq, int band_size);   // whether the NDFT kernel can score a pixel itself when the queue is full
 

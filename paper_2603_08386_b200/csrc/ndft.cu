@@ -57,12 +57,13 @@ constexpr unsigned kFull = 0xffffffffu;
 
 // Per-warp shared memory of k_ndft_score: the phasor table / phase words of the event loop and the
 // staged CSR events; the scoring scratch of comb.cuh (in-place scoring, only when the deferred queue is
-// full) aliases the table.  INPLACE = false (band sorter of 1024 values): the queue holds every pixel.
-template <int TM, int TN, int BS>
+// full) aliases the table.  INPLACE = false (lean variant, or band sorter of 1024 values): the queue holds every pixel,
+// and the small layout leaves the L1 cache to the kernel's spills and global loads.
+template <int TM, int TN, int BS, bool FB>
 struct Layout {
     static constexpr int NBL = TM * 2 * TN;                 // bins per lane
     static constexpr int NB = NBL * 32;                     // padded spectrum length
-    static constexpr bool INPLACE = BS <= 512;
+    static constexpr bool INPLACE = FB && BS <= 512;
     static constexpr int TAB_WORDS = kEC * TN * 2 + kEC * 4;
     static constexpr int EV_WORDS = 2 * kEC;                // staged CSR events, double buffered
     __host__ __device__ static constexpr int scratch_words(int cpad)
@@ -142,14 +143,16 @@ __device__ __forceinline__ WorkItem make_item()
 // The fused kernel.
 // ----------------------------------------------------------------------------------------
 // FULL: n_freq fills the padded grid (n_freq == 32 NBL) and k_lo <= 32, so no per-bin range checks
-template <int TM, int TN, int BS, bool FULL>
+// FB: carries the in-place scoring fallback for a full queue (launched only when the queue is smaller than
+// the sensor: the fallback's code costs the lean kernel 1.7 % of its time just by being there)
+template <int TM, int TN, int BS, bool FULL, bool FB>
 #ifdef DDHF_NDFT_MAXNREG
 __global__ void __maxnreg__(DDHF_NDFT_MAXNREG) k_ndft_score(NdftParams p)
 #else
 __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(NdftParams p)
 #endif
 {
-    using L = Layout<TM, TN, BS>;
+    using L = Layout<TM, TN, BS, FB>;
     constexpr int NBL = L::NBL;
     extern __shared__ __align__(16) uint32_t smem_raw[];
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -541,27 +544,27 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 4) k_comb_deferred(NdftParam
     if (blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(p.n_scored, n_rows);
 }
 
-template <int TM, int TN, int BS, bool FULL>
+template <int TM, int TN, int BS, bool FULL, bool FB>
 int launch_one(const NdftParams &p, int grid_ndft, int grid_score, cudaStream_t st, cudaEvent_t between)
 {
-    using L = Layout<TM, TN, BS>;
+    using L = Layout<TM, TN, BS, FB>;
     const size_t score_smem = static_cast<size_t>(CombSmem<L::NBL, BS>::words(p.sp.cpad)) * 4 * kScoreWarps;
-    k_ndft_score<TM, TN, BS, FULL><<<grid_ndft, kWarps * 32, L::smem_bytes(p.sp.cpad), st>>>(p);
+    k_ndft_score<TM, TN, BS, FULL, FB><<<grid_ndft, kWarps * 32, L::smem_bytes(p.sp.cpad), st>>>(p);
     if (between) cudaEventRecord(between, st);
     k_comb_deferred<L::NBL, BS><<<grid_score, kScoreWarps * 32, score_smem, st>>>(p);
     return 2;
 }
 
-template <int TM, int TN, int BS, bool FULL>
+template <int TM, int TN, int BS, bool FULL, bool FB>
 cudaError_t configure_one(int cpad, int *blocks_per_sm, int *score_blocks_per_sm)
 {
-    using L = Layout<TM, TN, BS>;
+    using L = Layout<TM, TN, BS, FB>;
     const size_t smem = L::smem_bytes(cpad);
     const size_t score_smem = static_cast<size_t>(CombSmem<L::NBL, BS>::words(cpad)) * 4 * kScoreWarps;
-    cudaError_t e = cudaFuncSetAttribute(k_ndft_score<TM, TN, BS, FULL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaError_t e = cudaFuncSetAttribute(k_ndft_score<TM, TN, BS, FULL, FB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          static_cast<int>(smem));
     if (e != cudaSuccess) return e;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, k_ndft_score<TM, TN, BS, FULL>, kWarps * 32, smem);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, k_ndft_score<TM, TN, BS, FULL, FB>, kWarps * 32, smem);
     if (e != cudaSuccess) return e;
     if (*blocks_per_sm < 1) return cudaErrorLaunchOutOfResources;
     e = cudaFuncSetAttribute(k_comb_deferred<L::NBL, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -622,39 +625,42 @@ auto dispatch(int n_freq, int bs, F &&f)
 }
 
 struct ConfigureFn {
-    int cpad; int *b1, *b2;
+    int cpad; bool fb; int *b1, *b2;
     template <int TM, int TN, int BS> cudaError_t operator()() const
     {
-        cudaError_t e = configure_one<TM, TN, BS, true>(cpad, b1, b2);
-        if (e != cudaSuccess) return e;
         int x, y;
-        e = configure_one<TM, TN, BS, false>(cpad, &x, &y);
+        cudaError_t e = fb ? configure_one<TM, TN, BS, true, true>(cpad, b1, b2) : configure_one<TM, TN, BS, true, false>(cpad, b1, b2);
+        if (e != cudaSuccess) return e;
+        e = fb ? configure_one<TM, TN, BS, false, true>(cpad, &x, &y) : configure_one<TM, TN, BS, false, false>(cpad, &x, &y);
         if (e == cudaSuccess) { *b1 = x < *b1 ? x : *b1; *b2 = y < *b2 ? y : *b2; }
         return e;
     }
 };
 
 struct LaunchFn {
-    const NdftParams &p; bool full; int g1, g2; cudaStream_t st; cudaEvent_t between;
+    const NdftParams &p; bool full, fb; int g1, g2; cudaStream_t st; cudaEvent_t between;
     template <int TM, int TN, int BS> int operator()() const
     {
-        return full ? launch_one<TM, TN, BS, true>(p, g1, g2, st, between)
-                    : launch_one<TM, TN, BS, false>(p, g1, g2, st, between);
+        if (fb)
+            return full ? launch_one<TM, TN, BS, true, true>(p, g1, g2, st, between)
+                        : launch_one<TM, TN, BS, false, true>(p, g1, g2, st, between);
+        return full ? launch_one<TM, TN, BS, true, false>(p, g1, g2, st, between)
+                    : launch_one<TM, TN, BS, false, false>(p, g1, g2, st, between);
     }
 };
 
 }  // namespace
 
-cudaError_t ndft_configure(int n_freq, int band_size, int cpad, int *blocks_per_sm, int *score_blocks_per_sm)
+cudaError_t ndft_configure(int n_freq, int band_size, int cpad, bool fallback, int *blocks_per_sm, int *score_blocks_per_sm)
 {
-    return dispatch(n_freq, band_size, ConfigureFn{cpad, blocks_per_sm, score_blocks_per_sm});
+    return dispatch(n_freq, band_size, ConfigureFn{cpad, fallback, blocks_per_sm, score_blocks_per_sm});
 }
 
-int launch_ndft(const NdftParams &p, int n_freq, int band_size, int grid_ndft, int grid_score, cudaStream_t st,
+int launch_ndft(const NdftParams &p, int n_freq, int band_size, bool fallback, int grid_ndft, int grid_score, cudaStream_t st,
                 cudaEvent_t between)
 {
     const bool full = (n_freq == ndft_bins_per_lane(n_freq) * 32) && (p.sp.k_lo <= 32);
-    return dispatch(n_freq, band_size, LaunchFn{p, full, grid_ndft, grid_score, st, between});
+    return dispatch(n_freq, band_size, LaunchFn{p, full, fallback, grid_ndft, grid_score, st, between});
 }
 
 }  // namespace ddhf
