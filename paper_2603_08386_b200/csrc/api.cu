@@ -29,10 +29,10 @@ struct ddhf_handle {
     uint64_t g_f0 = 0, g_d = 0, g_h = 0;
     unsigned char *d_tables = nullptr;      // comb tables (num_tab | piece_tab | meta)
     int band_size = 0;
-    int ndft_blocks_per_sm = 1, score_blocks_per_sm = 1;
+    int ndft_blocks_per_sm = 1, full_blocks_per_sm = 1, score_blocks_per_sm = 1;
     // workspace offsets (bytes)
     size_t off_cnt = 0, off_items = 0, off_scratch = 0, off_work = 0, off_tiles = 0, off_class = 0, off_cursor = 0, off_runs = 0, off_bkt = 0, off_rows = 0, off_spill = 0, off_spillrec = 0,
-           off_parent = 0, off_rec = 0, off_ctiles = 0, off_merge = 0, off_slide = 0, off_split = 0, off_splitcnt = 0, off_partial = 0, ws_bytes = 0;
+           off_parent = 0, off_rec = 0, off_ctiles = 0, off_merge = 0, off_slide = 0, off_segwork = 0, off_split = 0, off_splitcnt = 0, off_partial = 0, ws_bytes = 0;
     cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     bool timed_once = false;
     // buffers of the host-buffer variant
@@ -229,7 +229,8 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
         h->fallback = h->spill_cap < h->np;
     }
     if (ingest_configure() != cudaSuccess ||
-        ndft_configure(c.n_freq, band_size, cpad, h->fallback, &h->ndft_blocks_per_sm, &h->score_blocks_per_sm) != cudaSuccess) {
+        ndft_configure(c.n_freq, band_size, cpad, h->fallback, &h->ndft_blocks_per_sm, &h->full_blocks_per_sm,
+                       &h->score_blocks_per_sm) != cudaSuccess) {
         const std::string msg = std::string("ddhf_create: ") + cudaGetErrorString(cudaGetLastError());
         cudaFree(h->d_tables);
         delete h;
@@ -264,6 +265,7 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
     const size_t max_rows = static_cast<size_t>(c.max_events) / kSplitMin + 1;          // rows that can be split
     const size_t max_slots = max_segs * kSplitFan / (kSplitFan - 1) + 4 * max_rows + 64;   // leaves + inner nodes, rounding per level
     h->off_work = o;       o = align_up(o + sizeof(WorkItem) * (static_cast<size_t>(h->np) + max_segs));
+    h->off_segwork = o;    o = align_up(o + sizeof(WorkItem) * max_segs);            // segment list of the lean NDFT variant
     h->off_split = o;      o = align_up(o + sizeof(SplitRow) * max_rows);
     h->off_splitcnt = o;   o = align_up(o + sizeof(int32_t) * (max_segs + 4 * max_rows + 64));
     h->off_partial = o;    o = align_up(o + sizeof(float) * max_slots * 2 * ndft_padded_bins(c.n_freq));
@@ -365,6 +367,10 @@ static int run_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n, int
         ip.csr_cap = static_cast<int32_t>(c.max_events);
     }
     ip.split_tab = reinterpret_cast<SplitRow *>(ws + h->off_split);
+    if (!h->fallback) {
+        ip.seg_work = reinterpret_cast<WorkItem *>(ws + h->off_segwork);
+        ip.work_cursor2 = reinterpret_cast<unsigned long long *>(ws + h->off_cursor + 96);
+    }
     ip.split_cnt = reinterpret_cast<int32_t *>(ws + h->off_splitcnt);
     ip.ccl_parent = cp_parent;
 
@@ -400,7 +406,10 @@ static int run_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n, int
     if (timing) cudaEventRecord(h->ev[0], st);
     launches += (mode == 2) ? launch_ingest_slide(ip, st) : launch_ingest(ip, st);
     if (timing) cudaEventRecord(h->ev[1], st);
-    launches += launch_ndft(np, c.n_freq, h->band_size, h->fallback, h->sm_count * h->ndft_blocks_per_sm,
+    NdftParams seg = np;                                   // the segment pass of the lean variant
+    seg.work = ip.seg_work; seg.n_work = ip.sync + 9; seg.work_cursor = ip.work_cursor2;
+    launches += launch_ndft(np, h->fallback ? nullptr : &seg, c.n_freq, h->band_size, h->fallback,
+                            h->sm_count * h->ndft_blocks_per_sm, h->sm_count * h->full_blocks_per_sm,
                             h->sm_count * h->score_blocks_per_sm, st, timing ? h->ev[2] : nullptr);
     if (timing) cudaEventRecord(h->ev[3], st);
     launches += launch_ccl(cp, st);

@@ -29,6 +29,7 @@ struct __align__(16) WorkItem {
 constexpr int kSplitMin = 4096;
 constexpr int kSegEvents = 512;
 constexpr int kSplitFan = 8;
+constexpr int kMaxSegs = 1536;
 struct __align__(16) SplitRow {
     int32_t pix, arow;           // the row's identity (arow: row of the compact outputs)
     int32_t n_seg;               // segments of the row = leaves of its tree
@@ -113,9 +114,12 @@ struct IngestParams {
     int32_t *bkt_total, *bkt_base;   // [nb + 2] events per bucket; exclusive scan (bkt_base[nb] = n_in)
     int32_t *chunk_rows;         // [max_rows][4 + 2^bl] chunk table of the multi-chunk buckets
     int32_t *sync;               // [16] 0: tiles finished, 1: chunk rows handed out, 2-3: scoring queue counts,
-                                 //     4: work items, 5: split rows, 6: partials, 7: arrival counters handed out, 8: box-merge CTAs finished
+                                 //     4: work items, 5: split rows, 6: partials, 7: arrival counters handed out, 8: box-merge CTAs finished,
+                                 //     9: items of the segment list
     SplitRow *split_tab;         // rows longer than kSplitMin (see NdftParams)
     int32_t *split_cnt;
+    WorkItem *seg_work;          // when set: the segments of split rows go to this list (count in sync[9]) instead of `work`
+    unsigned long long *work_cursor2;   // cursor of the segment pass
     // sliding windows (ddhf_window_slide): NULL otherwise
     const int32_t *prev_row_ptr; // [np + 1] CSR of the previous window (workspace copy)
     const uint32_t *prev_csr;
@@ -164,15 +168,18 @@ int ingest_tile_events();                    // events per sort tile
 int ingest_tile_stride(bool compact);        // items per tile slot of IngestParams::items (run padding included)
 size_t ingest_tile_smem(bool compact);       // dynamic shared memory of k_tile_sort
 void ingest_plan(int np, int *bl, int *nb, int *hbits);   // digit split for a sensor of np pixels
-int launch_ndft(const NdftParams &p, int n_freq, int band_size, bool fallback, int grid_ndft, int grid_score, cudaStream_t st, cudaEvent_t between);
-                                             // fallback: the kernel variant that can score a pixel itself (queue smaller than the sensor)
+int launch_ndft(const NdftParams &p, const NdftParams *seg_pass, int n_freq, int band_size, bool fallback, int grid_ndft, int grid_seg,
+                int grid_score, cudaStream_t st, cudaEvent_t between);
+                                             // fallback: the full kernel variant (scores a pixel itself when the queue is full, combines
+                                             // split rows); else the lean variant, followed by the full one on `seg_pass` (the segment list)
                                              // `between` (optional) is recorded after the NDFT kernel, before the scoring kernel
 int launch_ccl(const CclParams &p, cudaStream_t st);
 int ndft_bins_per_lane(int n_freq);          // 8, 16, 32 or 64
 int ndft_tn(int n_freq);                     // offset pairs per centre for that kernel
 int ndft_padded_bins(int n_freq);            // row length of the deferred-scoring queue
 int ndft_band_size(int n_freq, int r0, int r1);   // sort capacity needed, 0 if unsupported
-cudaError_t ndft_configure(int n_freq, int band_size, int cpad, bool fallback, int *blocks_per_sm, int *score_blocks_per_sm);
+cudaError_t ndft_configure(int n_freq, int band_size, int cpad, bool fallback, int *blocks_per_sm, int *full_blocks_per_sm,
+                           int *score_blocks_per_sm);
                                              // opt in to the kernels' dynamic shared memory on the current device
 bool ndft_scores_in_place(int n_freq, int band_size);   // whether the NDFT kernel can score a pixel itself when the queue is full
 

@@ -71,13 +71,19 @@ __device__ __forceinline__ int size_class(int n)
     return min(kNumClasses - 1, max(0, bl - 3));
 }
 
-// A row longer than kSplitMin becomes n_seg work items of seg_len <= kSegEvents events (the last one shorter).
+// A row longer than kSplitMin becomes n_seg work items of seg_len events (the last one shorter); seg_len <= kSegEvents
+// unless the row is longer than kMaxSegs * kSegEvents.
 __device__ __forceinline__ int row_segments(int n, int &seg_len)
 {
-    const int n_seg = (n > kSplitMin) ? (n + kSegEvents - 1) / kSegEvents : 1;
+    // at most kMaxSegs segments per row: one round of the segment pass on a B200 (148 SMs x 12 warps)
+    const int n_seg = (n > kSplitMin) ? min((n + kSegEvents - 1) / kSegEvents, kMaxSegs) : 1;
     seg_len = (n + n_seg - 1) / n_seg;
     return n_seg;
 }
+
+// Items a row of n_seg segments adds to the size-classed work list: its segments, unless they go to the
+// segment list of their own (lean NDFT kernel followed by the segment pass)
+__device__ __forceinline__ int class_items(const IngestParams &p, int n_seg) { return (p.seg_work && n_seg > 1) ? 0 : n_seg; }
 
 // ---- k_init: per-pixel maps for inactive pixels, zeroed totals and counters ---------------
 __global__ void k_init(IngestParams p)
@@ -98,7 +104,7 @@ __global__ void k_init(IngestParams p)
             p.class_cur[threadIdx.x] = 0;
         }
         if (threadIdx.x < 16) p.sync[threadIdx.x] = 0;
-        if (threadIdx.x == 0) *p.work_cursor = 0ull;
+        if (threadIdx.x == 0) { *p.work_cursor = 0ull; if (p.work_cursor2) *p.work_cursor2 = 0ull; }
     }
 }
 
@@ -582,7 +588,7 @@ __global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
             int seg_len;
             const int n_seg = row_segments(n, seg_len);
             atomicAdd(&s_act, 1);
-            atomicAdd(&s_class[size_class(seg_len)], n_seg);
+            if (class_items(p, n_seg)) atomicAdd(&s_class[size_class(seg_len)], class_items(p, n_seg));
         }
     };
     auto publish_tally = [&]() {
@@ -830,7 +836,8 @@ __device__ __forceinline__ void emit_work(const IngestParams &p, WorkItem *dst, 
         *dst = it;
         return;
     }
-    // split row: the row's identity goes to the split table
+    // split row: the row's identity goes to the split table, its segments to the segment list if there is one
+    if (p.seg_work) dst = p.seg_work + atomicAdd(p.sync + 9, n_seg);
     const int sid = atomicAdd(p.sync + 5, 1);
     SplitRow sr;
     const int nodes = split_nodes(n_seg);
@@ -868,7 +875,7 @@ __global__ void __launch_bounds__(1024) k_scan_reduce(IngestParams p)
             ++act;
             int seg_len;
             const int n_seg = row_segments(v[j], seg_len);
-            atomicAdd(&s_cls[size_class(seg_len)], n_seg);
+            if (class_items(p, n_seg)) atomicAdd(&s_cls[size_class(seg_len)], class_items(p, n_seg));
         }
     }
     int ta, tb;
@@ -930,7 +937,7 @@ __global__ void __launch_bounds__(1024) k_scan_apply(IngestParams p)
             ++act;
             int seg_len;
             const int n_seg = row_segments(v[j], seg_len);
-            lrank[j] = atomicAdd(&s_cls[size_class(seg_len)], n_seg);
+            lrank[j] = atomicAdd(&s_cls[size_class(seg_len)], class_items(p, n_seg));
         }
     }
     int ta, tb;
@@ -1005,7 +1012,7 @@ __global__ void __launch_bounds__(1024) k_worklist(IngestParams p)
             ++act;
             int seg_len;
             const int n_seg = row_segments(v[j], seg_len);
-            lrank[j] = atomicAdd(&s_cls[size_class(seg_len)], n_seg);
+            lrank[j] = atomicAdd(&s_cls[size_class(seg_len)], class_items(p, n_seg));
         }
     }
     int t1, t2;

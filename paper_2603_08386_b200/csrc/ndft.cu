@@ -308,7 +308,7 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
         // children in index order, whoever that warp is, so the result does not depend on the schedule;
         // the warp that completes the root runs the row's epilogue.
         int out_pix = it.pix, out_arow = it.arow;
-        if (__builtin_expect(it.pix < 0, 0)) {
+        if (FB && it.pix < 0) {
             const SplitRow *sr = p.split_tab + (it.pix & 0x7fffffff);
             constexpr int PW = 2 * NBL * 32;                       // floats per partial
             int n_l = sr->n_seg, idx_l = it.arow;                  // nodes of the current level, this warp's node
@@ -545,14 +545,23 @@ __global__ void __launch_bounds__(kScoreWarps * 32, 4) k_comb_deferred(NdftParam
 }
 
 template <int TM, int TN, int BS, bool FULL, bool FB>
-int launch_one(const NdftParams &p, int grid_ndft, int grid_score, cudaStream_t st, cudaEvent_t between)
+int launch_one(const NdftParams &p, const NdftParams *seg_pass, int grid_ndft, int grid_seg, int grid_score, cudaStream_t st,
+               cudaEvent_t between)
 {
     using L = Layout<TM, TN, BS, FB>;
     const size_t score_smem = static_cast<size_t>(CombSmem<L::NBL, BS>::words(p.sp.cpad)) * 4 * kScoreWarps;
+    int launches = 2;
     k_ndft_score<TM, TN, BS, FULL, FB><<<grid_ndft, kWarps * 32, L::smem_bytes(p.sp.cpad), st>>>(p);
+    if (!FB && seg_pass) {
+        // the lean variant's work list holds whole rows only; the segments of split rows go through the
+        // full variant (it leaves at once when there are none)
+        using LF = Layout<TM, TN, BS, true>;
+        k_ndft_score<TM, TN, BS, FULL, true><<<grid_seg, kWarps * 32, LF::smem_bytes(p.sp.cpad), st>>>(*seg_pass);
+        ++launches;
+    }
     if (between) cudaEventRecord(between, st);
     k_comb_deferred<L::NBL, BS><<<grid_score, kScoreWarps * 32, score_smem, st>>>(p);
-    return 2;
+    return launches;
 }
 
 template <int TM, int TN, int BS, bool FULL, bool FB>
@@ -625,42 +634,52 @@ auto dispatch(int n_freq, int bs, F &&f)
 }
 
 struct ConfigureFn {
-    int cpad; bool fb; int *b1, *b2;
+    int cpad; bool fb; int *b1, *bf, *b2;
     template <int TM, int TN, int BS> cudaError_t operator()() const
     {
         int x, y;
-        cudaError_t e = fb ? configure_one<TM, TN, BS, true, true>(cpad, b1, b2) : configure_one<TM, TN, BS, true, false>(cpad, b1, b2);
+        // the full variant is always needed (as the main kernel, or for the segment pass)
+        cudaError_t e = configure_one<TM, TN, BS, true, true>(cpad, bf, b2);
         if (e != cudaSuccess) return e;
-        e = fb ? configure_one<TM, TN, BS, false, true>(cpad, &x, &y) : configure_one<TM, TN, BS, false, false>(cpad, &x, &y);
-        if (e == cudaSuccess) { *b1 = x < *b1 ? x : *b1; *b2 = y < *b2 ? y : *b2; }
+        e = configure_one<TM, TN, BS, false, true>(cpad, &x, &y);
+        if (e != cudaSuccess) return e;
+        *bf = x < *bf ? x : *bf; *b2 = y < *b2 ? y : *b2;
+        *b1 = *bf;
+        if (!fb) {
+            e = configure_one<TM, TN, BS, true, false>(cpad, b1, &y);
+            if (e != cudaSuccess) return e;
+            e = configure_one<TM, TN, BS, false, false>(cpad, &x, &y);
+            if (e == cudaSuccess) *b1 = x < *b1 ? x : *b1;
+        }
         return e;
     }
 };
 
 struct LaunchFn {
-    const NdftParams &p; bool full, fb; int g1, g2; cudaStream_t st; cudaEvent_t between;
+    const NdftParams &p; const NdftParams *seg; bool full, fb; int g1, gs, g2; cudaStream_t st; cudaEvent_t between;
     template <int TM, int TN, int BS> int operator()() const
     {
         if (fb)
-            return full ? launch_one<TM, TN, BS, true, true>(p, g1, g2, st, between)
-                        : launch_one<TM, TN, BS, false, true>(p, g1, g2, st, between);
-        return full ? launch_one<TM, TN, BS, true, false>(p, g1, g2, st, between)
-                    : launch_one<TM, TN, BS, false, false>(p, g1, g2, st, between);
+            return full ? launch_one<TM, TN, BS, true, true>(p, seg, g1, gs, g2, st, between)
+                        : launch_one<TM, TN, BS, false, true>(p, seg, g1, gs, g2, st, between);
+        return full ? launch_one<TM, TN, BS, true, false>(p, seg, g1, gs, g2, st, between)
+                    : launch_one<TM, TN, BS, false, false>(p, seg, g1, gs, g2, st, between);
     }
 };
 
 }  // namespace
 
-cudaError_t ndft_configure(int n_freq, int band_size, int cpad, bool fallback, int *blocks_per_sm, int *score_blocks_per_sm)
+cudaError_t ndft_configure(int n_freq, int band_size, int cpad, bool fallback, int *blocks_per_sm, int *full_blocks_per_sm,
+                           int *score_blocks_per_sm)
 {
-    return dispatch(n_freq, band_size, ConfigureFn{cpad, fallback, blocks_per_sm, score_blocks_per_sm});
+    return dispatch(n_freq, band_size, ConfigureFn{cpad, fallback, blocks_per_sm, full_blocks_per_sm, score_blocks_per_sm});
 }
 
-int launch_ndft(const NdftParams &p, int n_freq, int band_size, bool fallback, int grid_ndft, int grid_score, cudaStream_t st,
-                cudaEvent_t between)
+int launch_ndft(const NdftParams &p, const NdftParams *seg_pass, int n_freq, int band_size, bool fallback, int grid_ndft, int grid_seg,
+                int grid_score, cudaStream_t st, cudaEvent_t between)
 {
     const bool full = (n_freq == ndft_bins_per_lane(n_freq) * 32) && (p.sp.k_lo <= 32);
-    return dispatch(n_freq, band_size, LaunchFn{p, full, fallback, grid_ndft, grid_score, st, between});
+    return dispatch(n_freq, band_size, LaunchFn{p, seg_pass, full, fallback, grid_ndft, grid_seg, grid_score, st, between});
 }
 
 }  // namespace ddhf
