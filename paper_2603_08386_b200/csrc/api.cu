@@ -367,7 +367,7 @@ static int run_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n, int
         ip.csr_cap = static_cast<int32_t>(c.max_events);
     }
     ip.split_tab = reinterpret_cast<SplitRow *>(ws + h->off_split);
-    if (!h->fallback) {
+    if (!h->fallback && ndft_bins_per_lane(c.n_freq) == 64) {      // lean 2048-bin kernel: segments in a second pass
         ip.seg_work = reinterpret_cast<WorkItem *>(ws + h->off_segwork);
         ip.work_cursor2 = reinterpret_cast<unsigned long long *>(ws + h->off_cursor + 96);
     }
@@ -408,7 +408,7 @@ static int run_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n, int
     if (timing) cudaEventRecord(h->ev[1], st);
     NdftParams seg = np;                                   // the segment pass of the lean variant
     seg.work = ip.seg_work; seg.n_work = ip.sync + 9; seg.work_cursor = ip.work_cursor2;
-    launches += launch_ndft(np, h->fallback ? nullptr : &seg, c.n_freq, h->band_size, h->fallback,
+    launches += launch_ndft(np, ip.seg_work ? &seg : nullptr, c.n_freq, h->band_size, h->fallback,
                             h->sm_count * h->ndft_blocks_per_sm, h->sm_count * h->full_blocks_per_sm,
                             h->sm_count * h->score_blocks_per_sm, st, timing ? h->ev[2] : nullptr);
     if (timing) cudaEventRecord(h->ev[3], st);

@@ -308,7 +308,7 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
         // children in index order, whoever that warp is, so the result does not depend on the schedule;
         // the warp that completes the root runs the row's epilogue.
         int out_pix = it.pix, out_arow = it.arow;
-        if (FB && it.pix < 0) {
+        if ((FB || TM == 1) && it.pix < 0) {      // (the 168-register TM = 2 lean kernel leaves segments to a second pass)
             const SplitRow *sr = p.split_tab + (it.pix & 0x7fffffff);
             constexpr int PW = 2 * NBL * 32;                       // floats per partial
             int n_l = sr->n_seg, idx_l = it.arow;                  // nodes of the current level, this warp's node
@@ -552,7 +552,7 @@ int launch_one(const NdftParams &p, const NdftParams *seg_pass, int grid_ndft, i
     const size_t score_smem = static_cast<size_t>(CombSmem<L::NBL, BS>::words(p.sp.cpad)) * 4 * kScoreWarps;
     int launches = 2;
     k_ndft_score<TM, TN, BS, FULL, FB><<<grid_ndft, kWarps * 32, L::smem_bytes(p.sp.cpad), st>>>(p);
-    if (!FB && seg_pass) {
+    if (!FB && TM == 2 && seg_pass) {
         // the lean variant's work list holds whole rows only; the segments of split rows go through the
         // full variant (it leaves at once when there are none)
         using LF = Layout<TM, TN, BS, true>;
