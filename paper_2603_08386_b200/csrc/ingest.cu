@@ -539,9 +539,13 @@ template <bool COMPACT>
 __device__ __forceinline__ void sort_chunk_any(typename BucketItem<COMPACT>::type *buf, uint32_t *cnt, uint32_t *rstart,
                                                uint32_t *s_warp, int fill, int bl, int vb)
 {
-    if (fill <= 8 * kNT) sort_chunk<8, COMPACT>(buf, cnt, rstart, s_warp, fill, bl, vb);
-    else if (!COMPACT || fill <= 16 * kNT) sort_chunk<16, COMPACT>(buf, cnt, rstart, s_warp, fill, bl, vb);
-    else if (fill <= 24 * kNT) sort_chunk<COMPACT ? 24 : 16, COMPACT>(buf, cnt, rstart, s_warp, fill, bl, vb);
+    const int k = (fill + kNT - 1) / kNT;                      // items per thread needed
+    if (k <= 8) sort_chunk<8, COMPACT>(buf, cnt, rstart, s_warp, fill, bl, vb);
+    else if (k <= 12) sort_chunk<12, COMPACT>(buf, cnt, rstart, s_warp, fill, bl, vb);
+    else if (!COMPACT || k <= 16) sort_chunk<16, COMPACT>(buf, cnt, rstart, s_warp, fill, bl, vb);
+    else if (k <= 20) sort_chunk<COMPACT ? 20 : 16, COMPACT>(buf, cnt, rstart, s_warp, fill, bl, vb);
+    else if (k <= 24) sort_chunk<COMPACT ? 24 : 16, COMPACT>(buf, cnt, rstart, s_warp, fill, bl, vb);
+    else if (k <= 28) sort_chunk<COMPACT ? 28 : 16, COMPACT>(buf, cnt, rstart, s_warp, fill, bl, vb);
     else sort_chunk<BucketCfg<COMPACT>::kMaxK, COMPACT>(buf, cnt, rstart, s_warp, fill, bl, vb);
 }
 
