@@ -308,7 +308,7 @@ __global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(Nd
         // children in index order, whoever that warp is, so the result does not depend on the schedule;
         // the warp that completes the root runs the row's epilogue.
         int out_pix = it.pix, out_arow = it.arow;
-        if ((FB || TM == 1) && it.pix < 0) {      // (the 168-register TM = 2 lean kernel leaves segments to a second pass)
+        if ((FB || NBL < 64) && it.pix < 0) {     // (the 168-register 2048-bin lean kernel leaves segments to a second pass)
             const SplitRow *sr = p.split_tab + (it.pix & 0x7fffffff);
             constexpr int PW = 2 * NBL * 32;                       // floats per partial
             int n_l = sr->n_seg, idx_l = it.arow;                  // nodes of the current level, this warp's node
@@ -552,7 +552,7 @@ int launch_one(const NdftParams &p, const NdftParams *seg_pass, int grid_ndft, i
     const size_t score_smem = static_cast<size_t>(CombSmem<L::NBL, BS>::words(p.sp.cpad)) * 4 * kScoreWarps;
     int launches = 2;
     k_ndft_score<TM, TN, BS, FULL, FB><<<grid_ndft, kWarps * 32, L::smem_bytes(p.sp.cpad), st>>>(p);
-    if (!FB && TM == 2 && seg_pass) {
+    if (!FB && L::NBL == 64 && seg_pass) {
         // the lean variant's work list holds whole rows only; the segments of split rows go through the
         // full variant (it leaves at once when there are none)
         using LF = Layout<TM, TN, BS, true>;
@@ -601,7 +601,7 @@ int ndft_padded_bins(int n_freq) { return ndft_bins_per_lane(n_freq) * 32; }
 int ndft_tn(int n_freq)
 {
     const int nbl = ndft_bins_per_lane(n_freq);
-    return nbl >= 32 ? 16 : nbl / 2;
+    return nbl == 64 ? 16 : nbl == 32 ? 8 : nbl / 2;      // 32 bins per lane: two centres x 8 offset pairs
 }
 
 int ndft_band_size(int n_freq, int r0, int r1)
@@ -627,8 +627,8 @@ auto dispatch(int n_freq, int bs, F &&f)
     const int nbl = ndft_bins_per_lane(n_freq);
     if (nbl == 8) return f.template operator()<1, 4, 256>();
     if (nbl == 16) return bs == 256 ? f.template operator()<1, 8, 256>() : f.template operator()<1, 8, 512>();
-    if (nbl == 32) return bs == 256 ? f.template operator()<1, 16, 256>()
-                        : bs == 512 ? f.template operator()<1, 16, 512>() : f.template operator()<1, 16, 1024>();
+    if (nbl == 32) return bs == 256 ? f.template operator()<2, 8, 256>()
+                        : bs == 512 ? f.template operator()<2, 8, 512>() : f.template operator()<2, 8, 1024>();
     return bs == 256 ? f.template operator()<2, 16, 256>()
          : bs == 512 ? f.template operator()<2, 16, 512>() : f.template operator()<2, 16, 1024>();
 }
