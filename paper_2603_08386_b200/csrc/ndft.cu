@@ -52,6 +52,11 @@ namespace {
 #define DDHF_NDFT_BLOCKS 1         // CTAs per SM
 #endif
 constexpr int kWarps = DDHF_NDFT_WARPS;
+#ifndef DDHF_NDFT_WARPS_SMALL
+#define DDHF_NDFT_WARPS_SMALL 16   // kernels of <= 32 bins per lane need <= 128 registers: four warps per sub-partition
+#endif
+// warps per CTA of the kernel with NBL bins per lane
+__host__ __device__ constexpr int warps_of(int nbl) { return nbl >= 64 ? kWarps : DDHF_NDFT_WARPS_SMALL; }
 constexpr int kEC = 32;            // events per table chunk
 constexpr unsigned kFull = 0xffffffffu;
 
@@ -71,7 +76,7 @@ struct Layout {
         return INPLACE && CombSmem<NBL, BS>::words(cpad) > TAB_WORDS ? CombSmem<NBL, BS>::words(cpad) : TAB_WORDS;
     }
     __host__ __device__ static constexpr int warp_words(int cpad) { return ((scratch_words(cpad) + EV_WORDS + 3) / 4) * 4; }
-    static size_t smem_bytes(int cpad) { return static_cast<size_t>(warp_words(cpad)) * 4 * kWarps; }
+    static size_t smem_bytes(int cpad) { return static_cast<size_t>(warp_words(cpad)) * 4 * warps_of(NBL); }
 };
 
 __device__ __forceinline__ uint32_t phase_u32(uint64_t g, uint32_t t)
@@ -149,7 +154,7 @@ template <int TM, int TN, int BS, bool FULL, bool FB>
 #ifdef DDHF_NDFT_MAXNREG
 __global__ void __maxnreg__(DDHF_NDFT_MAXNREG) k_ndft_score(NdftParams p)
 #else
-__global__ void __launch_bounds__(kWarps * 32, DDHF_NDFT_BLOCKS) k_ndft_score(NdftParams p)
+__global__ void __launch_bounds__(warps_of(TM * 2 * TN) * 32, DDHF_NDFT_BLOCKS) k_ndft_score(NdftParams p)
 #endif
 {
     using L = Layout<TM, TN, BS, FB>;
@@ -551,12 +556,12 @@ int launch_one(const NdftParams &p, const NdftParams *seg_pass, int grid_ndft, i
     using L = Layout<TM, TN, BS, FB>;
     const size_t score_smem = static_cast<size_t>(CombSmem<L::NBL, BS>::words(p.sp.cpad)) * 4 * kScoreWarps;
     int launches = 2;
-    k_ndft_score<TM, TN, BS, FULL, FB><<<grid_ndft, kWarps * 32, L::smem_bytes(p.sp.cpad), st>>>(p);
+    k_ndft_score<TM, TN, BS, FULL, FB><<<grid_ndft, warps_of(L::NBL) * 32, L::smem_bytes(p.sp.cpad), st>>>(p);
     if (!FB && L::NBL == 64 && seg_pass) {
         // the lean variant's work list holds whole rows only; the segments of split rows go through the
         // full variant (it leaves at once when there are none)
         using LF = Layout<TM, TN, BS, true>;
-        k_ndft_score<TM, TN, BS, FULL, true><<<grid_seg, kWarps * 32, LF::smem_bytes(p.sp.cpad), st>>>(*seg_pass);
+        k_ndft_score<TM, TN, BS, FULL, true><<<grid_seg, warps_of(L::NBL) * 32, LF::smem_bytes(p.sp.cpad), st>>>(*seg_pass);
         ++launches;
     }
     if (between) cudaEventRecord(between, st);
@@ -573,7 +578,7 @@ cudaError_t configure_one(int cpad, int *blocks_per_sm, int *score_blocks_per_sm
     cudaError_t e = cudaFuncSetAttribute(k_ndft_score<TM, TN, BS, FULL, FB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          static_cast<int>(smem));
     if (e != cudaSuccess) return e;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, k_ndft_score<TM, TN, BS, FULL, FB>, kWarps * 32, smem);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(blocks_per_sm, k_ndft_score<TM, TN, BS, FULL, FB>, warps_of(L::NBL) * 32, smem);
     if (e != cudaSuccess) return e;
     if (*blocks_per_sm < 1) return cudaErrorLaunchOutOfResources;
     e = cudaFuncSetAttribute(k_comb_deferred<L::NBL, BS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
