@@ -82,17 +82,27 @@ __global__ void k_ccl_merge(CclParams p)
 __global__ void k_ccl_label(CclParams p)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= p.np) return;
-    if (!p.mask[i]) { p.parent[i] = -1; return; }
+    const int lane = threadIdx.x & 31;
+    const bool m = (i < p.np) && p.mask[i];
+    if (i < p.np && !m) p.parent[i] = -1;
+    const unsigned act = __ballot_sync(0xffffffffu, m);
+    if (!m) return;
     const int r = uf_find(p.parent, i);
     p.parent[i] = r;
     const int x = i % p.width, y = i / p.width;
-    int *c = p.rec + 5 * static_cast<size_t>(r);
-    atomicMin(c + 0, x);
-    atomicMin(c + 1, y);
-    atomicMax(c + 2, x);
-    atomicMax(c + 3, y);
-    atomicAdd(c + 4, 1);
+    // the pixels of the warp that share a root update its record once (a dense mask is a few large
+    // components: one atomic per pixel and field on the same five words serialises the whole kernel)
+    const unsigned peers = __match_any_sync(act, r);
+    const int x0 = __reduce_min_sync(peers, x), y0 = __reduce_min_sync(peers, y);
+    const int x1 = __reduce_max_sync(peers, x), y1 = __reduce_max_sync(peers, y);
+    if (lane == __ffs(peers) - 1) {
+        int *c = p.rec + 5 * static_cast<size_t>(r);
+        atomicMin(c + 0, x0);
+        atomicMin(c + 1, y0);
+        atomicMax(c + 2, x1);
+        atomicMax(c + 3, y1);
+        atomicAdd(c + 4, __popc(peers));
+    }
 }
 
 // 0: not a root, 1: root, 3: root whose bounding box passes A_min
