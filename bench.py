@@ -390,11 +390,23 @@ def main():
         for lo, n, t0 in ws:
             binding.ddhf_window_host(det.h, h_ev.data_ptr() + 16 * lo, n, t0, w.window_us, houts[0], cst)
 
+    # the same stream as 8-byte events (ddhf_event8: nothing is lost, results are bit-identical)
+    from paper_2603_08386_b200 import workloads as _wl
+    t_base = int(w.events["t"].min()) if len(w.events) else 0
+    h_ev8 = torch.from_numpy(_wl.pack_events(w.events, t_base).view(np.uint8).copy()).pin_memory()
+
+    def run_packed(ws):
+        for i, (lo, n, t0) in enumerate(ws):
+            binding.ddhf_host_submit_packed(det.h, h_ev8.data_ptr() + 8 * lo, n, t_base, t0, w.window_us, houts[i & 1], cst)
+            if i >= 1:
+                binding.ddhf_host_wait(det.h)
+        binding.ddhf_host_wait(det.h)
+
     e2e_terms = sum(terms_by_win[k][0] for k in e2e_wins)
     h2d = sum(16 * n for _, n, _ in e2e_wins)
     d2h = NP + 64 + 24 * det.cfg.max_boxes
     results = {}
-    for name, fn in (("pipelined", run_pipelined), ("serial", run_serial)):
+    for name, fn in (("pipelined", run_pipelined), ("serial", run_serial), ("packed", run_packed)):
         fn(wins[:2])
         barrier()
         t_start = time.perf_counter()
@@ -403,9 +415,12 @@ def main():
         sec, terms_e = aggregate_over_ranks((time.perf_counter() - t_start) * 1e3, e2e_terms, world, dev)
         sec *= 1e-3
         results[name] = {"value": terms_e / sec / 1e9, "unit": "Gterms/s", "ms_per_step": sec / e2e_steps * 1e3,
-                         "h2d_bytes_per_step": h2d // e2e_steps, "d2h_bytes_per_step": d2h, "steps": e2e_steps}
+                         "h2d_bytes_per_step": (h2d // 2 if name == "packed" else h2d) // e2e_steps, "d2h_bytes_per_step": d2h,
+                         "steps": e2e_steps}
     e2e = dict(results["pipelined"], api="ddhf_host_submit/ddhf_host_wait, 2 windows in flight")
     e2e_serial = dict(results["serial"], api="ddhf_window_host")
+    e2e_packed = dict(results["packed"], api="ddhf_host_submit_packed/ddhf_host_wait, 2 windows in flight, 8-byte events "
+                                             "(ddhf_event8: x, y | polarity << 15, dt from a base time; bit-identical results)")
 
     if rank != 0:
         if world > 1:
@@ -453,12 +468,12 @@ def main():
         "steps": steps, "warmup": warmup, "ms_per_step": rec["ms_per_step"], "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": rec["config"], "latency_ms": rec["latency_ms"],
-        "clocks": rec["clocks"], "e2e": e2e, "e2e_serial": e2e_serial, "gpu_launches": rec["gpu_launches"],
+        "clocks": rec["clocks"], "e2e": e2e, "e2e_serial": e2e_serial, "e2e_packed": e2e_packed, "gpu_launches": rec["gpu_launches"],
         "roofline": roofline, "roofline_stages": roofline_stages,
         "paper_context": "DDHF 2.39 ms/frame, YOLOv11-n 12.40 ms/frame on an NVIDIA L40-8Q, 33.3 ms windows (PAPER.md L154-156)",
     }
     det.close()
-    del h_ev, hbufs, st
+    del h_ev, h_ev8, hbufs, st
     torch.cuda.empty_cache()
 
     # ---- the variants of SURVEY.md section 8(d), each with its own clocks ------------------------------

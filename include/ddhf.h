@@ -73,6 +73,16 @@ typedef struct {
     int64_t  t_us;       /* timestamp in microseconds                                      */
 } ddhf_event;
 
+/* The same tuple in 8 bytes, for streams that cross PCIe every window: coordinates as above, the polarity in
+ * bit 15 of y_p (1: w = +1, 0: w = -1; sensors are < 32768 rows), the timestamp as an offset in microseconds
+ * from a base time that is passed with the call (71 minutes of range).  No information is lost: t = t_base_us
+ * + dt_us, and every result is bit-identical to the 16-byte form (the CSR value is (t - t0) << 1 | polarity). */
+typedef struct {
+    uint16_t x;
+    uint16_t y_p;        /* y | (p > 0) << 15                                              */
+    uint32_t dt_us;      /* t_us - t_base_us                                               */
+} ddhf_event8;
+
 /* Bounding box of one connected component, inclusive corners. */
 typedef struct {
     int32_t x0, y0, x1, y1;
@@ -165,6 +175,10 @@ int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n, int64_t t
                 int64_t window_us, void *d_workspace, const ddhf_outputs *out,
                 void *cuda_stream);
 
+/* ddhf_window() on 8-byte events (ddhf_event8, DEVICE): t = t_base_us + dt_us.  Same outputs, bit for bit. */
+int ddhf_window_packed(ddhf_handle *h, const ddhf_event8 *d_events, int64_t n, int64_t t_base_us, int64_t t0_us,
+                       int64_t window_us, void *d_workspace, const ddhf_outputs *out, void *cuda_stream);
+
 /* Sliding windows ("Events are streamed in temporal windows"): advance the
  * window kept in the workspace to [t0, t0+window).  d_new_events: DEVICE, the n_new events that follow,
  * in the stream, the events handed over by the previous call.  The row of a pixel becomes the previous
@@ -201,6 +215,9 @@ int ddhf_window_host(ddhf_handle *h, const ddhf_event *h_events, int64_t n, int6
 int ddhf_host_submit(ddhf_handle *h, const ddhf_event *h_events, int64_t n, int64_t t0_us,
                      int64_t window_us, const ddhf_host_outputs *out, void *cuda_stream);
 int ddhf_host_wait(ddhf_handle *h);
+/* ddhf_host_submit() on 8-byte events (HOST, pinned): half the bytes over PCIe per window. */
+int ddhf_host_submit_packed(ddhf_handle *h, const ddhf_event8 *h_events, int64_t n, int64_t t_base_us, int64_t t0_us,
+                            int64_t window_us, const ddhf_host_outputs *out, void *cuda_stream);
 
 /* With DDHF_FLAG_TIMING: waits for the last ddhf_window() on this handle and returns the
  * device time of its stages in ms: [0] ingest a0-a3, [1] the NDFT kernel (a4, a5 and the

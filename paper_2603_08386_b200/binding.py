@@ -22,7 +22,8 @@ DDHF_FLAG_SCORE_ALL, DDHF_FLAG_TIMING = 1, 2
 N_COUNTERS = 16
 
 #: every symbol include/ddhf.h declares
-EXPORTS = ["ddhf_create", "ddhf_workspace_bytes", "ddhf_window", "ddhf_window_slide", "ddhf_slide_reset",
+EXPORTS = ["ddhf_create", "ddhf_workspace_bytes", "ddhf_window", "ddhf_window_packed", "ddhf_window_slide", "ddhf_slide_reset",
+           "ddhf_host_submit_packed",
            "ddhf_window_host",
            "ddhf_host_submit", "ddhf_host_wait",
            "ddhf_stage_ms", "ddhf_launches_per_window", "ddhf_fma_peak_probe", "ddhf_destroy",
@@ -79,6 +80,12 @@ def lib() -> C.CDLL:
         L.ddhf_window.restype = C.c_int
         L.ddhf_window.argtypes = [vp, vp, C.c_int64, C.c_int64, C.c_int64, vp,
                                   C.POINTER(DdhfOutputs), vp]
+        L.ddhf_window_packed.restype = C.c_int
+        L.ddhf_window_packed.argtypes = [vp, vp, C.c_int64, C.c_int64, C.c_int64, C.c_int64, vp,
+                                         C.POINTER(DdhfOutputs), vp]
+        L.ddhf_host_submit_packed.restype = C.c_int
+        L.ddhf_host_submit_packed.argtypes = [vp, vp, C.c_int64, C.c_int64, C.c_int64, C.c_int64,
+                                              C.POINTER(DdhfHostOutputs), vp]
         L.ddhf_window_slide.restype = C.c_int
         L.ddhf_window_slide.argtypes = [vp, vp, C.c_int64, C.c_int64, C.c_int64, vp,
                                         C.POINTER(DdhfOutputs), vp]
@@ -149,6 +156,21 @@ def ddhf_window(h, d_events_ptr: int, n: int, t0_us: int, window_us: int, d_work
                 out: DdhfOutputs, stream_ptr: int = 0) -> None:
     rc = lib().ddhf_window(h, d_events_ptr, n, t0_us, window_us, d_workspace_ptr, C.byref(out),
                            stream_ptr)
+    if rc != DDHF_OK:
+        raise DdhfError(rc, (lib().ddhf_last_error(h) or b"").decode())
+
+
+def ddhf_window_packed(h, d_events_ptr: int, n: int, t_base_us: int, t0_us: int, window_us: int, d_workspace_ptr: int,
+                       out: DdhfOutputs, stream_ptr: int = 0) -> None:
+    rc = lib().ddhf_window_packed(h, d_events_ptr, n, t_base_us, t0_us, window_us, d_workspace_ptr, C.byref(out),
+                                  stream_ptr)
+    if rc != DDHF_OK:
+        raise DdhfError(rc, (lib().ddhf_last_error(h) or b"").decode())
+
+
+def ddhf_host_submit_packed(h, h_events_ptr: int, n: int, t_base_us: int, t0_us: int, window_us: int,
+                            out: "DdhfHostOutputs", stream_ptr: int = 0) -> None:
+    rc = lib().ddhf_host_submit_packed(h, h_events_ptr, n, t_base_us, t0_us, window_us, C.byref(out), stream_ptr)
     if rc != DDHF_OK:
         raise DdhfError(rc, (lib().ddhf_last_error(h) or b"").decode())
 
@@ -273,6 +295,15 @@ class Detector:
         ptr = d_events.data_ptr() + 16 * offset_events if n > 0 else 0
         ddhf_window(self.h, ptr, n, t0_us, window_us, self.workspace.data_ptr(), self.out,
                     st.cuda_stream)
+
+    def window_packed(self, d_events8, n: int, t_base_us: int, t0_us: int, window_us: int, *, offset_events: int = 0,
+                      stream=None) -> None:
+        """ddhf_window on 8-byte events (``workloads.pack_events``): uint8 CUDA tensor of ddhf_event8 records."""
+        torch = self.torch
+        st = stream if stream is not None else torch.cuda.current_stream(self.device)
+        ptr = d_events8.data_ptr() + 8 * offset_events if n > 0 else 0
+        ddhf_window_packed(self.h, ptr, n, t_base_us, t0_us, window_us, self.workspace.data_ptr(), self.out,
+                           st.cuda_stream)
 
     def slide(self, d_events, n_new: int, t0_us: int, window_us: int, *, offset_events: int = 0,
               stream=None) -> None:

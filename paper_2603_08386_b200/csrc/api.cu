@@ -307,7 +307,7 @@ extern "C" int ddhf_launches_per_window(const ddhf_handle *h) { return h ? h->la
 // workspace); 2: slide (d_events = the new slab, shift = t0 - previous t0)
 static int run_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n, int64_t t0_us,
                       int64_t window_us, void *d_workspace, const ddhf_outputs *out,
-                      void *cuda_stream, int mode, int64_t shift_us)
+                      void *cuda_stream, int mode, int64_t shift_us, bool packed = false, int64_t t_base_us = 0)
 {
     if (!h) return DDHF_E_INVAL;
     if (!out || !d_workspace || (n > 0 && !d_events))
@@ -318,6 +318,8 @@ static int run_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n, int
     if (n < 0 || window_us <= 0 || window_us >= (1ll << 31))
         return fail(h, DDHF_E_INVAL, "ddhf_window: n or window_us out of range");
     if (n > h->cfg.max_events) return fail(h, DDHF_E_CAPACITY, "ddhf_window: n > max_events");
+    if (packed && h->cfg.height > 32768)
+        return fail(h, DDHF_E_INVAL, "ddhf_window_packed: 8-byte events hold y < 32768");
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     char *ws = static_cast<char *>(d_workspace);
     const ddhf_config &c = h->cfg;
@@ -326,6 +328,7 @@ static int run_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n, int
     int32_t *cp_parent = out->labels ? out->labels : reinterpret_cast<int32_t *>(ws + h->off_parent);
     IngestParams ip{};
     ip.events = d_events; ip.n = n; ip.t0 = t0_us; ip.t1 = t0_us + window_us;
+    ip.packed = packed ? 1 : 0; ip.t_base = t_base_us;
     ip.width = c.width; ip.height = c.height; ip.np = h->np;
     ip.n_min = c.n_min; ip.max_active = c.max_active;
     ip.cnt = reinterpret_cast<int32_t *>(ws + h->off_cnt);
@@ -425,6 +428,13 @@ extern "C" int ddhf_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n
                            void *cuda_stream)
 {
     return run_window(h, d_events, n, t0_us, window_us, d_workspace, out, cuda_stream, 0, 0);
+}
+
+extern "C" int ddhf_window_packed(ddhf_handle *h, const ddhf_event8 *d_events, int64_t n, int64_t t_base_us, int64_t t0_us,
+                                  int64_t window_us, void *d_workspace, const ddhf_outputs *out, void *cuda_stream)
+{
+    return run_window(h, reinterpret_cast<const ddhf_event *>(d_events), n, t0_us, window_us, d_workspace, out, cuda_stream,
+                      0, 0, true, t_base_us);
 }
 
 extern "C" int ddhf_window_slide(ddhf_handle *h, const ddhf_event *d_new_events, int64_t n_new, int64_t t0_us,
@@ -570,11 +580,11 @@ extern "C" int ddhf_window_host(ddhf_handle *h, const ddhf_event *h_events, int6
     return DDHF_OK;
 }
 
-extern "C" int ddhf_host_submit(ddhf_handle *h, const ddhf_event *h_events, int64_t n, int64_t t0_us,
-                                int64_t window_us, const ddhf_host_outputs *out, void *cuda_stream)
+static int host_submit(ddhf_handle *h, const void *h_events, int64_t n, int64_t t0_us, int64_t window_us,
+                       const ddhf_host_outputs *out, void *cuda_stream, bool packed, int64_t t_base_us)
 {
     if (!h) return DDHF_E_INVAL;
-    const int arg_rc = check_host_args(h, "ddhf_host_submit", h_events, n, window_us, out);
+    const int arg_rc = check_host_args(h, "ddhf_host_submit", static_cast<const ddhf_event *>(h_events), n, window_us, out);
     if (arg_rc != DDHF_OK) return arg_rc;
     if (out->csr_ev || out->active_idx || out->power)
         return fail(h, DDHF_E_INVAL, "ddhf_host_submit: csr_ev, active_idx and power are not available in the pipelined call");
@@ -604,7 +614,7 @@ extern "C" int ddhf_host_submit(ddhf_handle *h, const ddhf_event *h_events, int6
     ddhf_handle::PipeSlot &s = h->pipe[h->pipe_head & 1];
     // the slot's previous window (two submits ago) has been waited for, so its buffers are free
     cudaError_t e = cudaSuccess;
-    if (n > 0) e = cudaMemcpyAsync(s.events, h_events, sizeof(ddhf_event) * static_cast<size_t>(n),
+    if (n > 0) e = cudaMemcpyAsync(s.events, h_events, (packed ? sizeof(ddhf_event8) : sizeof(ddhf_event)) * static_cast<size_t>(n),
                                    cudaMemcpyHostToDevice, h->copy_stream);
     if (e == cudaSuccess) e = cudaEventRecord(s.copied, h->copy_stream);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(st, s.copied, 0);
@@ -612,7 +622,7 @@ extern "C" int ddhf_host_submit(ddhf_handle *h, const ddhf_event *h_events, int6
         cudaStreamSynchronize(h->copy_stream);            // nothing was enqueued on `st`: the slot stays free
         return cuda_fail(e);
     }
-    const int rc = ddhf_window(h, s.events, n, t0_us, window_us, s.ws, &s.out, st);
+    const int rc = run_window(h, s.events, n, t0_us, window_us, s.ws, &s.out, st, 0, 0, packed, t_base_us);
     const ddhf_outputs &d = s.out;
     auto d2h = [&](void *dst, const void *src, size_t bytes) {
         if (e == cudaSuccess && dst) e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st);
@@ -640,6 +650,18 @@ extern "C" int ddhf_host_submit(ddhf_handle *h, const ddhf_event *h_events, int6
     }
     ++h->pipe_head;
     return DDHF_OK;
+}
+
+extern "C" int ddhf_host_submit(ddhf_handle *h, const ddhf_event *h_events, int64_t n, int64_t t0_us,
+                                int64_t window_us, const ddhf_host_outputs *out, void *cuda_stream)
+{
+    return host_submit(h, h_events, n, t0_us, window_us, out, cuda_stream, false, 0);
+}
+
+extern "C" int ddhf_host_submit_packed(ddhf_handle *h, const ddhf_event8 *h_events, int64_t n, int64_t t_base_us, int64_t t0_us,
+                                       int64_t window_us, const ddhf_host_outputs *out, void *cuda_stream)
+{
+    return host_submit(h, h_events, n, t0_us, window_us, out, cuda_stream, true, t_base_us);
 }
 
 extern "C" int ddhf_host_wait(ddhf_handle *h)

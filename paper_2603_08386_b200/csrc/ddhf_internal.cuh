@@ -94,7 +94,9 @@ struct NdftParams {
 };
 
 struct IngestParams {
-    const ddhf_event *events;
+    const ddhf_event *events;    // 16-byte events, or (packed) ddhf_event8 records through the same pointer
+    int32_t packed;
+    int64_t t_base;              // packed: t = t_base + dt_us
     int64_t n;
     int64_t t0, t1;              // window [t0, t1)
     int32_t width, height, np;

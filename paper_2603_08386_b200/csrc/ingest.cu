@@ -345,7 +345,7 @@ template <bool COMPACT> struct TileOut {
 
 // Decode one event: sort key = bucket << 13 | position in the tile (the sentinel bucket nb for dropped
 // events and for the padding of the last tile); payload = the item k_bucket_sort will read.
-template <bool FULL, bool COMPACT>
+template <bool FULL, bool COMPACT, bool PACKED>
 __device__ __forceinline__ uint32_t load_event(const IngestParams &p, int64_t idx, uint32_t e, uint32_t nb, uint32_t lmask,
                                                uint32_t window, typename BucketItem<COMPACT>::type &pay)
 {
@@ -353,13 +353,24 @@ __device__ __forceinline__ uint32_t load_event(const IngestParams &p, int64_t id
     uint32_t bucket = nb;
     pay = 0;
     if (FULL || idx < p.n) {
-        const int4 w = __ldg(reinterpret_cast<const int4 *>(p.events) + idx);
-        const uint32_t x = static_cast<uint32_t>(w.x) & 0xffffu, y = static_cast<uint32_t>(w.x) >> 16;
-        const uint64_t t = (static_cast<uint64_t>(static_cast<uint32_t>(w.w)) << 32) | static_cast<uint32_t>(w.z);
-        const uint64_t dt = t - static_cast<uint64_t>(p.t0);              // window < 2^31: in range iff dt < window
+        uint32_t x, y, pos;
+        uint64_t dt;                                                       // t - t0; window < 2^31: in range iff dt < window
+        if (PACKED) {
+            const uint2 w = __ldg(reinterpret_cast<const uint2 *>(p.events) + idx);
+            x = w.x & 0xffffu;
+            y = (w.x >> 16) & 0x7fffu;
+            pos = w.x >> 31;
+            dt = static_cast<uint64_t>(p.t_base - p.t0) + w.y;
+        } else {
+            const int4 w = __ldg(reinterpret_cast<const int4 *>(p.events) + idx);
+            x = static_cast<uint32_t>(w.x) & 0xffffu;
+            y = static_cast<uint32_t>(w.x) >> 16;
+            const uint64_t t = (static_cast<uint64_t>(static_cast<uint32_t>(w.w)) << 32) | static_cast<uint32_t>(w.z);
+            dt = t - static_cast<uint64_t>(p.t0);
+            pos = (static_cast<int32_t>(static_cast<uint32_t>(w.y) << 16) > 0) ? 1u : 0u;    // int16 p > 0
+        }
         const bool ok = (dt < window) && (x < static_cast<uint32_t>(p.width)) && (y < static_cast<uint32_t>(p.height));
         const uint32_t px = y * static_cast<uint32_t>(p.width) + x;
-        const uint32_t pos = (static_cast<int32_t>(static_cast<uint32_t>(w.y) << 16) > 0) ? 1u : 0u;    // int16 p > 0
         const uint32_t val = (static_cast<uint32_t>(dt) << 1) | pos;
         if (ok) bucket = px >> p.bl;
         if (COMPACT) pay = static_cast<TO>(((px & lmask) << p.vb) | val);
@@ -368,7 +379,7 @@ __device__ __forceinline__ uint32_t load_event(const IngestParams &p, int64_t id
     return (bucket << 13) | e;
 }
 
-template <bool COMPACT>
+template <bool COMPACT, bool PACKED>
 __global__ void __launch_bounds__(kNT, 2) k_tile_sort(IngestParams p)
 {
     typedef typename BucketItem<COMPACT>::type TO;
@@ -394,7 +405,7 @@ __global__ void __launch_bounds__(kNT, 2) k_tile_sort(IngestParams p)
         for (int i = 0; i < K; ++i) {
             const uint32_t e = static_cast<uint32_t>(t + kNT * i);
             TO py;
-            keys[pad_pos<uint32_t>(e)] = load_event<true, COMPACT>(p, tile_beg + e, e, nb, lmask, window, py);
+            keys[pad_pos<uint32_t>(e)] = load_event<true, COMPACT, PACKED>(p, tile_beg + e, e, nb, lmask, window, py);
             pay[e] = py;
         }
     } else {
@@ -402,7 +413,7 @@ __global__ void __launch_bounds__(kNT, 2) k_tile_sort(IngestParams p)
         for (int i = 0; i < K; ++i) {
             const uint32_t e = static_cast<uint32_t>(t + kNT * i);
             TO py;
-            keys[pad_pos<uint32_t>(e)] = load_event<false, COMPACT>(p, tile_beg + e, e, nb, lmask, window, py);
+            keys[pad_pos<uint32_t>(e)] = load_event<false, COMPACT, PACKED>(p, tile_beg + e, e, nb, lmask, window, py);
             pay[e] = py;
         }
     }
@@ -1101,8 +1112,11 @@ namespace {
 template <bool COMPACT>
 cudaError_t configure_sort_kernels()
 {
-    cudaError_t e = cudaFuncSetAttribute(k_tile_sort<COMPACT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaError_t e = cudaFuncSetAttribute(k_tile_sort<COMPACT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          static_cast<int>(ingest_tile_smem(COMPACT)));
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(k_tile_sort<COMPACT, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             static_cast<int>(ingest_tile_smem(COMPACT)));
     if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(k_bucket_sort<COMPACT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 static_cast<int>(BucketCfg<COMPACT>::smem_bytes(12)));
@@ -1142,10 +1156,18 @@ int launch_sort(const IngestParams &p, cudaStream_t st)
     const int ev_tiles = static_cast<int>((p.n + kTile - 1) / kTile);
     int launches = 0;
     if (p.compact) {
-        if (ev_tiles > 0) { k_tile_sort<true><<<ev_tiles, kNT, ingest_tile_smem(true), st>>>(p); ++launches; }
+        if (ev_tiles > 0) {
+            if (p.packed) k_tile_sort<true, true><<<ev_tiles, kNT, ingest_tile_smem(true), st>>>(p);
+            else k_tile_sort<true, false><<<ev_tiles, kNT, ingest_tile_smem(true), st>>>(p);
+            ++launches;
+        }
         k_bucket_sort<true><<<p.nb, kNT, BucketCfg<true>::smem_bytes(p.bl), st>>>(p); ++launches;
     } else {
-        if (ev_tiles > 0) { k_tile_sort<false><<<ev_tiles, kNT, ingest_tile_smem(false), st>>>(p); ++launches; }
+        if (ev_tiles > 0) {
+            if (p.packed) k_tile_sort<false, true><<<ev_tiles, kNT, ingest_tile_smem(false), st>>>(p);
+            else k_tile_sort<false, false><<<ev_tiles, kNT, ingest_tile_smem(false), st>>>(p);
+            ++launches;
+        }
         k_bucket_sort<false><<<p.nb, kNT, BucketCfg<false>::smem_bytes(p.bl), st>>>(p); ++launches;
     }
     return launches;

@@ -29,6 +29,21 @@ EVENT_DTYPE = np.dtype(
     [("x", "<u2"), ("y", "<u2"), ("p", "<i2"), ("pad", "<u2"), ("t", "<i8")], align=True
 )
 assert EVENT_DTYPE.itemsize == 16
+#: ddhf_event8 of include/ddhf.h: the same tuple in 8 bytes (timestamp as an offset from a base time)
+EVENT8_DTYPE = np.dtype([("x", "<u2"), ("y_p", "<u2"), ("dt", "<u4")])
+assert EVENT8_DTYPE.itemsize == 8
+
+
+def pack_events(ev: np.ndarray, t_base_us: int) -> np.ndarray:
+    """16-byte events -> 8-byte events (a change of container, nothing of the method): y and the polarity
+    bit share a word, t becomes t - t_base_us in 32 bits."""
+    dt = ev["t"].astype(np.int64) - int(t_base_us)
+    assert dt.min(initial=0) >= 0 and dt.max(initial=0) < (1 << 32) and ev["y"].max(initial=0) < 32768
+    out = np.zeros(len(ev), dtype=EVENT8_DTYPE)
+    out["x"] = ev["x"]
+    out["y_p"] = ev["y"].astype(np.uint16) | ((ev["p"] > 0).astype(np.uint16) << 15)
+    out["dt"] = dt.astype(np.uint32)
+    return out
 
 
 @dataclasses.dataclass

@@ -406,3 +406,28 @@ def test_stuck_pixel_million_events_on_config2(oracle):
     terms = prm["n_freq"] * float(cnt[cnt >= prm["n_min"]].sum())
     budget_ms = 2.0 * terms / 10.0e12 * 1e3
     assert gpu["stage_ms"][1] <= budget_ms, (gpu["stage_ms"], budget_ms)
+
+
+@pytest.mark.parametrize("t_base_off", [0, -7_000, 3_000])
+def test_packed_events_bit_identical(oracle, t_base_off):
+    """8-byte events (ddhf_event8: y | polarity << 15, dt from a base time): every output equals the
+    16-byte call bit for bit, and the CSR equals the oracle's; events before t_base cannot be expressed,
+    so the base is at or before the first event; bad coordinates and out-of-window times included."""
+    from paper_2603_08386_b200 import binding
+    ev = wl.random_window(41, 48, 40, 25_000, 30_000, hot_fraction=0.3, out_of_range=0.1, time_sorted=False)
+    ev["t"] += 10_000
+    t_base = int(ev["t"].min()) + min(t_base_off, 0)
+    t0 = 12_000 + max(t_base_off, 0)
+    prm = dict(SMALL, n_min=2)
+    ref = gu.run_gpu(prm, ev, t0, 20_000, score_all=True)
+    ev8 = wl.pack_events(ev, t_base)
+    det = binding.Detector(prm, max_events=len(ev), score_all=True, want_power=True)
+    d8 = det.torch.from_numpy(ev8.view(np.uint8).copy()).to(det.device)
+    det.window_packed(d8, len(ev8), t_base, t0, 20_000)
+    got = det.results()
+    det.close()
+    row_ptr, csr, dropped = oracle.bucket(ev, 48, 40, t0, 20_000)
+    assert np.array_equal(got["row_ptr"], row_ptr) and np.array_equal(got["csr_ev"], csr) and got["n_dropped"] == dropped
+    for k in ("row_ptr", "csr_ev", "active_idx", "power", "sf", "score", "f0_idx", "mask", "boxes"):
+        same = (np.array_equal(got[k], ref[k], equal_nan=True) if got[k].dtype.kind == "f" else np.array_equal(got[k], ref[k]))
+        assert same, k
