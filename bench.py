@@ -376,7 +376,7 @@ def main():
         hbufs.append(t)
         houts.append(o)
     cst = torch.cuda.current_stream(dev).cuda_stream
-    e2e_steps = min(steps, 10)
+    e2e_steps = steps
     e2e_wins = wins[warmup:warmup + e2e_steps]
 
     def run_pipelined(ws):
