@@ -45,9 +45,9 @@ struct ddhf_handle {
         ddhf_event *events = nullptr;
         void *ws = nullptr;
         ddhf_outputs out{};
-        cudaEvent_t copied = nullptr, done = nullptr;
+        cudaEvent_t copied = nullptr, kernels = nullptr, done = nullptr;
     } pipe[2];
-    cudaStream_t copy_stream = nullptr;
+    cudaStream_t copy_stream = nullptr, d2h_stream = nullptr;   // H2D of the next window / D2H of the finished one, both beside the kernels
     bool pipe_ready = false;
     long long pipe_head = 0, pipe_tail = 0;      // windows submitted / waited for
     // sliding-window state (ddhf_window_slide): the previous window's CSR lives in the workspace
@@ -600,9 +600,11 @@ static int host_submit(ddhf_handle *h, const void *h_events, int64_t n, int64_t 
         // all or nothing: a failure part-way leaves no buffer behind, so the next call starts clean
         cudaError_t e = cudaSuccess;
         if (!h->copy_stream) e = cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking);
+        if (e == cudaSuccess && !h->d2h_stream) e = cudaStreamCreateWithFlags(&h->d2h_stream, cudaStreamNonBlocking);
         for (auto &s : h->pipe) {
             if (e == cudaSuccess) e = alloc_set(h, s.events, s.ws, s.out);
             if (e == cudaSuccess && !s.copied) e = cudaEventCreateWithFlags(&s.copied, cudaEventDisableTiming);
+            if (e == cudaSuccess && !s.kernels) e = cudaEventCreateWithFlags(&s.kernels, cudaEventDisableTiming);
             if (e == cudaSuccess && !s.done) e = cudaEventCreateWithFlags(&s.done, cudaEventDisableTiming);
         }
         if (e != cudaSuccess) {
@@ -624,10 +626,13 @@ static int host_submit(ddhf_handle *h, const void *h_events, int64_t n, int64_t 
     }
     const int rc = run_window(h, s.events, n, t0_us, window_us, s.ws, &s.out, st, 0, 0, packed, t_base_us);
     const ddhf_outputs &d = s.out;
+    // the results leave on a stream of their own, so that the next window's kernels start at once
     auto d2h = [&](void *dst, const void *src, size_t bytes) {
-        if (e == cudaSuccess && dst) e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && dst) e = cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, h->d2h_stream);
     };
     if (rc == DDHF_OK) {
+        e = cudaEventRecord(s.kernels, st);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(h->d2h_stream, s.kernels, 0);
         d2h(out->counters, d.counters, sizeof(int32_t) * DDHF_N_COUNTERS);
         d2h(out->mask, d.mask, np);
         d2h(out->boxes, d.boxes, sizeof(ddhf_box) * static_cast<size_t>(c.max_boxes));
@@ -642,10 +647,12 @@ static int host_submit(ddhf_handle *h, const void *h_events, int64_t n, int64_t 
         // kernels or copies of this window may already be queued on the slot's buffers: drain them so
         // that the slot can be reused by the next submit, and report the failure (nothing is in flight)
         cudaStreamSynchronize(st);
+        cudaStreamSynchronize(h->d2h_stream);
         return rc != DDHF_OK ? rc : cuda_fail(e);
     }
-    if ((e = cudaEventRecord(s.done, st)) != cudaSuccess) {
+    if ((e = cudaEventRecord(s.done, h->d2h_stream)) != cudaSuccess) {
         cudaStreamSynchronize(st);
+        cudaStreamSynchronize(h->d2h_stream);
         return cuda_fail(e);
     }
     ++h->pipe_head;
@@ -690,9 +697,11 @@ extern "C" int ddhf_destroy(ddhf_handle *h)
     for (auto &s : h->pipe) {
         free_set(s.events, s.ws, s.out);
         if (s.copied) cudaEventDestroy(s.copied);
+        if (s.kernels) cudaEventDestroy(s.kernels);
         if (s.done) cudaEventDestroy(s.done);
     }
     if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
+    if (h->d2h_stream) cudaStreamDestroy(h->d2h_stream);
     delete h;
     return DDHF_OK;
 }
