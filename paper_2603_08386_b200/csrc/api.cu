@@ -23,6 +23,7 @@ struct ddhf_handle {
     int n_tiles = 0;
     int launches = 0;
     int bl = 5, nb = 1, hbits = 1;          // ingest digit split (ingest_plan)
+    int giant_row0 = 0, giant_rows = 0;     // chunk rows reserved for giant buckets
     int spill_cap = 0;
     bool fallback = true;                  // the NDFT kernel variant with in-place scoring (queue smaller than the sensor)
     ScoreParams sp{};
@@ -32,7 +33,7 @@ struct ddhf_handle {
     int ndft_blocks_per_sm = 1, full_blocks_per_sm = 1, score_blocks_per_sm = 1;
     // workspace offsets (bytes)
     size_t off_cnt = 0, off_items = 0, off_scratch = 0, off_work = 0, off_tiles = 0, off_class = 0, off_cursor = 0, off_runs = 0, off_bkt = 0, off_rows = 0, off_spill = 0, off_spillrec = 0,
-           off_parent = 0, off_rec = 0, off_ctiles = 0, off_merge = 0, off_slide = 0, off_segwork = 0, off_split = 0, off_splitcnt = 0, off_partial = 0, ws_bytes = 0;
+           off_parent = 0, off_rec = 0, off_ctiles = 0, off_merge = 0, off_giant = 0, off_slide = 0, off_segwork = 0, off_split = 0, off_splitcnt = 0, off_partial = 0, ws_bytes = 0;
     cudaEvent_t ev[5] = {nullptr, nullptr, nullptr, nullptr, nullptr};
     bool timed_once = false;
     // buffers of the host-buffer variant
@@ -278,8 +279,13 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
         ingest_plan(h->np, &h->bl, &h->nb, &h->hbits);
         const size_t ev_tiles = (static_cast<size_t>(c.max_events) + ingest_tile_events() - 1) / ingest_tile_events();
         h->off_runs = o;    o = align_up(o + sizeof(uint32_t) * ev_tiles * static_cast<size_t>(h->nb));
-        h->off_bkt = o;     o = align_up(o + sizeof(int32_t) * 4 * (static_cast<size_t>(h->nb) + 2));
-        h->off_rows = o;    o = align_up(o + sizeof(int32_t) * (2 * ev_tiles + h->nb + 2) * (4 + (static_cast<size_t>(1) << h->bl)));
+        h->off_bkt = o;     o = align_up(o + sizeof(int32_t) * 6 * (static_cast<size_t>(h->nb) + 2));
+        h->off_giant = o;   o = align_up(o + 32 * (static_cast<size_t>(h->nb) + 2));
+        // chunk rows: header + counts + bases per pixel of a bucket; the one-CTA path needs at most 2 n / capacity + nb
+        // rows, the giant buckets get 4 rows per tile more (a bucket that finds no room there stays on the one-CTA path)
+        h->giant_row0 = static_cast<int>(2 * ev_tiles + h->nb + 2);
+        h->giant_rows = static_cast<int>(4 * ev_tiles + 64);
+        h->off_rows = o;    o = align_up(o + sizeof(int32_t) * (static_cast<size_t>(h->giant_row0) + h->giant_rows) * (4 + (static_cast<size_t>(2) << h->bl)));
     }
     // deferred-scoring queue (row count decided above)
     h->off_spill = o;      o = align_up(o + sizeof(float) * static_cast<size_t>(h->spill_cap) * ndft_padded_bins(c.n_freq));
@@ -350,6 +356,10 @@ static int run_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n, int
     ip.bkt_base = ip.bkt_total + h->nb + 2;
     ip.bkt_order = ip.bkt_base + h->nb + 2;
     ip.bkt_act = ip.bkt_order + h->nb + 2;
+    ip.bkt_maxrun = ip.bkt_act + h->nb + 2;
+    ip.giant_of = ip.bkt_maxrun + h->nb + 2;
+    ip.giant_tab = ws + h->off_giant;
+    ip.giant_row0 = h->giant_row0; ip.giant_rows = h->giant_rows;
     ip.chunk_rows = reinterpret_cast<int32_t *>(ws + h->off_rows);
     ip.sync = reinterpret_cast<int32_t *>(ws + h->off_cursor + 16);       // [16]; the scoring queue counts are sync[2..3]
 

@@ -113,11 +113,16 @@ struct IngestParams {
     uint32_t *run_tab;           // [ev_tiles][nb] run of every bucket inside its tile: first item | length << 16
     int32_t *bkt_order;          // [nb] buckets by descending size class
     int32_t *bkt_act;            // [nb] active pixels (count >= n_min) of every bucket
+    int32_t *bkt_maxrun;         // [nb + 2] longest run of the bucket in one tile
+    int32_t *giant_of;           // [nb + 2] index into giant_tab, -1: the bucket is sorted by its own CTA
+    void *giant_tab;             // [nb] GiantBucket (ingest.cu)
+    int32_t giant_row0, giant_rows;   // chunk rows reserved for giant buckets: first row, count
     int32_t *bkt_total, *bkt_base;   // [nb + 2] events per bucket; exclusive scan (bkt_base[nb] = n_in)
     int32_t *chunk_rows;         // [max_rows][4 + 2^bl] chunk table of the multi-chunk buckets
     int32_t *sync;               // [16] 0: tiles finished, 1: chunk rows handed out, 2-3: scoring queue counts,
                                  //     4: work items, 5: split rows, 6: partials, 7: arrival counters handed out, 8: box-merge CTAs finished,
-                                 //     9: items of the segment list
+                                 //     9: items of the segment list, 10: giant buckets, 11: their chunks, 12-13: chunk tickets of
+                                 //     k_bucket_sort / k_worklist, 14: giant chunk rows handed out
     SplitRow *split_tab;         // rows longer than kSplitMin (see NdftParams)
     int32_t *split_cnt;
     WorkItem *seg_work;          // when set: the segments of split rows go to this list (count in sync[9]) instead of `work`

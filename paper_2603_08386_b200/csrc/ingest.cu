@@ -42,6 +42,17 @@ constexpr int kCntStride = kNT + kNT / 32 + 16; // words per counter row: one pa
 constexpr int kCntWords = 16 * kCntStride;     // 32 digits, two 16-bit counters per word
 constexpr unsigned kFullMask = 0xffffffffu;
 
+// a bucket with more events than kGiantMin is sorted by several CTAs (see "giant buckets" below)
+struct __align__(16) GiantBucket {
+    int32_t bucket, tiles_per_chunk, n_chunks, row0;      // row0: first of n_chunks consecutive chunk rows
+    int32_t chunk0;                                       // first of the bucket's chunks in the flat numbering
+    int32_t done;                                         // chunks sorted so far
+    int32_t _pad[2];
+};
+constexpr int kGiantMin = 4 * 16384;
+constexpr int kGiantHelpers = 74;      // extra CTAs of k_bucket_sort (and half as many of k_worklist) for their chunks
+
+
 struct Ev {
     int32_t pix;       // -1 if dropped
     uint32_t val;      // (t - t0) << 1 | (p > 0)
@@ -96,7 +107,10 @@ __global__ void k_init(IngestParams p)
         p.mask[i] = 0;
         p.ccl_parent[i] = 0x7fffffff;           // no parent yet
     }
-    if (i <= p.nb + 1) { p.bkt_total[i] = 0; p.bkt_base[i] = 0; p.bkt_order[i] = i; }   // identity order: no tile ran
+    if (i <= p.nb + 1) {
+        p.bkt_total[i] = 0; p.bkt_base[i] = 0; p.bkt_order[i] = i;      // identity order: no tile ran
+        p.bkt_maxrun[i] = 64; p.giant_of[i] = -1;
+    }
     if (blockIdx.x == 0) {
         if (threadIdx.x < DDHF_N_COUNTERS) p.counters[threadIdx.x] = 0;
         if (threadIdx.x < kNumClasses) {
@@ -313,6 +327,32 @@ __device__ __forceinline__ void finish_buckets(const IngestParams &p, uint32_t *
         p.counters[DDHF_CNT_N_IN] = grand;
         p.counters[DDHF_CNT_N_DROPPED] = static_cast<int32_t>(p.n - grand);
     }
+    // giant buckets: cut into chunks of whole tiles that fit one chunk each (not on the sliding-window path,
+    // whose slab is small; a bucket that finds no room in the giant rows stays on the one-CTA path)
+    if (!p.prev_csr) {
+        GiantBucket *tab = reinterpret_cast<GiantBucket *>(p.giant_tab);
+        const int n_tiles = static_cast<int>((p.n + kTile - 1) / kTile);
+        const int cap = p.compact ? 16384 : 8192;
+#pragma unroll
+        for (int q = 0; q < 2; ++q) {
+            const uint32_t b = b0 + q;
+            const int m = q ? v1 : v0;
+            if (b < nb && m > kGiantMin) {
+                const int tr = max(1, cap / max(__ldcg(p.bkt_maxrun + b), 1));
+                const int n_chunks = (n_tiles + tr - 1) / tr;
+                const int row0 = atomicAdd(p.sync + 14, n_chunks);
+                if (row0 + n_chunks <= p.giant_rows) {
+                    const int g = atomicAdd(p.sync + 10, 1);
+                    GiantBucket gb;
+                    gb.bucket = static_cast<int32_t>(b); gb.tiles_per_chunk = tr; gb.n_chunks = n_chunks;
+                    gb.row0 = p.giant_row0 + row0; gb.chunk0 = atomicAdd(p.sync + 11, n_chunks); gb.done = 0;
+                    gb._pad[0] = 0; gb._pad[1] = 0;
+                    tab[g] = gb;
+                    p.giant_of[b] = g;
+                }
+            }
+        }
+    }
     int mx = __reduce_max_sync(kFullMask, max(v0, v1));
     __syncthreads();
     if (lane == 0) s_warp[t >> 5] = static_cast<uint32_t>(mx);
@@ -326,7 +366,11 @@ __device__ __forceinline__ void finish_buckets(const IngestParams &p, uint32_t *
     __syncthreads();
     sort_subpass<2, uint32_t, 5>(it, cnt, buf32, s_warp, 16, 5);
     __syncthreads();
-    for (uint32_t r = t; r < nb; r += kNT) p.bkt_order[r] = static_cast<int32_t>(buf32[pad_pos<uint32_t>(static_cast<int>(r))] & 0xffffu);
+    // (the list entries of giant buckets are marked: their CTAs of k_bucket_sort leave at once)
+    for (uint32_t r = t; r < nb; r += kNT) {
+        const uint32_t b = buf32[pad_pos<uint32_t>(static_cast<int>(r))] & 0xffffu;
+        p.bkt_order[r] = static_cast<int32_t>(b | (__ldcg(p.giant_of + b) >= 0 ? 0x80000000u : 0u));
+    }
 }
 
 // ---- k_tile_sort: decode + filter one tile, sort it by bucket, publish its runs -----------------
@@ -457,7 +501,10 @@ __global__ void __launch_bounds__(kNT, 2) k_tile_sort(IngestParams p)
             if (b < nb) {
                 row[b] = a | (len[q] << 16);
                 delta[b] = a - rstart[b];
-                if (len[q]) atomicAdd(&p.bkt_total[b], static_cast<int>(len[q]));
+                if (len[q]) {
+                    atomicAdd(&p.bkt_total[b], static_cast<int>(len[q]));
+                    if (len[q] > 64) atomicMax(&p.bkt_maxrun[b], static_cast<int>(len[q]));      // only giant buckets need it
+                }
                 a += alen[q];
             }
         }
@@ -566,12 +613,16 @@ __device__ __forceinline__ void sort_chunk_any(typename BucketItem<COMPACT>::typ
 constexpr int kRowHdr = 4;
 constexpr int kLongRun = 256;      // runs longer than this are gathered by the whole CTA
 
+// Bucket b, tiles [tile_lo, tile_hi).  giant_row < 0: the whole bucket (every tile), as described above.
+// giant_row >= 0: one chunk of a giant bucket (a tile range that fits one chunk by construction; giant_off = the
+// bucket's events in earlier tiles): sort it, leave the sorted chunk in the workspace and its per-pixel counts in
+// chunk row giant_row; giant_finish() and the placement CTAs of k_worklist do the rest.
 template <bool COMPACT>
-__global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
+__device__ __forceinline__ void bucket_body(const IngestParams &p, uint32_t *s_raw, int b, int tile_lo, int tile_hi,
+                                            int giant_row, int giant_off)
 {
     typedef BucketCfg<COMPACT> C;
     typedef typename C::T T;
-    extern __shared__ __align__(16) uint32_t s_raw[];
     __shared__ uint32_t s_warp[kNT / 32];
     __shared__ int s_cut, s_row;
     T *buf = reinterpret_cast<T *>(s_raw);
@@ -580,12 +631,13 @@ __global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
     const int bl = p.bl, vb = p.vb, nl = 1 << bl;
     uint32_t *pixtot = rstart + nl + 4;                        // [nl]
     const int t = threadIdx.x;
-    const int b = p.bkt_order[blockIdx.x];                     // largest buckets first
+    const bool giant = giant_row >= 0;
     const int m = p.bkt_total[b];
     const int gbase = p.bkt_base[b];
     const int pix0 = b << bl;
     __shared__ int s_act, s_class[kNumClasses];           // active pixels / work items per class of this bucket
-    if (t == 0) { s_act = 0; p.bkt_act[b] = 0; }
+    __syncthreads();                                      // (a helper CTA comes back here chunk after chunk)
+    if (t == 0) { s_act = 0; if (!giant) p.bkt_act[b] = 0; }
     if (t < kNumClasses) s_class[t] = 0;
     if (m == 0) {
         for (int l = t; l < nl; l += kNT)
@@ -611,16 +663,15 @@ __global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
         if (t == 0) p.bkt_act[b] = s_act;
         if (t < kNumClasses && s_class[t]) atomicAdd(&p.class_cnt[t], s_class[t]);
     };
-    const bool single = m <= C::kCap;
+    const bool single = !giant && m <= C::kCap;
     if (!single)
         for (int l = t; l < nl; l += kNT) pixtot[l] = 0u;
-    const int n_tiles = static_cast<int>((p.n + kTile - 1) / kTile);
     const uint4 *items = reinterpret_cast<const uint4 *>(p.items);         // runs start on 16-byte boundaries
     constexpr int kPer16 = TileOut<COMPACT>::kAlign;                        // items per 128-bit load
     T *scratch = reinterpret_cast<T *>(p.scratch);
-    const int row_words = kRowHdr + nl;
+    const int row_words = kRowHdr + 2 * nl;
     int fill = 0;            // items gathered for the chunk being formed
-    int chunk_off = 0;       // offset of that chunk inside the bucket
+    int chunk_off = giant ? giant_off : 0;       // offset of that chunk inside the bucket
     int last_row = -1;
 
     // Emit the chunk in buf[0, fill): the only chunk of the bucket -> csr_ev and counts; else loop 1.
@@ -635,6 +686,11 @@ __global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
                     tally(static_cast<int>(rstart[l + 1] - rstart[l]));
                 }
             for (int r = t; r < fill; r += kNT) p.csr_ev[gbase + r] = C::val_of(buf[pad_pos<T>(r)], vb);
+        } else if (giant) {
+            int32_t *rw = p.chunk_rows + static_cast<size_t>(giant_row) * row_words;
+            if (t == 0) { rw[0] = -1; rw[1] = chunk_off; rw[2] = fill; rw[3] = 0; }
+            for (int l = t; l < nl; l += kNT) rw[kRowHdr + l] = static_cast<int32_t>(rstart[l + 1] - rstart[l]);
+            for (int r = t; r < fill; r += kNT) scratch[static_cast<size_t>(gbase) + chunk_off + r] = buf[pad_pos<T>(r)];
         } else {
             if (t == 0) s_row = atomicAdd(p.sync + 1, 1);
             __syncthreads();
@@ -655,13 +711,13 @@ __global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
     };
 
     // runs of this bucket, 2 kNT tiles at a time, in tile order = input order
-    for (int tb = 0; tb < n_tiles; tb += 2 * kNT) {
+    for (int tb = tile_lo; tb < tile_hi; tb += 2 * kNT) {
         int src[2], len[2];
 #pragma unroll
         for (int q = 0; q < 2; ++q) {
             const int j = tb + 2 * t + q;
             src[q] = 0; len[q] = 0;
-            if (j < n_tiles) {
+            if (j < tile_hi) {
                 const uint32_t e = __ldg(p.run_tab + static_cast<size_t>(j) * p.nb + b);
                 src[q] = static_cast<int>(e & 0xffffu); len[q] = static_cast<int>(e >> 16);
             }
@@ -745,6 +801,7 @@ __global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
     }
     flush();
     if (single) { publish_tally(); return; }
+    if (giant) return;
 
     // loop 2: row starts of the bucket's pixels, then every chunk goes to its place
     {
@@ -791,6 +848,130 @@ __global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
     publish_tally();
 }
 
+// ---- giant buckets ------------------------------------------------------------------------------------------
+// A bucket of more than kGiantMin events (a stuck pixel puts all of its events into one bucket) would keep one CTA
+// busy chunk after chunk.  The last CTA of k_tile_sort lists such buckets (giant_tab) and cuts each into chunks of
+// TR consecutive tiles, TR = capacity / (the bucket's longest run in a tile), so that every chunk fits; helper CTAs of
+// k_bucket_sort sort the chunks (bucket_body in giant mode), the helper that finishes a bucket's last chunk turns the
+// per-chunk counts into row starts and per-chunk bases (giant_finish), and helper CTAs of k_worklist move the sorted
+// chunks to their places.  Everything is a function of the data alone: same bits as the one-CTA path.
+// chunk row of a giant bucket: header {-, offset in the bucket, items, -}, counts [nl], then bases [nl] (giant_finish)
+template <bool COMPACT>
+__device__ __forceinline__ void giant_finish(const IngestParams &p, uint32_t *s_raw, const GiantBucket &gb)
+{
+    typedef BucketCfg<COMPACT> C;
+    __shared__ uint32_t s_w[kNT / 32];
+    __shared__ int s_act2, s_class2[kNumClasses];
+    uint32_t *rowstart = s_raw;                            // [nl] (the sort buffers are idle)
+    const int t = threadIdx.x, nl = 1 << p.bl, b = gb.bucket, pix0 = b << p.bl, gbase = p.bkt_base[b];
+    const int row_words = kRowHdr + 2 * nl;
+    const int per = (nl + kNT - 1) / kNT;                  // <= 8
+    if (t == 0) s_act2 = 0;
+    if (t < kNumClasses) s_class2[t] = 0;
+    __syncthreads();
+    // per pixel: events in earlier chunks (prefix over the chunk rows), total
+    uint32_t v[8];
+    uint32_t sum = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const int l = t * per + k;
+        v[k] = 0;
+        if (k < per && l < nl) {
+            uint32_t run = 0;
+            for (int c = 0; c < gb.n_chunks; ++c) {
+                int32_t *rw = p.chunk_rows + static_cast<size_t>(gb.row0 + c) * row_words;
+                const uint32_t n = static_cast<uint32_t>(__ldcg(rw + kRowHdr + l));
+                rw[kRowHdr + nl + l] = static_cast<int32_t>(run);
+                run += n;
+            }
+            v[k] = run;
+        }
+        sum += v[k];
+    }
+    int tot;
+    uint32_t ex = static_cast<uint32_t>(block_excl_sum(static_cast<int>(sum), tot, s_w));
+    const int nmin = p.prev_csr ? 0x7fffffff : max(p.n_min, 1);
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const int l = t * per + k;
+        if (k < per && l < nl) {
+            rowstart[l] = ex;
+            if (pix0 + l < p.np) {
+                p.cnt[pix0 + l] = static_cast<int32_t>(v[k]);
+                if (p.slab_row_ptr) p.slab_row_ptr[pix0 + l] = gbase + static_cast<int32_t>(ex);
+                if (static_cast<int>(v[k]) >= nmin) {
+                    int seg_len;
+                    const int n_seg = row_segments(static_cast<int>(v[k]), seg_len);
+                    atomicAdd(&s_act2, 1);
+                    if (class_items(p, n_seg)) atomicAdd(&s_class2[size_class(seg_len)], class_items(p, n_seg));
+                }
+            }
+            ex += v[k];
+        }
+    }
+    __syncthreads();
+    // bases: row start of the pixel + its events in earlier chunks
+    for (int c = 0; c < gb.n_chunks; ++c) {
+        int32_t *rw = p.chunk_rows + static_cast<size_t>(gb.row0 + c) * row_words;
+        for (int l = t; l < nl; l += kNT) rw[kRowHdr + nl + l] += static_cast<int32_t>(rowstart[l]);
+    }
+    if (t == 0) p.bkt_act[b] = s_act2;
+    if (t < kNumClasses && s_class2[t]) atomicAdd(&p.class_cnt[t], s_class2[t]);
+    __syncthreads();
+}
+
+template <bool COMPACT>
+__global__ void __launch_bounds__(kNT, 2) k_bucket_sort(IngestParams p)
+{
+    extern __shared__ __align__(16) uint32_t s_raw[];
+    __shared__ int s_ticket, s_g;
+    __shared__ bool s_lastc;
+    const int t = threadIdx.x;
+    const int n_tiles = static_cast<int>((p.n + kTile - 1) / kTile);
+    if (static_cast<int>(blockIdx.x) < p.nb) {
+        const int b = p.bkt_order[blockIdx.x];                 // largest buckets first
+        if (b < 0) return;                                     // a giant bucket: its chunks go to the helper CTAs
+        bucket_body<COMPACT>(p, s_raw, b, 0, n_tiles, -1, 0);
+        return;
+    }
+    // helper CTAs: chunks of giant buckets
+    GiantBucket *tab = reinterpret_cast<GiantBucket *>(p.giant_tab);
+    const int n_giant = p.sync[10], n_chunks_all = p.sync[11];
+    while (true) {
+        __syncthreads();
+        if (t == 0) {
+            const int ch = atomicAdd(p.sync + 12, 1);
+            s_ticket = ch;
+            int g = 0;
+            if (ch < n_chunks_all)
+                while (g + 1 < n_giant && !(ch >= tab[g].chunk0 && ch < tab[g].chunk0 + tab[g].n_chunks)) ++g;
+            s_g = g;
+        }
+        __syncthreads();
+        const int ch = s_ticket;
+        if (ch >= n_chunks_all) return;
+        GiantBucket &gb = tab[s_g];
+        const int c = ch - gb.chunk0, b = gb.bucket;
+        const int tile_lo = c * gb.tiles_per_chunk, tile_hi = min(n_tiles, tile_lo + gb.tiles_per_chunk);
+        // the bucket's events in earlier tiles
+        int off = 0;
+        for (int j = t; j < tile_lo; j += kNT) off += static_cast<int>(__ldg(p.run_tab + static_cast<size_t>(j) * p.nb + b) >> 16);
+        __shared__ uint32_t s_w2[kNT / 32];
+        int total_before;
+        block_excl_sum(off, total_before, s_w2);
+        bucket_body<COMPACT>(p, s_raw, b, tile_lo, tile_hi, gb.row0 + c, total_before);
+        __threadfence();
+        __syncthreads();
+        if (t == 0) s_lastc = (atomicAdd(&gb.done, 1) == gb.n_chunks - 1);
+        __syncthreads();
+        if (s_lastc) {
+            __threadfence();
+            giant_finish<COMPACT>(p, s_raw, gb);
+        }
+    }
+}
+
+
 // ---- block-wide exclusive scan of two ints (1024 threads) -----------------------------
 __device__ __forceinline__ void block_scan2(int &a, int &b, int &tot_a, int &tot_b, int *s_a, int *s_b)
 {
@@ -824,6 +1005,40 @@ __device__ __forceinline__ void block_scan2(int &a, int &b, int &tot_a, int &tot
     b = ib - b + s_b[wid];
     tot_a = s_a[32];
     tot_b = s_b[32];
+    __syncthreads();
+}
+
+// placement of one sorted chunk of a giant bucket (helper CTAs of k_worklist, 1024 threads)
+template <bool COMPACT>
+__device__ __forceinline__ void giant_place(const IngestParams &p, const GiantBucket &gb, int c, int *s_delta, int *s_a, int *s_b)
+{
+    typedef BucketCfg<COMPACT> C;
+    typedef typename C::T T;
+    const int t = threadIdx.x, nl = 1 << p.bl, gbase = p.bkt_base[gb.bucket];
+    const int row_words = kRowHdr + 2 * nl;
+    const int32_t *rw = p.chunk_rows + static_cast<size_t>(gb.row0 + c) * row_words;
+    const int coff = rw[1], cfill = rw[2];
+    // run start of every pixel inside the sorted chunk = exclusive scan of the chunk's counts (nl <= 4096: 4 per thread)
+    int v[4], sum = 0, dummy = 0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int l = t * 4 + k;
+        v[k] = (l < nl) ? rw[kRowHdr + l] : 0;
+        sum += v[k];
+    }
+    int ta, tb;
+    block_scan2(sum, dummy, ta, tb, s_a, s_b);              // sum -> exclusive prefix
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int l = t * 4 + k;
+        if (l < nl) { s_delta[l] = rw[kRowHdr + nl + l] - sum; sum += v[k]; }
+    }
+    __syncthreads();
+    const T *scratch = reinterpret_cast<const T *>(p.scratch);
+    for (int r = t; r < cfill; r += 1024) {
+        const T item = scratch[static_cast<size_t>(gbase) + coff + r];
+        p.csr_ev[gbase + s_delta[C::low_of(item, p.vb)] + r] = C::val_of(item, p.vb);
+    }
     __syncthreads();
 }
 
@@ -994,6 +1209,30 @@ __global__ void __launch_bounds__(1024) k_worklist(IngestParams p)
     __shared__ int s_a[33], s_b[33];
     __shared__ int s_cls[kNumClasses], s_base[kNumClasses], s_tot[kNumClasses];
     const int t = threadIdx.x;
+    const int n_list_ctas = (p.np + kScanTile - 1) / kScanTile;
+    if (static_cast<int>(blockIdx.x) >= n_list_ctas) {
+        // helper CTAs: the sorted chunks of giant buckets go to their places in csr_ev
+        __shared__ int s_delta[4096], s_ticket, s_g;
+        const GiantBucket *tab = reinterpret_cast<const GiantBucket *>(p.giant_tab);
+        const int n_giant = p.sync[10], n_chunks_all = p.sync[11];
+        while (true) {
+            __syncthreads();
+            if (t == 0) {
+                const int ch = atomicAdd(p.sync + 13, 1);
+                s_ticket = ch;
+                int g = 0;
+                if (ch < n_chunks_all)
+                    while (g + 1 < n_giant && !(ch >= tab[g].chunk0 && ch < tab[g].chunk0 + tab[g].n_chunks)) ++g;
+                s_g = g;
+            }
+            __syncthreads();
+            const int ch = s_ticket;
+            if (ch >= n_chunks_all) return;
+            const GiantBucket &gb = tab[s_g];
+            if (p.compact) giant_place<true>(p, gb, ch - gb.chunk0, s_delta, s_a, s_b);
+            else giant_place<false>(p, gb, ch - gb.chunk0, s_delta, s_a, s_b);
+        }
+    }
     if (t < kNumClasses) { s_cls[t] = 0; s_tot[t] = p.class_cnt[t]; }
     // a tile of kScanTile pixels holds whole buckets (2^bL divides it): active pixels in the buckets before it
     const int nl = 1 << p.bl;
@@ -1161,14 +1400,14 @@ int launch_sort(const IngestParams &p, cudaStream_t st)
             else k_tile_sort<true, false><<<ev_tiles, kNT, ingest_tile_smem(true), st>>>(p);
             ++launches;
         }
-        k_bucket_sort<true><<<p.nb, kNT, BucketCfg<true>::smem_bytes(p.bl), st>>>(p); ++launches;
+        k_bucket_sort<true><<<p.nb + kGiantHelpers, kNT, BucketCfg<true>::smem_bytes(p.bl), st>>>(p); ++launches;
     } else {
         if (ev_tiles > 0) {
             if (p.packed) k_tile_sort<false, true><<<ev_tiles, kNT, ingest_tile_smem(false), st>>>(p);
             else k_tile_sort<false, false><<<ev_tiles, kNT, ingest_tile_smem(false), st>>>(p);
             ++launches;
         }
-        k_bucket_sort<false><<<p.nb, kNT, BucketCfg<false>::smem_bytes(p.bl), st>>>(p); ++launches;
+        k_bucket_sort<false><<<p.nb + kGiantHelpers, kNT, BucketCfg<false>::smem_bytes(p.bl), st>>>(p); ++launches;
     }
     return launches;
 }
@@ -1191,7 +1430,7 @@ int launch_ingest(const IngestParams &p, cudaStream_t st)
     IngestParams q = p;                      // k_bucket_sort writes row_ptr itself
     q.slab_row_ptr = p.row_ptr;
     launches += launch_sort(q, st);
-    k_worklist<<<(p.np + kScanTile - 1) / kScanTile, 1024, 0, st>>>(p); ++launches;
+    k_worklist<<<(p.np + kScanTile - 1) / kScanTile + kGiantHelpers / 2, 1024, 0, st>>>(p); ++launches;
     if (p.next_csr) { k_slide_save<<<592, 256, 0, st>>>(p); ++launches; }      // first window of a sliding sequence
     return launches;
 }
