@@ -63,7 +63,9 @@ extern "C" {
 #define DDHF_CNT_N_SCORED      6  /* active pixels on which the comb score was evaluated   */
 #define DDHF_CNT_N_COMPONENTS  7  /* connected components before the A_min filter          */
 #define DDHF_CNT_N_MERGED      8  /* detections written to merged_boxes (eq. 12)           */
-#define DDHF_N_COUNTERS        16 /* 9..15 reserved, written as 0                          */
+#define DDHF_CNT_N_GIANT       9  /* buckets of the ingest sort that were cut into chunks for
+                                     several CTAs (> 65536 events in 2^bL pixels)          */
+#define DDHF_N_COUNTERS        16 /* 10..15 reserved, written as 0                         */
 
 /* Event tuple (x, y, p, t) of a temporal-contrast sensor (L55).  16 bytes. */
 typedef struct {

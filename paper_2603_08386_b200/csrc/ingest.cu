@@ -366,6 +366,7 @@ __device__ __forceinline__ void finish_buckets(const IngestParams &p, uint32_t *
     __syncthreads();
     sort_subpass<2, uint32_t, 5>(it, cnt, buf32, s_warp, 16, 5);
     __syncthreads();
+    if (t == 0) p.counters[DDHF_CNT_N_GIANT] = *reinterpret_cast<volatile int32_t *>(p.sync + 10);
     // (the list entries of giant buckets are marked: their CTAs of k_bucket_sort leave at once)
     for (uint32_t r = t; r < nb; r += kNT) {
         const uint32_t b = buf32[pad_pos<uint32_t>(static_cast<int>(r))] & 0xffffu;

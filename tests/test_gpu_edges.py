@@ -380,6 +380,7 @@ def test_stuck_pixel_million_events_on_config2(oracle):
     base = gu.run_gpu(prm, w.events, w.t0_us, w.window_us)
     gpu = gu.run_gpu(prm, ev, w.t0_us, w.window_us, timing=True)
     pix = 17 * w.width + 301
+    assert gpu["counters"][9] >= 1                                         # the pixel's bucket went the giant way
     # the stuck pixel against the oracle's direct sum on its row (one pixel: seconds on one core)
     row_ptr, csr, _ = oracle.bucket(ev, w.width, w.height, w.t0_us, w.window_us)
     assert np.array_equal(gpu["row_ptr"], row_ptr) and np.array_equal(gpu["csr_ev"], csr)
@@ -431,3 +432,29 @@ def test_packed_events_bit_identical(oracle, t_base_off):
     for k in ("row_ptr", "csr_ev", "active_idx", "power", "sf", "score", "f0_idx", "mask", "boxes"):
         same = (np.array_equal(got[k], ref[k], equal_nan=True) if got[k].dtype.kind == "f" else np.array_equal(got[k], ref[k]))
         assert same, k
+
+
+@pytest.mark.parametrize("window_us", [50_000, (1 << 31) - 1])
+def test_giant_buckets_sorted_by_helper_ctas(oracle, window_us):
+    """Buckets of more than 65 536 events are cut into chunks of whole tiles and sorted by helper CTAs
+    (ingest.cu, "giant buckets"): two stuck pixels in different buckets, one bucket with two hot pixels and a
+    background, input not time-sorted, with 4-byte and (window 2^31 - 1 us) 8-byte items.  CSR bit-exact."""
+    W, H = 346, 260
+    rng = np.random.default_rng(window_us % 1000)
+    parts = [wl.random_window(5, W, H, 150_000, 50_000, hot_fraction=0.1)]
+    for (x, y, n) in ((10, 3, 300_000), (200, 200, 120_000), (40, 100, 90_000), (41, 100, 70_000)):
+        e = np.zeros(n, dtype=wl.EVENT_DTYPE)
+        e["x"], e["y"] = x, y
+        e["t"] = rng.integers(0, 50_000, size=n)
+        e["p"] = rng.integers(0, 2, size=n) * 2 - 1
+        parts.append(e)
+    ev = np.concatenate(parts)
+    ev = ev[rng.permutation(len(ev))]
+    prm = dict(wl.preset(2), n_min=6)
+    gpu = gu.run_gpu(prm, ev, 0, window_us, want_power=False)
+    row_ptr, csr, dropped = oracle.bucket(ev, W, H, 0, window_us)
+    assert gpu["counters"][9] >= 3, gpu["counters"]                     # DDHF_CNT_N_GIANT
+    assert gpu["n_dropped"] == dropped and gpu["n_in"] == len(csr)
+    assert np.array_equal(gpu["row_ptr"], row_ptr) and np.array_equal(gpu["csr_ev"], csr)
+    cnt = np.diff(row_ptr)
+    assert gpu["n_active"] == int((cnt >= 6).sum())
