@@ -254,6 +254,8 @@ __global__ void __launch_bounds__(warps_of(TM * 2 * TN) * 32, DDHF_NDFT_BLOCKS) 
             // software pipelined by hand, two events per trip: the centre phasors of the next
             // event (shared-memory read, integer phase, two SFU ops per centre) are produced under
             // the FFMA2 block of the current one, in alternating register sets (no copies)
+            static_assert(TM <= 2, "centre stride is applied as one shift");
+            constexpr int kLog4TN = (TN == 16) ? 6 : (TN == 8) ? 5 : (TN == 4) ? 4 : 3;
             float a0r[TM], a0i[TM], a1r[TM], a1i[TM];
             const uint32_t lane_u = static_cast<uint32_t>(lane);
 #define DDHF_CENTRES(AR, AI, K)                                                                  \
@@ -261,7 +263,7 @@ __global__ void __launch_bounds__(warps_of(TM * 2 * TN) * 32, DDHF_NDFT_BLOCKS) 
                 const uint4 ph = phs[K];                                                         \
                 const uint32_t pc0 = ph.x + lane_u * ph.y;                                       \
                 _Pragma("unroll") for (int g = 0; g < TM; ++g)                                   \
-                    sincos_u32(pc0 + static_cast<uint32_t>(g * 4 * TN) * ph.z, AI[g], AR[g]);    \
+                    sincos_u32(pc0 + (g ? (ph.z << kLog4TN) : 0u), AI[g], AR[g]);               \
             }
 #define DDHF_FMA_BLOCK(AR, AI, K)                                                                \
             {                                                                                    \
