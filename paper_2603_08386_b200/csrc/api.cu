@@ -292,7 +292,7 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
     h->off_spillrec = o;   o = align_up(o + sizeof(SpillRec) * static_cast<size_t>(h->spill_cap));
     h->off_parent = o;     o = align_up(o + sizeof(int32_t) * h->np);
     h->off_rec = o;        o = align_up(o + sizeof(int32_t) * 5 * static_cast<size_t>(h->np));
-    h->off_ctiles = o;     o = align_up(o + sizeof(int32_t) * 1024);
+    h->off_ctiles = o;     o = align_up(o + sizeof(int32_t) * 1032);
     // sliding windows: two copies of (row_ptr, csr_ev) used alternately, the new slab's own CSR
     h->off_slide = o;      o = align_up(o + 2 * (sizeof(int32_t) * (static_cast<size_t>(h->np) + 2) + sizeof(uint32_t) * static_cast<size_t>(c.max_events))
                                          + sizeof(int32_t) * static_cast<size_t>(h->np) + sizeof(uint32_t) * static_cast<size_t>(c.max_events) + 1024);
@@ -407,7 +407,8 @@ static int run_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n, int
     cp.a_min = c.a_min; cp.max_boxes = c.max_boxes;
     cp.parent = cp_parent;
     cp.rec = reinterpret_cast<int32_t *>(ws + h->off_rec);
-    cp.tile_sum = reinterpret_cast<int32_t *>(ws + h->off_ctiles);
+    cp.tile_state = reinterpret_cast<int32_t *>(ws + h->off_ctiles);
+    ip.ccl_tile_state = cp.tile_state;
     cp.boxes = out->boxes; cp.counters = out->counters;
     cp.merged = (c.merge_alpha > 0.f) ? out->merged_boxes : nullptr;
     cp.merge_alpha = c.merge_alpha;

@@ -13,8 +13,8 @@
 //   k_ccl_merge     every mask pixel resets its box record and unites with the start of its
 //                   horizontal run and with its N (else NW, NE) neighbours
 //   k_ccl_label     parent[i] = root (labels; -1 off the mask); box record of the root updated
-//   k_ccl_count     per tile of 4096 pixels: roots, and roots whose box passes A_min
-//   k_ccl_emit      ordered compaction of the passing roots into boxes[] (ascending label)
+//   k_ccl_boxes     per tile of 4096 pixels: roots, roots whose box passes A_min, and their ordered compaction
+//                   into boxes[] (ascending label) with a chained count over the tiles
 //   k_box_merge_pairs   (optional) eq. 12: boxes with close centres merged into the final detections
 #include "ddhf_internal.cuh"
 
@@ -132,50 +132,48 @@ __device__ __forceinline__ int block_sum(int a, int *s)
     return t;
 }
 
-__global__ void __launch_bounds__(1024) k_ccl_count(CclParams p)
-{
-    __shared__ int s[33];
-    const int base = blockIdx.x * kTile + threadIdx.x * 4;
-    int roots = 0, pass = 0;
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-        const int f = root_flags(p, base + j);
-        roots += f & 1;
-        pass += f >> 1;
-    }
-    const int tr = block_sum(roots, s);
-    const int tp = block_sum(pass, s);
-    if (threadIdx.x == 0) {
-        p.tile_sum[blockIdx.x] = tp;
-        if (tr) atomicAdd(&p.counters[DDHF_CNT_N_COMPONENTS], tr);
-    }
-}
-
-__global__ void __launch_bounds__(1024) k_ccl_emit(CclParams p, int n_tiles)
+// ---- k_ccl_boxes: count the roots of every tile and emit the passing ones in order, one pass -----------------
+// Tiles take tickets (so that a tile only ever waits for tiles that are already running), publish their number
+// of passing roots (tile_state[t] = count << 1 | 1; zeroed by the ingest stage) and add up the published counts of
+// the tiles before them: an ordered compaction without a second kernel.
+__global__ void __launch_bounds__(1024) k_ccl_boxes(CclParams p, int n_tiles)
 {
     __shared__ int s[33];
     __shared__ int s_scan[33];
-    // boxes before this tile, and (block 0) the total
-    int before = 0, total = 0;
-    for (int t = threadIdx.x; t < n_tiles; t += 1024) {
-        const int v = p.tile_sum[t];
-        total += v;
-        if (t < static_cast<int>(blockIdx.x)) before += v;
+    __shared__ int s_tile;
+    if (threadIdx.x == 0) s_tile = atomicAdd(p.tile_state + 1024, 1);
+    __syncthreads();
+    const int tile = s_tile;
+    const int base = tile * kTile + threadIdx.x * 4;
+    int f[4], roots = 0, a = 0;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const int fl = root_flags(p, base + j);
+        roots += fl & 1;
+        f[j] = fl >> 1;
+        a += f[j];
+    }
+    const int tr = block_sum(roots, s);
+    const int tp = block_sum(a, s);
+    if (threadIdx.x == 0) {
+        atomicExch(p.tile_state + tile, (tp << 1) | 1);
+        if (tr) atomicAdd(&p.counters[DDHF_CNT_N_COMPONENTS], tr);
+    }
+    // boxes in the tiles before this one (n_tiles <= 1024: one predecessor per thread)
+    int before = 0;
+    if (static_cast<int>(threadIdx.x) < tile) {
+        int v;
+        do { v = *reinterpret_cast<volatile int *>(p.tile_state + threadIdx.x); } while ((v & 1) == 0);
+        before = v >> 1;
     }
     before = block_sum(before, s);
-    if (blockIdx.x == 0) {
-        total = block_sum(total, s);
-        if (threadIdx.x == 0) {
-            p.counters[DDHF_CNT_N_BOXES_TOTAL] = total;
-            p.counters[DDHF_CNT_N_BOXES] = min(total, p.max_boxes);
-            if (total > p.max_boxes) atomicOr(&p.counters[DDHF_CNT_OVERFLOW], 2);
-        }
+    if (tile == n_tiles - 1 && threadIdx.x == 0) {
+        const int total = before + tp;
+        p.counters[DDHF_CNT_N_BOXES_TOTAL] = total;
+        p.counters[DDHF_CNT_N_BOXES] = min(total, p.max_boxes);
+        if (total > p.max_boxes) atomicOr(&p.counters[DDHF_CNT_OVERFLOW], 2);
     }
-    if (p.tile_sum[blockIdx.x] == 0) return;
-    const int base = blockIdx.x * kTile + threadIdx.x * 4;
-    int f[4], a = 0;
-#pragma unroll
-    for (int j = 0; j < 4; ++j) { f[j] = root_flags(p, base + j) >> 1; a += f[j]; }
+    if (tp == 0) return;
     // exclusive scan over the block
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     int inc = a;
@@ -404,8 +402,7 @@ int launch_ccl(const CclParams &p, cudaStream_t st)
     int launches = 0;
     k_ccl_merge<<<g256, 256, 0, st>>>(p); ++launches;
     k_ccl_label<<<g256, 256, 0, st>>>(p); ++launches;
-    k_ccl_count<<<n_tiles, 1024, 0, st>>>(p); ++launches;
-    k_ccl_emit<<<n_tiles, 1024, 0, st>>>(p, n_tiles); ++launches;
+    k_ccl_boxes<<<n_tiles, 1024, 0, st>>>(p, n_tiles); ++launches;
     if (p.merged != nullptr) {
         const int nt = (p.max_boxes + kMergeTile - 1) / kMergeTile;
         const int pair_tiles = nt * (nt + 1) / 2;

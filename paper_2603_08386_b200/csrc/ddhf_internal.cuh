@@ -148,6 +148,7 @@ struct IngestParams {
     uint8_t *mask;
     unsigned long long *work_cursor;
     int32_t *ccl_parent;         // [np] union-find array of the CCL stage, reset here
+    int32_t *ccl_tile_state;     // [1025] chained tile counts of k_ccl_boxes, zeroed here
 };
 
 struct CclParams {
@@ -156,7 +157,7 @@ struct CclParams {
     int32_t a_min, max_boxes;
     int32_t *parent;             // [np] = labels output or workspace; arrives filled with INT_MAX
     int32_t *rec;                // [np][5] x0,y0,x1,y1,n of the component rooted at the pixel (mask pixels only)
-    int32_t *tile_sum;           // [<= 1024] boxes that pass A_min per tile of 4096 pixels
+    int32_t *tile_state;         // [1024 + 1] per tile of 4096 pixels: passing boxes << 1 | published; [1024]: tickets (zeroed by k_init)
     ddhf_box *boxes;
     int32_t *counters;
     ddhf_box *merged;            // optional: eq. 12 detections

@@ -111,6 +111,7 @@ __global__ void k_init(IngestParams p)
         p.bkt_total[i] = 0; p.bkt_base[i] = 0; p.bkt_order[i] = i;      // identity order: no tile ran
         p.bkt_maxrun[i] = 64; p.giant_of[i] = -1;
     }
+    if (i <= 1024) p.ccl_tile_state[i] = 0;
     if (blockIdx.x == 0) {
         if (threadIdx.x < DDHF_N_COUNTERS) p.counters[threadIdx.x] = 0;
         if (threadIdx.x < kNumClasses) {
@@ -1426,7 +1427,7 @@ int launch_scans(const IngestParams &p, cudaStream_t st)
 int launch_ingest(const IngestParams &p, cudaStream_t st)
 {
     int launches = 0;
-    const int init_items = p.np > p.nb + 2 ? p.np : p.nb + 2;
+    const int init_items = max(max(p.np, p.nb + 2), 1025);      // pixels, buckets, CCL tile states
     k_init<<<(init_items + 255) / 256, 256, 0, st>>>(p); ++launches;
     IngestParams q = p;                      // k_bucket_sort writes row_ptr itself
     q.slab_row_ptr = p.row_ptr;
@@ -1440,7 +1441,7 @@ int launch_ingest(const IngestParams &p, cudaStream_t st)
 int launch_ingest_slide(const IngestParams &p, cudaStream_t st)
 {
     int launches = 0;
-    const int init_items = p.np > p.nb + 2 ? p.np : p.nb + 2;
+    const int init_items = max(max(p.np, p.nb + 2), 1025);      // pixels, buckets, CCL tile states
     k_init<<<(init_items + 255) / 256, 256, 0, st>>>(p); ++launches;
     IngestParams q = p;                      // the slab is bucketed into its own CSR
     q.csr_ev = p.slab_csr;
