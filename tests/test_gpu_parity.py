@@ -365,3 +365,36 @@ def test_sliding_window_restarts_and_empty_slabs(oracle):
         row_ptr, csr, _ = oracle.bucket(ev[lo:hi], W, H, t0, T)
         assert np.array_equal(g["row_ptr"], row_ptr) and np.array_equal(g["csr_ev"], csr), t0
     det.close()
+
+
+def test_sliding_window_with_a_stuck_pixel(oracle):
+    """ddhf_window_slide() with a pixel that fires 400 k events per window: the first window takes the giant-bucket
+    path, the slabs (80 k events of that pixel each) the chunked one-CTA path; every window bit-exact."""
+    from paper_2603_08386_b200 import binding
+    W, H, T, hop = 346, 260, 50_000, 10_000
+    rng = np.random.default_rng(5)
+    bg = wl.random_window(9, W, H, 300_000, 100_000, hot_fraction=0.2)
+    hot = np.zeros(800_000, dtype=wl.EVENT_DTYPE)
+    hot["x"], hot["y"] = 123, 45
+    hot["t"] = rng.integers(0, 100_000, size=len(hot))
+    hot["p"] = rng.integers(0, 2, size=len(hot)) * 2 - 1
+    ev = np.concatenate([bg, hot])
+    ev = ev[np.argsort(ev["t"], kind="stable")]
+    prm = dict(wl.preset(2), n_min=6)
+    t = ev["t"]
+    det = binding.Detector(prm, max_events=len(ev), want_power=False)
+    d_ev = det.upload(ev)
+    prev_hi = None
+    for k in range(5):
+        t0 = k * hop
+        lo, hi = int(np.searchsorted(t, t0, "left")), int(np.searchsorted(t, t0 + T, "left"))
+        if prev_hi is None:
+            det.slide(d_ev, hi - lo, t0, T, offset_events=lo)
+        else:
+            det.slide(d_ev, hi - prev_hi, t0, T, offset_events=prev_hi)
+        prev_hi = hi
+        g = det.results()
+        row_ptr, csr, _ = oracle.bucket(ev[lo:hi], W, H, t0, T)
+        assert np.array_equal(g["row_ptr"], row_ptr) and np.array_equal(g["csr_ev"], csr), k
+        assert (g["counters"][9] >= 1) == (k == 0), (k, g["counters"][9])
+    det.close()
