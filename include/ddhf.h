@@ -51,6 +51,18 @@ extern "C" {
 #define DDHF_FLAG_SCORE_ALL   1u  /* comb score on every active pixel (R14); default is the
                                      paper's order: only where SF <= tau_sf (L139)        */
 #define DDHF_FLAG_TIMING      2u  /* record per-stage CUDA events (ddhf_stage_ms)          */
+#define DDHF_FLAG_NUFFT       4u  /* spectra of long rows by a type-1 non-uniform FFT (footnote 1:
+                                     "NUFFTs [22] offer asymptotic acceleration for large sample counts") instead
+                                     of the direct sum of eq. 6.  Rows of at least (flags >> 16) events take it
+                                     (0: DDHF_NUFFT_MIN_DEFAULT); longer than 4096 events they are split and
+                                     summed directly as always.  Approximate: spreading on a 2x oversampled
+                                     grid with an 8-cell kernel, aliasing error <= 1e-6 of sum |w| in amplitude,
+                                     i.e. far inside the 1e-3-of-peak power tolerance of the direct path; the
+                                     cost of such a row does not depend on its length.  Honoured only where it
+                                     applies: 1024 < n_freq <= 2048, one queue row per pixel (max_scored = 0
+                                     default), and windows with df_hz * window <= 0.24 (events within a quarter
+                                     turn of the finest grid phase); otherwise the call runs the direct path. */
+#define DDHF_NUFFT_MIN_DEFAULT 96
 
 /* indices into ddhf_outputs.counters (int32[DDHF_N_COUNTERS]) */
 #define DDHF_CNT_N_IN          0  /* events kept (inside window and sensor)                */

@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("DDHF_LIB", os.path.join(_HERE, "libddhf.so"))
 
 DDHF_OK, DDHF_E_INVAL, DDHF_E_CAPACITY, DDHF_E_CUDA, DDHF_E_NOMEM = 0, -1, -2, -3, -4
-DDHF_FLAG_SCORE_ALL, DDHF_FLAG_TIMING = 1, 2
+DDHF_FLAG_SCORE_ALL, DDHF_FLAG_TIMING, DDHF_FLAG_NUFFT = 1, 2, 4
 (CNT_N_IN, CNT_N_DROPPED, CNT_N_ACTIVE, CNT_N_BOXES, CNT_N_BOXES_TOTAL, CNT_OVERFLOW,
  CNT_N_SCORED, CNT_N_COMPONENTS, CNT_N_MERGED) = range(9)
 N_COUNTERS = 16
@@ -244,7 +244,7 @@ class Detector:
     def __init__(self, params: dict[str, Any], *, max_events: int, max_active: int | None = None,
                  max_boxes: int = 4096, max_scored: int = 0, score_all: bool = False, timing: bool = False,
                  want_power: bool = False, want_labels: bool = True, want_debug: bool = False,
-                 device: str = "cuda:0"):
+                 nufft: bool = False, nufft_min: int = 0, device: str = "cuda:0"):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("DDHF needs a CUDA device (no CPU fallback)")
@@ -252,6 +252,10 @@ class Detector:
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
         flags = (DDHF_FLAG_SCORE_ALL if score_all else 0) | (DDHF_FLAG_TIMING if timing else 0)
+        if nufft:       # long rows by a non-uniform FFT (ddhf.h: DDHF_FLAG_NUFFT; bits 16-31: minimum row length)
+            if not 0 <= nufft_min < 65536:
+                raise ValueError("nufft_min must be in [0, 65535]")
+            flags |= DDHF_FLAG_NUFFT | (int(nufft_min) << 16)
         self.params = dict(params)
         self.cfg = make_config(params, max_events=max_events, max_active=max_active,
                                max_boxes=max_boxes, max_scored=max_scored, flags=flags)

@@ -28,6 +28,10 @@ struct ddhf_handle {
     bool fallback = true;                  // the NDFT kernel variant with in-place scoring (queue smaller than the sensor)
     ScoreParams sp{};
     uint64_t g_f0 = 0, g_d = 0, g_h = 0;
+    bool nufft = false;                     // DDHF_FLAG_NUFFT and the grid / queue allow it
+    int nufft_min = 0;                      // rows of at least that many events take the NUFFT path
+    uint64_t g_nc = 0, g_nt = 0;            // its frequency constants (nufft.cu)
+    size_t off_hot = 0, off_nuscr = 0;
     unsigned char *d_tables = nullptr;      // comb tables (num_tab | piece_tab | meta)
     int band_size = 0;
     int ndft_blocks_per_sm = 1, full_blocks_per_sm = 1, score_blocks_per_sm = 1;
@@ -248,6 +252,19 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
     h->g_h = 0ull - freq_const(16.0 * c.df_hz);
     h->g_d = 0ull - freq_const(c.df_hz);
     h->g_f0 = 0ull - freq_const(c.f_min_hz + (32.0 * tn - 16.0) * c.df_hz);
+    // NUFFT path for long rows: needs the 4096-cell grid and a queue row per pixel (it never scores in place)
+    if ((c.flags & DDHF_FLAG_NUFFT) && nufft_supported(c.n_freq) && !h->fallback) {
+        if (nufft_configure() != cudaSuccess) {
+            const std::string msg = std::string("ddhf_create: ") + cudaGetErrorString(cudaGetLastError());
+            cudaFree(h->d_tables);
+            delete h;
+            return fail(nullptr, DDHF_E_CUDA, msg);
+        }
+        h->nufft = true;
+        h->nufft_min = static_cast<int>(c.flags >> 16) ? static_cast<int>(c.flags >> 16) : DDHF_NUFFT_MIN_DEFAULT;
+        h->g_nc = 0ull - freq_const(c.f_min_hz + 1024.0 * c.df_hz);
+        h->g_nt = freq_const(c.df_hz);
+    }
 
     // ---- workspace layout -----------------------------------------------------------------------
     h->n_tiles = (h->np + kScanTile - 1) / kScanTile;
@@ -297,6 +314,10 @@ extern "C" int ddhf_create(const ddhf_config *cfg, ddhf_handle **out)
     h->off_slide = o;      o = align_up(o + 2 * (sizeof(int32_t) * (static_cast<size_t>(h->np) + 2) + sizeof(uint32_t) * static_cast<size_t>(c.max_events))
                                          + sizeof(int32_t) * static_cast<size_t>(h->np) + sizeof(uint32_t) * static_cast<size_t>(c.max_events) + 1024);
     h->off_merge = o;      o = align_up(o + sizeof(int32_t) * 6 * static_cast<size_t>(c.max_boxes));
+    if (h->nufft) {
+        h->off_hot = o;    o = align_up(o + sizeof(WorkItem) * static_cast<size_t>(h->np));
+        h->off_nuscr = o;  o = align_up(o + sizeof(float) * 2048 * static_cast<size_t>(h->sm_count) * nufft_warps());
+    }
     h->ws_bytes = o;
 
     if (c.flags & DDHF_FLAG_TIMING)
@@ -386,6 +407,12 @@ static int run_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n, int
     }
     ip.split_cnt = reinterpret_cast<int32_t *>(ws + h->off_splitcnt);
     ip.ccl_parent = cp_parent;
+    const bool use_nufft = h->nufft && nufft_window_fits(c.df_hz, window_us);
+    if (use_nufft) {
+        ip.hot_work = reinterpret_cast<WorkItem *>(ws + h->off_hot);
+        ip.hot_min = h->nufft_min;
+        ip.hot_cursor = reinterpret_cast<int32_t *>(ws + h->off_cursor + 104);
+    }
 
     NdftParams np{};
     np.work = ip.work; np.csr_ev = out->csr_ev; np.counters = out->counters;
@@ -420,6 +447,13 @@ static int run_window(ddhf_handle *h, const ddhf_event *d_events, int64_t n, int
     if (timing) cudaEventRecord(h->ev[0], st);
     launches += (mode == 2) ? launch_ingest_slide(ip, st) : launch_ingest(ip, st);
     if (timing) cudaEventRecord(h->ev[1], st);
+    if (use_nufft) {
+        NufftParams nq{};
+        nq.nd = np; nq.hot = ip.hot_work; nq.n_hot = ip.sync + 15; nq.cursor = ip.hot_cursor;
+        nq.g_c = h->g_nc; nq.g_t = h->g_nt;
+        nq.scratch = reinterpret_cast<float *>(ws + h->off_nuscr);
+        launches += launch_nufft(nq, h->sm_count, st);
+    }
     NdftParams seg = np;                                   // the segment pass of the lean variant
     seg.work = ip.seg_work; seg.n_work = ip.sync + 9; seg.work_cursor = ip.work_cursor2;
     launches += launch_ndft(np, ip.seg_work ? &seg : nullptr, c.n_freq, h->band_size, h->fallback,

@@ -93,6 +93,16 @@ struct NdftParams {
     ScoreParams sp;
 };
 
+// The NUFFT path for long rows (nufft.cu): the rows of the hot list, one warp each
+struct NufftParams {
+    NdftParams nd;               // csr_ev, outputs, scoring queue and constants, as for k_ndft_score
+    const WorkItem *hot;         // DEVICE [*n_hot] rows (unordered)
+    const int32_t *n_hot;
+    int32_t *cursor;             // rows handed out
+    uint64_t g_c, g_t;           // 2^64 1e-6 x: -(f_min + 1024 df) (mod 2^64), df
+    float *scratch;              // [warps of the grid][2048] the row in bin order
+};
+
 struct IngestParams {
     const ddhf_event *events;    // 16-byte events, or (packed) ddhf_event8 records through the same pointer
     int32_t packed;
@@ -122,11 +132,14 @@ struct IngestParams {
     int32_t *sync;               // [16] 0: tiles finished, 1: chunk rows handed out, 2-3: scoring queue counts,
                                  //     4: work items, 5: split rows, 6: partials, 7: arrival counters handed out, 8: box-merge CTAs finished,
                                  //     9: items of the segment list, 10: giant buckets, 11: their chunks, 12-13: chunk tickets of
-                                 //     k_bucket_sort / k_worklist, 14: giant chunk rows handed out
+                                 //     k_bucket_sort / k_worklist, 14: giant chunk rows handed out, 15: rows of the hot list
     SplitRow *split_tab;         // rows longer than kSplitMin (see NdftParams)
     int32_t *split_cnt;
     WorkItem *seg_work;          // when set: the segments of split rows go to this list (count in sync[9]) instead of `work`
     unsigned long long *work_cursor2;   // cursor of the segment pass
+    WorkItem *hot_work;          // when set: unsplit rows of >= hot_min events go to this list (count in sync[15]), for k_nufft_score
+    int32_t hot_min;
+    int32_t *hot_cursor;         // rows of the hot list handed out (zeroed by k_init)
     // sliding windows (ddhf_window_slide): NULL otherwise
     const int32_t *prev_row_ptr; // [np + 1] CSR of the previous window (workspace copy)
     const uint32_t *prev_csr;
@@ -182,6 +195,12 @@ int launch_ndft(const NdftParams &p, const NdftParams *seg_pass, int n_freq, int
                                              // split rows); else the lean variant, followed by the full one on `seg_pass` (the segment list)
                                              // `between` (optional) is recorded after the NDFT kernel, before the scoring kernel
 int launch_ccl(const CclParams &p, cudaStream_t st);
+bool nufft_supported(int n_freq);            // frequency grids the NUFFT path is built for (1024 < n_freq <= 2048)
+bool nufft_window_fits(double df_hz, int64_t window_us);   // the window's events stay inside the quarter turn the path holds
+size_t nufft_smem_bytes();
+int nufft_warps();                           // warps per CTA of k_nufft_score (one scratch row each)
+cudaError_t nufft_configure();               // tables and shared-memory opt-in on the current device
+int launch_nufft(const NufftParams &q, int grid, cudaStream_t st);
 int ndft_bins_per_lane(int n_freq);          // 8, 16, 32 or 64
 int ndft_tn(int n_freq);                     // offset pairs per centre for that kernel
 int ndft_padded_bins(int n_freq);            // row length of the deferred-scoring queue

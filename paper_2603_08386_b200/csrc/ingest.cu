@@ -94,7 +94,12 @@ __device__ __forceinline__ int row_segments(int n, int &seg_len)
 
 // Items a row of n_seg segments adds to the size-classed work list: its segments, unless they go to the
 // segment list of their own (lean NDFT kernel followed by the segment pass)
-__device__ __forceinline__ int class_items(const IngestParams &p, int n_seg) { return (p.seg_work && n_seg > 1) ? 0 : n_seg; }
+// (nor a long unsplit row that goes to the hot list of the NUFFT path)
+__device__ __forceinline__ bool is_hot(const IngestParams &p, int n, int n_seg) { return p.hot_work && n_seg == 1 && n >= p.hot_min; }
+__device__ __forceinline__ int class_items(const IngestParams &p, int n, int n_seg)
+{
+    return ((p.seg_work && n_seg > 1) || is_hot(p, n, n_seg)) ? 0 : n_seg;
+}
 
 // ---- k_init: per-pixel maps for inactive pixels, zeroed totals and counters ---------------
 __global__ void k_init(IngestParams p)
@@ -119,7 +124,11 @@ __global__ void k_init(IngestParams p)
             p.class_cur[threadIdx.x] = 0;
         }
         if (threadIdx.x < 16) p.sync[threadIdx.x] = 0;
-        if (threadIdx.x == 0) { *p.work_cursor = 0ull; if (p.work_cursor2) *p.work_cursor2 = 0ull; }
+        if (threadIdx.x == 0) {
+            *p.work_cursor = 0ull;
+            if (p.work_cursor2) *p.work_cursor2 = 0ull;
+            if (p.hot_cursor) *p.hot_cursor = 0;
+        }
     }
 }
 
@@ -657,7 +666,7 @@ __device__ __forceinline__ void bucket_body(const IngestParams &p, uint32_t *s_r
             int seg_len;
             const int n_seg = row_segments(n, seg_len);
             atomicAdd(&s_act, 1);
-            if (class_items(p, n_seg)) atomicAdd(&s_class[size_class(seg_len)], class_items(p, n_seg));
+            if (class_items(p, n, n_seg)) atomicAdd(&s_class[size_class(seg_len)], class_items(p, n, n_seg));
         }
     };
     auto publish_tally = [&]() {
@@ -905,7 +914,7 @@ __device__ __forceinline__ void giant_finish(const IngestParams &p, uint32_t *s_
                     int seg_len;
                     const int n_seg = row_segments(static_cast<int>(v[k]), seg_len);
                     atomicAdd(&s_act2, 1);
-                    if (class_items(p, n_seg)) atomicAdd(&s_class2[size_class(seg_len)], class_items(p, n_seg));
+                    if (class_items(p, static_cast<int>(v[k]), n_seg)) atomicAdd(&s_class2[size_class(seg_len)], class_items(p, static_cast<int>(v[k]), n_seg));
                 }
             }
             ex += v[k];
@@ -1061,6 +1070,7 @@ __device__ __forceinline__ void emit_work(const IngestParams &p, WorkItem *dst, 
 {
     WorkItem it;
     if (n_seg == 1) {
+        if (is_hot(p, n, n_seg)) dst = p.hot_work + atomicAdd(p.sync + 15, 1);
         it.row_begin = off;
         it.n = n;
         it.pix = pix;
@@ -1107,7 +1117,7 @@ __global__ void __launch_bounds__(1024) k_scan_reduce(IngestParams p)
             ++act;
             int seg_len;
             const int n_seg = row_segments(v[j], seg_len);
-            if (class_items(p, n_seg)) atomicAdd(&s_cls[size_class(seg_len)], class_items(p, n_seg));
+            if (class_items(p, v[j], n_seg)) atomicAdd(&s_cls[size_class(seg_len)], class_items(p, v[j], n_seg));
         }
     }
     int ta, tb;
@@ -1169,7 +1179,7 @@ __global__ void __launch_bounds__(1024) k_scan_apply(IngestParams p)
             ++act;
             int seg_len;
             const int n_seg = row_segments(v[j], seg_len);
-            lrank[j] = atomicAdd(&s_cls[size_class(seg_len)], class_items(p, n_seg));
+            lrank[j] = atomicAdd(&s_cls[size_class(seg_len)], class_items(p, v[j], n_seg));
         }
     }
     int ta, tb;
@@ -1268,7 +1278,7 @@ __global__ void __launch_bounds__(1024) k_worklist(IngestParams p)
             ++act;
             int seg_len;
             const int n_seg = row_segments(v[j], seg_len);
-            lrank[j] = atomicAdd(&s_cls[size_class(seg_len)], class_items(p, n_seg));
+            lrank[j] = atomicAdd(&s_cls[size_class(seg_len)], class_items(p, v[j], n_seg));
         }
     }
     int t1, t2;

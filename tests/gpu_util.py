@@ -17,11 +17,11 @@ REL_TOL = 1e-3
 
 
 def run_gpu(params, events, t0, window_us, *, score_all=False, want_power=True, want_debug=False,
-            max_active=None, max_boxes=4096, max_events=None, timing=False, max_scored=0):
+            max_active=None, max_boxes=4096, max_events=None, timing=False, max_scored=0, **det_kw):
     from paper_2603_08386_b200 import binding
     det = binding.Detector(params, max_events=max_events or max(len(events), 1),
                            max_active=max_active, max_boxes=max_boxes, max_scored=max_scored, score_all=score_all,
-                           want_power=want_power, want_debug=want_debug, timing=timing)
+                           want_power=want_power, want_debug=want_debug, timing=timing, **det_kw)
     d_ev = det.upload(events) if len(events) else None
     det.window(d_ev, len(events), t0, window_us)
     res = det.results()

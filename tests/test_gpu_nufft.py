@@ -1,0 +1,100 @@
+"""GPU parity of the optional NUFFT path for long rows (DDHF_FLAG_NUFFT, PAPER.md L141 footnote 1)
+against the same float64 oracle and the same tolerances as the direct sum.  Run with `pytest -m gpu` on a B200."""
+import numpy as np
+import pytest
+
+from paper_2603_08386_b200 import workloads as wl
+
+import gpu_util as gu
+from test_gpu_parity import _full_compare, _sampled_compare, _whole_window_compare
+
+pytestmark = pytest.mark.gpu
+
+
+def _grid2048(width, height, window_us=100_000):
+    prm = dict(wl.make(1).params)
+    prm.update(width=width, height=height, f_min_hz=0.0, df_hz=5000.0 / 2048, n_freq=2048, n_harm=8, half_bw_bins=10,
+               f0_min_hz=100.0, f0_step_hz=5.0, n_f0=81, h_min=4, n_min=1, k_lo=1)
+    return prm
+
+
+@pytest.mark.parametrize("score_all", [False, True])
+def test_nufft_config4_quarter_scale(oracle, score_all):
+    """Every spectrum of the config-4 scene on a 320x180 sensor, rows of >= 32 events through the NUFFT."""
+    w = wl.make(4, scale=0.25)
+    gpu, orc, err = _full_compare(oracle, w, w.params, score_all=score_all, nufft=True, nufft_min=32)
+    n = np.diff(orc["row_ptr"])[orc["active_idx"]]
+    assert (n >= 32).sum() > 1000 and gpu["launches"] == 12
+    print(f"nufft cfg4/16 score_all={score_all}: rows through the NUFFT {(n >= 32).sum()} of {len(n)}, "
+          f"power err/peak {err:.2e}, mask {gpu['mask'].sum()}")
+
+
+def test_nufft_every_row_length(oracle):
+    """Rows of 1 .. 4096 events (the longest unsplit row), one pixel each, all through the NUFFT (nufft_min = 1);
+    a row of 4097 events is split and summed directly as always."""
+    lens = [1, 2, 3, 4, 5, 7, 8, 9, 31, 32, 33, 63, 64, 65, 100, 255, 256, 257, 1000, 2047, 4095, 4096, 4097]
+    W = len(lens)
+    prm = _grid2048(W, 1)
+    rng = np.random.default_rng(5)
+    x = np.repeat(np.arange(W), lens)
+    t = rng.integers(0, 100_000, size=len(x))
+    t[:3] = [0, 99_999, 99_999]                      # both ends of the window
+    ev = wl._pack(x, np.zeros_like(x), rng.integers(0, 2, size=len(x)) * 2 - 1, t)
+    ev = ev[rng.permutation(len(ev))]                # unsorted input: rows keep the input order
+    orc = oracle.window(prm, ev, 0, 100_000, score_all=True, want_power=True)
+    gpu = gu.run_gpu(prm, ev, 0, 100_000, score_all=True, want_power=True, nufft=True, nufft_min=1)
+    gu.check_csr(gpu, orc)
+    err = np.abs(gpu["power"].astype(np.float64) - orc["power"]).max(axis=1) / orc["power"].max(axis=1)
+    print("  power err / peak by row length:", {n: f"{e:.1e}" for n, e in zip(lens, err)})
+    assert err.max() <= gu.POWER_TOL
+    gu.check_maps(gpu, orc, prm, score_all=True, oracle_mod=oracle, orc_power=orc["power"])
+    # and against the direct path on the same device: both within FP32 of each other
+    ref = gu.run_gpu(prm, ev, 0, 100_000, score_all=True, want_power=True)
+    d = np.abs(gpu["power"] - ref["power"]).max(axis=1) / ref["power"].max(axis=1)
+    assert d.max() <= 2e-4, d
+    assert np.array_equal(gpu["power"][-1], ref["power"][-1])        # the split row took the same path
+
+
+def test_nufft_periodic_train_peaks(oracle):
+    """A strictly periodic train at f0 puts its peaks at k f0 (north_star's pin), here through the NUFFT."""
+    prm = _grid2048(4, 1)
+    f0 = 250.0
+    t = np.round(np.arange(25) * 1e6 / f0).astype(np.int64)
+    ev = wl._pack(np.full(25, 2), np.zeros(25, int), np.ones(25, int), t)
+    gpu = gu.run_gpu(prm, ev, 0, 100_000, score_all=True, want_power=True, nufft=True, nufft_min=1)
+    P = gpu["power"][0]
+    for k in (1, 2, 3, 4):
+        j = int(round(k * f0 / prm["df_hz"]))
+        assert abs(int(np.argmax(P[j - 20:j + 21])) - 20) <= 1 and P[j] >= 0.95 * 25 ** 2
+    assert abs(P[0] - 625.0) <= 1e-3 * 625.0                         # P_0 = (sum w)^2
+
+
+def test_nufft_ignored_where_it_does_not_apply(oracle):
+    """1024-bin grids, windows longer than a quarter turn of the grid phase and handles whose scoring queue is
+    smaller than the sensor run the direct path: results identical to a handle without the flag."""
+    w = wl.make(2)
+    a = gu.run_gpu(w.params, w.events, 0, w.window_us, want_power=True, nufft=True, nufft_min=1)
+    b = gu.run_gpu(w.params, w.events, 0, w.window_us, want_power=True)
+    assert np.array_equal(a["power"], b["power"]) and np.array_equal(a["sf"], b["sf"], equal_nan=True)
+    prm = _grid2048(64, 64)
+    ev = wl.random_window(3, 64, 64, 60_000, 110_000, hot_fraction=0.5)
+    for kw, win in ((dict(), 110_000), (dict(max_scored=100), 100_000)):
+        e = ev[ev["t"] < win]
+        a = gu.run_gpu(prm, e, 0, win, want_power=True, nufft=True, nufft_min=1, **kw)
+        b = gu.run_gpu(prm, e, 0, win, want_power=True, **kw)
+        assert np.array_equal(a["power"], b["power"]) and a["launches"] == b["launches"]
+
+
+@pytest.mark.slow
+def test_nufft_config4_whole_window(oracle):
+    """Whole config-4 window, every active pixel's SF / score / mask and the boxes, rows of >= 96 events (the
+    default) through the NUFFT: same bars as test_config4_whole_window."""
+    w = wl.make(4)
+    _whole_window_compare(oracle, w, w.params, w.events, 0, score_all=False, name="cfg4 whole window, NUFFT", nufft=True)
+
+
+@pytest.mark.slow
+def test_nufft_config3_full_size_sampled(oracle):
+    w = wl.make(3)
+    gpu, wp, wsf, ws = _sampled_compare(oracle, w, w.params, w.events, 0, 400, score_all=False, nufft=True, nufft_min=48)
+    print(f"nufft cfg3: worst power {wp:.2e}, SF {wsf:.2e}, score {ws:.2e}")

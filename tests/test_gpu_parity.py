@@ -10,12 +10,12 @@ import gpu_util as gu
 pytestmark = pytest.mark.gpu
 
 
-def _full_compare(oracle, w, params, *, score_all, events=None, t0=None):
+def _full_compare(oracle, w, params, *, score_all, events=None, t0=None, **det_kw):
     ev = w.events if events is None else events
     t0 = w.t0_us if t0 is None else t0
     orc = oracle.window(params, ev, t0, w.window_us, score_all=score_all, want_power=True)
     gpu = gu.run_gpu(params, ev, t0, w.window_us, score_all=score_all, want_power=True,
-                     want_debug=True)
+                     want_debug=True, **det_kw)
     gu.check_csr(gpu, orc)
     err = gu.power_error(gpu["power"], orc["power"])
     assert err <= gu.POWER_TOL, f"power error / peak = {err}"
@@ -97,10 +97,10 @@ def test_config4_quarter_scale(oracle):
           f"scored {gpu['n_scored']}, mask {gpu['mask'].sum()}, boxes {gpu['n_boxes']}")
 
 
-def _sampled_compare(oracle, w, params, ev, t0, n_sample, score_all, seed=0):
+def _sampled_compare(oracle, w, params, ev, t0, n_sample, score_all, seed=0, **det_kw):
     """Full-size run on the GPU; CSR compared in full; spectra / SF / comb on sampled pixels
     the oracle computes one by one; CCL against the oracle's CCL of the same mask."""
-    gpu = gu.run_gpu(params, ev, t0, w.window_us, score_all=score_all, want_power=True)
+    gpu = gu.run_gpu(params, ev, t0, w.window_us, score_all=score_all, want_power=True, **det_kw)
     row_ptr, csr, dropped = oracle.bucket(ev, params["width"], params["height"], t0, w.window_us)
     assert np.array_equal(gpu["row_ptr"], row_ptr) and np.array_equal(gpu["csr_ev"], csr)
     assert gpu["n_dropped"] == dropped
@@ -242,12 +242,12 @@ def test_config4_bench_launch_configuration(oracle):
 # merged detections; only the spectra stay sampled (tests above).  The oracle needs 10-30 s per
 # window on the box's host cores.
 # ---------------------------------------------------------------------------------------------
-def _whole_window_compare(oracle, w, params, ev, t0, *, score_all, name):
+def _whole_window_compare(oracle, w, params, ev, t0, *, score_all, name, **det_kw):
     import time
     t = time.perf_counter()
     orc = oracle.window(params, ev, t0, w.window_us, score_all=score_all, want_power=False)
     t_orc = time.perf_counter() - t
-    gpu = gu.run_gpu(params, ev, t0, w.window_us, score_all=score_all, want_power=False)
+    gpu = gu.run_gpu(params, ev, t0, w.window_us, score_all=score_all, want_power=False, **det_kw)
     gu.check_csr(gpu, orc)
 
     def power_of(pix):
