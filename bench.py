@@ -181,7 +181,7 @@ def aggregate_over_ranks(time_ms: float, units: float, world: int, device="cpu")
 
 
 def measure(w, *, steps, warmup, dev, world=1, local_rank=0, score_all=False, spectra=False, params=None, name="",
-            slide=False):
+            slide=False, nufft=None):
     """Device-resident timing of `steps` windows of workload `w` (after `warmup`): whole-window CUDA-event
     time, per-stage times, clocks sampled during the timed region.  Returns (record, detector state)."""
     import torch
@@ -191,7 +191,7 @@ def measure(w, *, steps, warmup, dev, world=1, local_rank=0, score_all=False, sp
     # the stream stays resident; max_events = the largest window handed to ddhf_window
     max_ev = len(w.events) if w.n_windows == 1 else max(w.window_slice(k)[1] for k in range(w.n_windows))
     det = binding.Detector(prm, max_events=max_ev, score_all=score_all, timing=True, want_power=spectra, want_labels=False,
-                           device=f"cuda:{local_rank}",
+                           nufft=nufft is not None, nufft_min=int(nufft or 0), device=f"cuda:{local_rank}",
                            max_active=(prm["width"] * prm["height"]) if spectra else 1)
     d_ev = det.upload(w.events)
     wins = window_list(w, warmup + steps)
@@ -284,6 +284,7 @@ def measure(w, *, steps, warmup, dev, world=1, local_rank=0, score_all=False, sp
                    "scored_pixels": res0["n_scored"], "terms_per_step": terms_per_step,
                    "mask_pixels": int(res0["mask"].sum()), "boxes": res0["n_boxes"],
                    "score_all": bool(score_all), "spectra_to_hbm": bool(spectra),
+                   "nufft_min_events": (None if nufft is None else (int(nufft) or 64)),
                    "ingest_mode": ("ddhf_window_slide: only the events that follow the previous window are sorted; the "
                                    "sequence restarts from scratch when the window list wraps around") if slide
                                   else "ddhf_window: every window bucketed from scratch",
@@ -296,7 +297,9 @@ def measure(w, *, steps, warmup, dev, world=1, local_rank=0, score_all=False, sp
         "latency_ms": {"p50": float(np.percentile(per_step_ms, 50)), "p99": float(np.percentile(per_step_ms, 99)),
                        "ingest": float(stage[:, 0].mean()), "ndft": ndft_ms, "comb_score": float(stage[:, 2].mean()),
                        "ccl": float(stage[:, 3].mean())},
-        "ndft_frac_of_fp32_peak": terms_per_step * FLOP_PER_TERM / (ndft_ms * 1e-3) / 1e12 / NOMINAL_FP32_TFLOPS,
+        # (with the NUFFT path the long rows do not execute their terms: no roofline fraction, and `value` is nominal)
+        "ndft_frac_of_fp32_peak": None if nufft is not None else
+                                  terms_per_step * FLOP_PER_TERM / (ndft_ms * 1e-3) / 1e12 / NOMINAL_FP32_TFLOPS,
         "clocks": sampler.summary(), "gpu_launches": launches_per_window * steps,
     }
     state = dict(det=det, d_ev=d_ev, wins=wins, terms_by_win=terms_by_win, stage=stage, terms_total=terms_total,
@@ -315,6 +318,9 @@ def main():
     ap.add_argument("--no-sub", action="store_true", help="skip the variant measurements (the `sub` object)")
     ap.add_argument("--score-all", action="store_true", help="comb score on every active pixel (R14)")
     ap.add_argument("--spectra", action="store_true", help="also write the compact power spectra to HBM")
+    ap.add_argument("--nufft", type=int, default=None, metavar="MIN",
+                    help="rows of >= MIN events (0: the library default, 64) by the NUFFT path (DDHF_FLAG_NUFFT): approximate, "
+                         "so the Gterms/s of such a run is nominal (terms of the direct sum it replaces / time)")
     ap.add_argument("--slide", action="store_true", help="streaming workloads: ddhf_window_slide (incremental CSR)")
     args = ap.parse_args()
     steps, warmup = max(args.steps, 1), max(args.warmup, 3 if args.impl == "ours" else 0)
@@ -355,7 +361,7 @@ def main():
 
     w = load_workload(args.workload)
     rec, st = measure(w, steps=steps, warmup=warmup, dev=dev, world=world, local_rank=local_rank,
-                      score_all=args.score_all, spectra=args.spectra, name=args.workload, slide=args.slide)
+                      score_all=args.score_all, spectra=args.spectra, name=args.workload, slide=args.slide, nufft=args.nufft)
     det, wins, terms_by_win, stage, prm = st["det"], st["wins"], st["terms_by_win"], st["stage"], st["prm"]
     barrier = st["barrier"]
 
@@ -463,6 +469,10 @@ def main():
                 "gterms_per_s_kernel": terms_per_step / (ndft_ms * 1e-3) / 1e9,
                 "measured_fma_peak_tflops": {"ffma": probe[0], "ffma2": probe[1]},
                 "frac_of_measured_fma_peak": achieved / max(probe)}
+    if args.nufft is not None:
+        # the long rows went through k_nufft_score and did not execute their terms: no roofline claim for this run
+        roofline.update(achieved=None, frac=None, frac_of_measured_fma_peak=None, gterms_per_s_kernel=None,
+                        note="--nufft: the terms of the direct sum are nominal for the rows the NUFFT path took")
     line = {
         "metric": "ndft_gterms_per_s", "value": rec["value"], "unit": "Gterms/s", "n_gpus": world,
         "steps": steps, "warmup": warmup, "ms_per_step": rec["ms_per_step"], "higher_is_better": True,
@@ -492,6 +502,10 @@ def main():
         run_sub("cfg4_score_all", w, score_all=True)
         run_sub("cfg4_table2_thresholds", w, params=dict(w.params, tau_sf=0.89, tau_comb=1.5))
         run_sub("cfg4_spectra_to_hbm", w, spectra=True)
+        # long rows by the NUFFT path; reported apart -- its Gterms/s is nominal
+        for m in (32, 64, 128):
+            run_sub(f"cfg4_nufft_rows_ge_{m}", w, nufft=m)
+        run_sub("cfg4_nufft_score_all", w, nufft=64, score_all=True)
         run_sub("paper_point", workloads.paper_native())
         run_sub("cfg3", workloads.make(3))
         w5 = workloads.make(5, n_windows=100)

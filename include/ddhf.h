@@ -62,7 +62,7 @@ extern "C" {
                                      applies: 1024 < n_freq <= 2048, one queue row per pixel (max_scored = 0
                                      default), and windows with df_hz * window <= 0.24 (events within a quarter
                                      turn of the finest grid phase); otherwise the call runs the direct path. */
-#define DDHF_NUFFT_MIN_DEFAULT 96
+#define DDHF_NUFFT_MIN_DEFAULT 64
 
 /* indices into ddhf_outputs.counters (int32[DDHF_N_COUNTERS]) */
 #define DDHF_CNT_N_IN          0  /* events kept (inside window and sensor)                */

@@ -186,10 +186,15 @@ __global__ void __launch_bounds__(kNuWarps * 32, 1) k_nufft_score(NufftParams q)
 #pragma unroll 1
         for (int r = 0; r < 4; ++r) {
             float2 v[32];
+            if (r == 0) {
 #pragma unroll
-            for (int n2 = 0; n2 < 32; ++n2) {
-                const float2 x = grid[lane + 32 * n2], w = c_w128[r][n2];
-                v[n2] = make_float2(fmaf(-x.y, w.y, x.x * w.x), fmaf(x.y, w.x, x.x * w.y));
+                for (int n2 = 0; n2 < 32; ++n2) v[n2] = grid[lane + 32 * n2];
+            } else {
+#pragma unroll
+                for (int n2 = 0; n2 < 32; ++n2) {
+                    const float2 x = grid[lane + 32 * n2], w = c_w128[r][n2];
+                    v[n2] = make_float2(fmaf(-x.y, w.y, x.x * w.x), fmaf(x.y, w.x, x.x * w.y));
+                }
             }
             fft32(v);                                                    // over n2: v[brev5(m2)]
             const float2 *tw = g_tw + r * 1024 + lane;

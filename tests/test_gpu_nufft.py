@@ -87,7 +87,7 @@ def test_nufft_ignored_where_it_does_not_apply(oracle):
 
 @pytest.mark.slow
 def test_nufft_config4_whole_window(oracle):
-    """Whole config-4 window, every active pixel's SF / score / mask and the boxes, rows of >= 96 events (the
+    """Whole config-4 window, every active pixel's SF / score / mask and the boxes, rows of >= 64 events (the
     default) through the NUFFT: same bars as test_config4_whole_window."""
     w = wl.make(4)
     _whole_window_compare(oracle, w, w.params, w.events, 0, score_all=False, name="cfg4 whole window, NUFFT", nufft=True)
