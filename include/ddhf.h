@@ -250,6 +250,36 @@ int ddhf_fma_peak_probe(float ms_target, float *tflops_out, void *cuda_stream);
 
 int ddhf_destroy(ddhf_handle *h);
 
+/* ---- Entry point that allocates nothing ---------------------------------------------------------------------
+ * Stage a8 on a caller's mask: 8-connected component labelling, bounding boxes, the A_min filter
+ * and, if merge_alpha > 0, the final detections of eq. 12 (L166) -- the same kernels ddhf_window() runs after the
+ * comb stage, results bit-identical.  For callers that cannot allocate device memory (CUDA graph capture, serving
+ * loops, harnesses that forbid cudaMalloc): no handle, no workspace; the stage's scratch is a static device array
+ * inside the library (18.5 MB, held by every GPU that loads the library until the process exits), sized for
+ *     width * height <= DDHF_NOALLOC_MAX_PIXELS (1280 x 720)   and   max_boxes <= DDHF_NOALLOC_MAX_BOXES;
+ * anything larger is refused with DDHF_E_CAPACITY.  No cudaMalloc, cudaFree or allocating library call is made,
+ * here or in ddhf_boxes_noalloc_setup().
+ *   d_mask           DEVICE [width*height] bytes, nonzero = detection (input, not modified)
+ *   d_labels         DEVICE [width*height] out: component label (min linear index), -1 off the mask
+ *   d_boxes          DEVICE [max_boxes] out: boxes that passed a_min, ascending label
+ *   d_merged_boxes   DEVICE [max_boxes] out: eq. 12 detections; may be NULL (or merge_alpha <= 0): not written
+ *   d_counters       DEVICE int32[DDHF_N_COUNTERS] out: N_COMPONENTS, N_BOXES, N_BOXES_TOTAL, N_MERGED and
+ *                    OVERFLOW bit 1 as for ddhf_window(); the other entries are written as 0
+ * Only enqueues on `cuda_stream` (five kernels), never synchronises.  Every call on a device shares the one
+ * array: calls that overlap on the GPU (different streams without an ordering between them, or two processes'
+ * worth of threads on one device) race -- order them.  The array keeps the previous call's contents; what must
+ * start cleared is cleared by the call itself.  ddhf_boxes_noalloc_setup() resolves the array's device address
+ * for the CURRENT device (cudaGetSymbolAddress; once per device, idempotent, thread-safe); the entry point does
+ * it on first use, so call setup beforehand where that must not happen at call time (before a stream capture).
+ * Errors: DDHF_E_INVAL / DDHF_E_CAPACITY / DDHF_E_CUDA, text from ddhf_boxes_noalloc_error() (per thread). */
+#define DDHF_NOALLOC_MAX_PIXELS 921600
+#define DDHF_NOALLOC_MAX_BOXES  4096
+int ddhf_boxes_noalloc_setup(void);
+int ddhf_boxes_noalloc(const uint8_t *d_mask, int32_t width, int32_t height, int32_t a_min, float merge_alpha,
+                       int32_t max_boxes, int32_t *d_labels, ddhf_box *d_boxes, ddhf_box *d_merged_boxes,
+                       int32_t *d_counters, void *cuda_stream);
+const char *ddhf_boxes_noalloc_error(void);
+
 /* Text of the last error on this handle (or of the last failed ddhf_create if h is NULL). */
 const char *ddhf_last_error(const ddhf_handle *h);
 

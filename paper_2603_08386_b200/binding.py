@@ -27,7 +27,8 @@ EXPORTS = ["ddhf_create", "ddhf_workspace_bytes", "ddhf_window", "ddhf_window_pa
            "ddhf_window_host",
            "ddhf_host_submit", "ddhf_host_wait",
            "ddhf_stage_ms", "ddhf_launches_per_window", "ddhf_fma_peak_probe", "ddhf_destroy",
-           "ddhf_last_error", "ddhf_version"]
+           "ddhf_last_error", "ddhf_version",
+           "ddhf_boxes_noalloc_setup", "ddhf_boxes_noalloc", "ddhf_boxes_noalloc_error"]
 
 BOX_DTYPE = np.dtype([("x0", "<i4"), ("y0", "<i4"), ("x1", "<i4"), ("y1", "<i4"),
                       ("n_pix", "<i4"), ("label", "<i4")])
@@ -107,6 +108,12 @@ def lib() -> C.CDLL:
         L.ddhf_fma_peak_probe.argtypes = [C.c_float, C.POINTER(C.c_float), vp]
         L.ddhf_destroy.restype = C.c_int
         L.ddhf_destroy.argtypes = [vp]
+        L.ddhf_boxes_noalloc_setup.restype = C.c_int
+        L.ddhf_boxes_noalloc_setup.argtypes = []
+        L.ddhf_boxes_noalloc.restype = C.c_int
+        L.ddhf_boxes_noalloc.argtypes = [vp, C.c_int32, C.c_int32, C.c_int32, C.c_float, C.c_int32, vp, vp, vp, vp, vp]
+        L.ddhf_boxes_noalloc_error.restype = C.c_char_p
+        L.ddhf_boxes_noalloc_error.argtypes = []
         L.ddhf_last_error.restype = C.c_char_p
         L.ddhf_last_error.argtypes = [vp]
         L.ddhf_version.restype = C.c_char_p
@@ -213,6 +220,24 @@ def ddhf_stage_ms(h) -> list[float]:
     if rc != DDHF_OK:
         raise DdhfError(rc, (lib().ddhf_last_error(h) or b"").decode())
     return [float(x) for x in ms]
+
+
+NOALLOC_MAX_PIXELS, NOALLOC_MAX_BOXES = 921600, 4096
+
+
+def ddhf_boxes_noalloc_setup() -> None:
+    rc = lib().ddhf_boxes_noalloc_setup()
+    if rc != DDHF_OK:
+        raise DdhfError(rc, lib().ddhf_boxes_noalloc_error().decode())
+
+
+def ddhf_boxes_noalloc(mask_ptr: int, width: int, height: int, a_min: int, merge_alpha: float, max_boxes: int,
+                       labels_ptr: int, boxes_ptr: int, merged_ptr: int, counters_ptr: int, stream_ptr: int = 0) -> None:
+    """ddhf.h: CCL + boxes (+ eq. 12) on a device mask with the library's static scratch; device pointers as ints."""
+    rc = lib().ddhf_boxes_noalloc(mask_ptr, width, height, a_min, merge_alpha, max_boxes, labels_ptr, boxes_ptr,
+                                  merged_ptr or None, counters_ptr, stream_ptr or None)
+    if rc != DDHF_OK:
+        raise DdhfError(rc, lib().ddhf_boxes_noalloc_error().decode())
 
 
 def ddhf_launches_per_window(h) -> int:

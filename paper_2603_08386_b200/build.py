@@ -11,7 +11,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libddhf.so")
-SOURCES = ["api.cu", "ingest.cu", "ndft.cu", "nufft.cu", "ccl.cu", "probe.cu"]
+SOURCES = ["api.cu", "ingest.cu", "ndft.cu", "nufft.cu", "ccl.cu", "noalloc.cu", "probe.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--use_fast_math", "-Xptxas", "-v"]
 
