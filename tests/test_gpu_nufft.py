@@ -98,3 +98,47 @@ def test_nufft_config3_full_size_sampled(oracle):
     w = wl.make(3)
     gpu, wp, wsf, ws = _sampled_compare(oracle, w, w.params, w.events, 0, 400, score_all=False, nufft=True, nufft_min=48)
     print(f"nufft cfg3: worst power {wp:.2e}, SF {wsf:.2e}, score {ws:.2e}")
+
+
+def test_nufft_on_sliding_windows(oracle):
+    """ddhf_window_slide() with the NUFFT path on: the hot list is filled by the scan kernels of the sliding path.
+    Every window equals ddhf_window() on the same slice bit for bit (same kernels on the same rows) and the oracle
+    within the usual bars; one pixel is long enough to be split (> 4096 events: direct sum)."""
+    from paper_2603_08386_b200 import binding
+    W, H, T, hop = 40, 24, 100_000, 20_000
+    prm = _grid2048(W, H)
+    prm.update(n_min=4, a_min=1)
+    ev = wl.random_window(11, W, H, 150_000, 200_000, hot_fraction=0.6)      # hot 2 x 1 corner: rows of thousands of events
+    rng = np.random.default_rng(3)
+    hot = ev[rng.random(len(ev)) < 0.25].copy()
+    hot["x"], hot["y"] = 7, 5                                               # > 4096 events per window on one pixel
+    ev = np.concatenate([ev, hot])
+    ev = ev[np.argsort(ev["t"], kind="stable")]
+    kw = dict(max_events=len(ev), want_power=True, nufft=True, nufft_min=16, max_active=W * H)
+    det, ref = binding.Detector(prm, **kw), binding.Detector(prm, **kw)
+    d_ev = det.upload(ev)
+    t = ev["t"]
+    prev_hi = None
+    for k in range(6):
+        t0 = k * hop
+        lo, hi = int(np.searchsorted(t, t0, "left")), int(np.searchsorted(t, t0 + T, "left"))
+        if prev_hi is None:
+            det.slide(d_ev, hi - lo, t0, T, offset_events=lo)
+        else:
+            det.slide(d_ev, hi - prev_hi, t0, T, offset_events=prev_hi)
+        prev_hi = hi
+        g = det.results()
+        ref.window(d_ev, hi - lo, t0, T, offset_events=lo)
+        r = ref.results()
+        for key in ("row_ptr", "csr_ev", "active_idx", "power", "sf", "score", "f0_idx", "mask", "boxes"):
+            same = np.array_equal(g[key], r[key], equal_nan=True) if g[key].dtype.kind == "f" else np.array_equal(g[key], r[key])
+            assert same, (k, key)
+        if k in (0, 3):
+            orc = oracle.window(prm, ev[lo:hi], t0, T, score_all=False, want_power=True)
+            gu.check_csr(g, orc)
+            n = np.diff(orc["row_ptr"])[orc["active_idx"]]
+            assert (n > 4096).any() and ((n >= 16) & (n <= 4096)).sum() > 20
+            assert gu.power_error(g["power"], orc["power"]) <= gu.POWER_TOL
+            gu.check_maps(g, orc, prm, score_all=False, oracle_mod=oracle, orc_power=orc["power"])
+    det.close()
+    ref.close()
