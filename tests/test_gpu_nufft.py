@@ -142,3 +142,48 @@ def test_nufft_on_sliding_windows(oracle):
             gu.check_maps(g, orc, prm, score_all=False, oracle_mod=oracle, orc_power=orc["power"])
     det.close()
     ref.close()
+
+
+def _random_case(seed):
+    """A random configuration on which the NUFFT path applies: 1024 < n_freq <= 2048, df x window <= 0.24."""
+    rng = np.random.default_rng([2603, 8386, 4141, seed])
+    W, H = int(rng.integers(8, 120)), int(rng.integers(8, 90))
+    T = int(rng.choice([5_000, 20_000, 100_000]))
+    nf = int(rng.choice([1025, 1030, 1500, 2047, 2048]))
+    fmin = float(rng.choice([0.0, 0.0, 37.5]))
+    df = float(rng.uniform(0.05, 0.24)) / (T * 1e-6)
+    klo = int(rng.integers(0, 3)) if fmin == 0 else 0
+    d = int(rng.integers(0, 4))
+    n_harm = int(rng.integers(1, 7))
+    prm = dict(width=W, height=H, window_us=T, f_min_hz=fmin, df_hz=df, n_freq=nf, k_lo=klo,
+               f0_min_hz=fmin + (d + klo + 2 + float(rng.uniform(0, 40))) * df, f0_step_hz=float(rng.choice([0.5, 2.0, 7.0])) * df,
+               n_f0=int(rng.integers(1, 100)), n_harm=n_harm, half_bw_bins=d,
+               h_min=int(rng.integers(1, n_harm + 1)), n_min=int(rng.integers(3, 8)),
+               a_min=int(rng.integers(1, 12)), tau_sf=float(rng.uniform(0.3, 0.95)),
+               tau_comb=float(rng.uniform(1.5, 8.0)), sf_eps=1e-12, merge_alpha=float(rng.choice([0.0, 19.05])))
+    ev = wl.random_window(3000 + seed, W, H, int(rng.integers(2_000, 80_000)), T, hot_fraction=float(rng.choice([0.3, 0.8])),
+                          out_of_range=float(rng.choice([0.0, 0.05])), time_sorted=bool(rng.integers(0, 2)))
+    return prm, ev, T, bool(rng.integers(0, 2)), int(rng.choice([1, 8, 64]))
+
+
+@pytest.mark.parametrize("seed", range(8))
+def test_nufft_random_configuration(oracle, seed):
+    """Random grids (n_freq not a multiple of 32, f_min > 0, k_lo 0..2), sensors and event mixes, rows of >= 1 / 8 / 64
+    events through the NUFFT: every stage against the oracle with the bars of test_gpu_fuzz.py."""
+    from paper_2603_08386_b200 import binding
+    from test_gpu_fuzz import ILL_CAP
+    prm, ev, T, score_all, nmin = _random_case(seed)
+    try:
+        gpu = gu.run_gpu(prm, ev, 0, T, score_all=score_all, nufft=True, nufft_min=nmin)
+    except binding.DdhfError as e:
+        assert "band sorter" in str(e), str(e)
+        pytest.skip(str(e))
+    assert gpu["launches"] == (12 if prm["merge_alpha"] > 0 else 11)       # the NUFFT kernel did run
+    orc = oracle.window(prm, ev, 0, T, score_all=score_all)
+    gu.check_csr(gpu, orc)
+    assert gu.power_error(gpu["power"], orc["power"], gu.active_counts(orc)) <= gu.POWER_TOL
+    n_act = max(int(orc["n_active"]), 1)
+    gu.check_maps(gpu, orc, prm, score_all=score_all, oracle_mod=oracle, orc_power=orc["power"],
+                  allow_ill=True, max_ill=int(ILL_CAP[min(prm["n_min"], 3)] * n_act) + 2)
+    print(f"nufft seed {seed}: n_freq {prm['n_freq']}, rows >= {nmin}, {gu.last_counts}")
+    gu.check_boxes_against_oracle_ccl(gpu, oracle, prm["a_min"])
