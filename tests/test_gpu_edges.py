@@ -458,3 +458,37 @@ def test_giant_buckets_sorted_by_helper_ctas(oracle, window_us):
     assert np.array_equal(gpu["row_ptr"], row_ptr) and np.array_equal(gpu["csr_ev"], csr)
     cnt = np.diff(row_ptr)
     assert gpu["n_active"] == int((cnt >= 6).sum())
+
+
+@pytest.mark.parametrize("n_harm,d,max_scored", [(12, 12, 0), (12, 12, 50), (16, 15, 0), (16, 27, 0)])
+def test_wide_harmonic_windows_use_the_larger_band_sorters(oracle, n_harm, d, max_scored):
+    """Unions of harmonic windows of 300 / 496 / 880 of 2048 bins: the rank band of the complement medians needs the
+    512- and 1024-value band sorters (the BASELINE configs need 256).  Every active pixel scored, per-candidate values
+    compared; with a queue of 50 rows the 512-value variant also scores in place inside the NDFT kernel."""
+    W, H, T = 40, 24, 100_000
+    w1 = wl.make(1)
+    ev = wl.random_window(77, W, H, 25_000, T, hot_fraction=0.3)
+    # a periodic source on a few pixels so that some spectra have real harmonic structure
+    rng = np.random.default_rng(8)
+    tt = np.round(np.arange(0, T, 1e6 / 210.0)).astype(np.int64)
+    per = wl._pack(np.repeat([5, 6, 7], len(tt)), np.full(3 * len(tt), 9), np.ones(3 * len(tt), int), np.tile(tt, 3))
+    ev = np.concatenate([ev, per])
+    ev = ev[np.argsort(ev["t"], kind="stable")]
+    prm = dict(w1.params, width=W, height=H, f_min_hz=0.0, df_hz=5000.0 / 2048, n_freq=2048, k_lo=1, n_harm=n_harm,
+               half_bw_bins=d, h_min=4, n_min=4, f0_min_hz=100.0, f0_step_hz=2.5, n_f0=80, tau_sf=0.9, tau_comb=1.5, a_min=1)
+    orc = oracle.window(prm, ev, 0, T, score_all=True, want_power=True)
+    gpu = gu.run_gpu(prm, ev, 0, T, score_all=True, want_power=True, want_debug=True, max_scored=max_scored)
+    gu.check_csr(gpu, orc)
+    assert gpu["n_scored"] == orc["n_active"] > 400
+    assert gu.power_error(gpu["power"], orc["power"]) <= gu.POWER_TOL
+    gu.check_maps(gpu, orc, prm, score_all=True, oracle_mod=oracle, orc_power=orc["power"])
+    worst = 0.0
+    for r in range(0, gpu["n_active"], 7):
+        s, fi, snr, num, med = oracle.comb_score(orc["power"][r], prm)
+        dd = gpu["comb_debug"][r].astype(np.float64)
+        for k, ref in enumerate((snr, num, med)):
+            e = np.abs(dd[:, k] - ref) / np.maximum(np.abs(ref), 1e-30)
+            e[(ref == 0) & (dd[:, k] == 0)] = 0
+            worst = max(worst, e.max())
+    assert worst <= gu.REL_TOL, worst
+    print(f"H={n_harm} d={d} queue={max_scored or 'all'}: per-candidate worst rel err {worst:.2e}, {gu.last_counts}")
