@@ -14,7 +14,10 @@ pytestmark = pytest.mark.gpu
 
 N_SEEDS = int(os.environ.get("DDHF_FUZZ_SEEDS", "12"))
 #: largest share of the active pixels that may be ill-conditioned, by n_min (1, 2, >= 3)
-ILL_CAP = {1: 1.0, 2: 0.6, 3: 0.5}       # n_min >= 3: up to 44 % measured over 80 seeds (seed 16)
+# n_min 2: a pixel with exactly two events has exact spectral nulls (opposite polarities: the DC bin; equal ones: every
+# bin with f dt = 1/2 mod 1), and such pixels can be most of the active ones (seed 16: 302 of 360 active pixels hold two
+# events, 273 are ill-conditioned); n_min >= 3: up to 44 % measured over 80 seeds
+ILL_CAP = {1: 1.0, 2: 1.0, 3: 0.5}
 
 
 def _case(seed):
